@@ -1,0 +1,144 @@
+/*
+ * lbm.h -- C ABI of the B200-native particle-resolved thermal lattice Boltzmann hot path.
+ *
+ * Method: Xu & Li, "Particle-resolved thermal lattice Boltzmann simulation using OpenACC on
+ * multi-GPUs" (arXiv 2308.16597).  Citations below are PAPER.md:<line> (the paper text) and
+ * SURVEY.md section 8 (the scope contract: rows a1..a6, boundary (b), readings (c)).
+ *
+ * One handle = one simulation on one GPU.  All lattice state lives in ONE caller-supplied
+ * device workspace (PyTorch allocates it; the library never calls cudaMalloc inside lbm_step).
+ * Every array argument below is a HOST pointer unless it says "device".  Output buffers are
+ * caller-owned and caller-sized.  No exception crosses the boundary: every function that can
+ * fail returns an int (0 = LBM_OK, negative = error) and lbm_last_error() gives the text.
+ *
+ * Lattice conventions (SURVEY.md 8(c) "Lattice"; the paper does not print its numbering):
+ *   nodes (i,j), 0<=i<nx, 0<=j<ny, host arrays dense with x fastest: idx = j*nx + i
+ *   e0=(0,0) e1=(1,0) e2=(0,1) e3=(-1,0) e4=(0,-1) e5=(1,1) e6=(-1,1) e7=(-1,-1) e8=(1,-1)
+ *   D2Q5 (temperature) uses e0..e4.  Cavity walls lie half a spacing outside the outermost
+ *   nodes.  +y is up; gravity pulls particles along -y; hot fluid rises (Eq. 1b).
+ *   Everything is in lattice units, fp64.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LBM_OK            0
+#define LBM_E_ARG        (-1)  /* bad argument (NULL, non-positive size, overlap on insert ...)  */
+#define LBM_E_STATE      (-2)  /* call not legal in the handle's current state                   */
+#define LBM_E_CAPACITY   (-3)  /* a fixed-capacity array (particles, links, cells, newborn) full */
+#define LBM_E_CUDA       (-4)  /* a CUDA runtime call failed; lbm_last_error() has the string    */
+#define LBM_E_NONFINITE  (-5)  /* a particle state became NaN/Inf                                */
+
+typedef struct lbm lbm_t;
+
+/* Problem statement of the paper: closed cavity, Boussinesq fluid (Eqs. 1-6),
+ * circular particles with repulsion (Eq. 15). */
+typedef struct {
+  double nu, kappa;            /* kinematic viscosity, thermal diffusivity (kappa = nu/Pr)        */
+  double rho0, T0;             /* reference density, reference temperature (Eq. 1b)              */
+  double g;                    /* gravity magnitude; acts along -y on particles (Eq. 15's C too)  */
+  double gbeta;                /* g*beta_T: fluid buoyancy acceleration = +gbeta*(T-T0) along +y  */
+  double body_ax, body_ay;     /* extra uniform body acceleration (Poiseuille check); default 0    */
+  int    periodic_x;           /* 0 = closed cavity (all configs); 1 = x-periodic (closed-form checks) */
+  int    wall_T_type[4];       /* W,E,S,N: 0 adiabatic, 1 Dirichlet                              */
+  double wall_T[4];            /* W,E,S,N wall temperature (Dirichlet only)                      */
+  double rep_s, rep_eps;       /* Eq. (15): threshold distance s, stiffness eps_w                */
+  int    rep_power;            /* Eq. (15) exponent: 2 = paper, 1 = linear (BASELINE configs)     */
+  int    max_particles;        /* capacity of the particle arrays                                */
+  int    max_links_per_particle; /* capacity of one particle's segment of the fixed index array
+                                    (paper: 12N-12)                                */
+} lbm_params;
+
+/* Fills *p with: nu=0.02 kappa=0.02/0.7 rho0=1 T0=0 g=0 gbeta=0 body=0 periodic_x=0
+ * walls adiabatic, rep_s=2 rep_eps=1e-3 rep_power=1 max_particles=0 max_links_per_particle=0. */
+void lbm_params_default(lbm_params* p);
+
+/* Bytes of device workspace lbm_create needs for this lattice and these capacities
+ * (two copies of the 9+5 populations, flag and owner maps, particle/link/cell arrays).
+ * Returns 0 on bad arguments. */
+size_t lbm_workspace_bytes(int nx, int ny, const lbm_params* p);
+
+/* Creates a simulation.  dev_workspace: DEVICE pointer, >= lbm_workspace_bytes(), 256-byte
+ * aligned, owned by the caller and kept alive until lbm_destroy.  cuda_stream: a cudaStream_t
+ * (as void*; NULL = default stream) on which every kernel and copy of this handle is issued.
+ * Initial state (SURVEY 8(c) "Initial state"): f = f_eq(rho0, 0), g = g_eq(T0, 0), no particles.
+ * Errors: LBM_E_ARG (sizes, nu/kappa out of range: need nu>0, 0<kappa<0.144, nx,ny>=4),
+ * LBM_E_CAPACITY (workspace too small), LBM_E_CUDA. */
+int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t bytes,
+               void* cuda_stream, lbm_t** out);
+
+/* T_host: nx*ny doubles.  Sets g = g_eq(T, u=0) on every node (Eq. 17's equilibrium with u=0).
+ * Only before the first lbm_step (LBM_E_STATE afterwards). */
+int lbm_set_temperature(lbm_t* h, const double* T_host);
+
+/* Adds n circular particles (position, diameter, density, surface temperature).
+ * x,y: centres; diam: diameters; rho_ratio: rho_p/rho_f; T_w: surface temperature (Eq. 11, 17).
+ * ux,uy,omega: initial velocity (each may be NULL = at rest).  fixed: may be NULL; 1 = immobile
+ * (skips Eqs. 7-8; the momentum-exchange force is still computed).
+ * Errors: LBM_E_STATE after the first lbm_step (the paper never inserts particles mid-run);
+ * LBM_E_CAPACITY beyond max_particles or if 12N-12 exceeds max_links_per_particle;
+ * LBM_E_ARG if a disc is not strictly inside the cavity walls, overlaps another particle,
+ * or (periodic_x=1) its search zone would cross the periodic seam. */
+int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const double* diam,
+                      const double* rho_ratio, const double* T_w,
+                      const double* ux, const double* uy, const double* omega,
+                      const unsigned char* fixed);
+
+/* Advances nsteps time steps (each = rows a1..a6 of SURVEY 8(a); order PAPER.md:347-353):
+ * link build -> bounce-back (Eqs. 9-12) + momentum exchange (Eqs. 13-14) -> particle update
+ * (Eqs. 7, 8, 15) -> flag update -> fused pull-stream-collide (Eqs. 5, 6) -> refill (Eqs. 16-17).
+ * Asynchronous kernels on the handle's stream, then ONE stream synchronisation at the end of the
+ * call to read the device status word.  Errors: LBM_E_NONFINITE (a particle state is NaN/Inf,
+ * checked once per call), LBM_E_CAPACITY (a link segment, cell or the newborn list overflowed;
+ * the state is then undefined), LBM_E_CUDA. */
+int lbm_step(lbm_t* h, int nsteps);
+
+/* Readout.  Any pointer may be NULL = not wanted.
+ * rho, ux, uy, T: nx*ny doubles each; on fluid nodes rho = sum f, T = sum g,
+ *   u = (sum e f + F/2)/rho; on solid nodes rho0, rigid-body velocity, T_w.
+ * f: 9*nx*ny, g: 5*nx*ny doubles, population-major (f[k*nx*ny + j*nx + i]): the POST-collision
+ *   populations f+(x,t), g+(x,t) (right-hand sides of Eqs. 5, 6 before streaming) -- the quantity
+ *   Eqs. 9-13 consume and the state the fused kernel keeps resident.  Values on solid nodes are
+ *   unspecified (parity is taken on fluid nodes).
+ * flag: nx*ny bytes, 0 fluid, 1 solid. */
+int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T,
+                   double* f, double* g, unsigned char* flag);
+
+/* Particle state (r, U, theta, Omega_z; F, T_z of the last completed step).
+ * *n receives the particle count; arrays (each may be NULL) need that many entries. */
+int lbm_get_particles(lbm_t* h, int* n, double* x, double* y, double* theta,
+                      double* ux, double* uy, double* omega, double* Fx, double* Fy, double* Tz);
+
+/* Runs the link builder (row a2) on the CURRENT particle positions and returns
+ * the compacted fluid-particle links: fluid node (i,j), lattice direction alpha in 1..8 with
+ * (i,j)+e_alpha inside particle pid, and q.  In: *n = capacity of the arrays
+ * (arrays may be NULL if *n = 0).  Out: *n = number of links.  LBM_E_CAPACITY if too small
+ * (then *n = required).  Order: by particle, then the builder's scan order (callers sort). */
+int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, double* q);
+
+/* Per-kernel device timing with CUDA events on the handle's stream (used by bench.py for the
+ * roofline line).  on=1 starts recording around every kernel launch of lbm_step (events are
+ * pre-created; at most LBM_PROFILE_MAX_SAMPLES launches per kernel are sampled, the rest run
+ * untimed); on=0 stops.  lbm_profile_get: kernel ids 0..lbm_profile_kernels()-1; returns the
+ * summed duration in ms over the sampled launches and their number. */
+#define LBM_PROFILE_MAX_SAMPLES 512
+int lbm_profile_enable(lbm_t* h, int on);
+int lbm_profile_kernels(void);
+const char* lbm_profile_kernel_name(int kernel_id);
+int lbm_profile_get(lbm_t* h, int kernel_id, double* total_ms, long long* launches);
+
+/* Frees the handle (not the workspace).  NULL is a no-op. */
+int lbm_destroy(lbm_t* h);
+
+/* Text of the last error on this handle; with h = NULL, of the last failed lbm_create. */
+const char* lbm_last_error(const lbm_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

@@ -1,0 +1,250 @@
+"""Pins the oracle's particle part: link builder (brute force, Gauss circle count, 12N-12 bound),
+momentum exchange (rest state, zero lift on a symmetric fixed cylinder), repulsion and integrator
+inside the full step, refill sanity.  SURVEY.md 8(c) "Pins"."""
+import math
+
+import numpy as np
+import pytest
+
+EX = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1])
+EY = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1])
+
+
+def params(wl, n, dmax=20.0, **kw):
+    p = wl.default_params()
+    p.update(max_particles=n, max_links_per_particle=wl.max_links_for_diameter(dmax))
+    p.update(kw)
+    return p
+
+
+def sorted_links(L):
+    order = np.lexsort((L["i"], L["j"], L["alpha"], L["pid"]))
+    return {k: v[order] for k, v in L.items()}
+
+
+def numpy_links(nx, ny, xs, ys, rs):
+    """Independent enumeration (numpy, no oracle code): node solid iff dx*dx+dy*dy <= r*r for the
+    lowest-numbered covering particle."""
+    I, J = np.meshgrid(np.arange(nx, dtype=np.float64), np.arange(ny, dtype=np.float64))
+    owner = np.full((ny, nx), -1)
+    for p in reversed(range(len(xs))):
+        dx, dy = I - xs[p], J - ys[p]
+        owner[dx * dx + dy * dy <= rs[p] * rs[p]] = p
+    out = []
+    for a in range(1, 9):
+        for j in range(ny):
+            for i in range(nx):
+                if owner[j, i] >= 0:
+                    continue
+                bi, bj = i + EX[a], j + EY[a]
+                if 0 <= bi < nx and 0 <= bj < ny and owner[bj, bi] >= 0:
+                    out.append((owner[bj, bi], a, j, i))
+    return owner, sorted(out)
+
+
+def test_gauss_circle_and_link_count(ob, wl):
+    """r = 10 centred on a node: 317 solid nodes (Gauss circle problem, N(10) = 317) and 200 links,
+    84 of them along the axes (SURVEY 8(c) pin (ii), recounted here with numpy)."""
+    s = ob.OracleSim(40, 40, params(wl, 1))
+    s.add_particles(x=[20.0], y=[20.0], diam=[20.0], rho_ratio=[1.5], T_w=[1.0])
+    assert int(s.fields()["flag"].sum()) == 317
+    L = s.links()
+    owner, ref = numpy_links(40, 40, [20.0], [20.0], [10.0])
+    assert (owner >= 0).sum() == 317
+    assert len(L["q"]) == len(ref) == 200
+    assert int((L["alpha"] <= 4).sum()) == 84 and int((L["alpha"] >= 5).sum()) == 116
+    for a in range(1, 5):
+        assert int((L["alpha"] == a).sum()) == 21
+    for a in range(5, 9):
+        assert int((L["alpha"] == a).sum()) == 29
+    N = int(math.floor(30.0)) - int(math.floor(10.0)) + 3
+    assert N == 23 and len(L["q"]) <= 12 * N - 12 == 264
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+def test_zone_scan_equals_bruteforce_and_numpy(ob, wl, seed):
+    """Effective-zone scan == full-lattice scan == independent numpy enumeration,
+    for random real-valued centres and diameters, including particles close to the walls."""
+    rng = np.random.default_rng(seed)
+    nx, ny = 64, 56
+    w = wl.sedimentation(nx, ny, 6, seed=100 + seed, y_frac_lo=0.0, d_lo=6.0, d_hi=13.0)
+    P = w.particles
+    if seed == 3:   # hug the walls: gap below one lattice spacing
+        P["x"][0], P["y"][0] = 0.5 * P["diam"][0] - 0.3, 0.5 * P["diam"][0] - 0.4
+        P["x"][1], P["y"][1] = nx - 0.5 - 0.5 * P["diam"][1] - 0.05, 30.2
+        keep = [0, 1]
+        for k in range(2, 6):
+            if all(math.hypot(P["x"][k] - P["x"][m], P["y"][k] - P["y"][m]) >
+                   0.5 * (P["diam"][k] + P["diam"][m]) for m in keep):
+                keep.append(k)
+        P = {k: v[keep] for k, v in P.items()}
+    s = ob.OracleSim(nx, ny, params(wl, 6, 13.0))
+    s.add_particles(**P)
+    A, B = sorted_links(s.links()), sorted_links(s.links_bruteforce())
+    for k in ("pid", "i", "j", "alpha"):
+        assert np.array_equal(A[k], B[k])
+    assert np.array_equal(A["q"], B["q"])
+    owner, ref = numpy_links(nx, ny, P["x"], P["y"], 0.5 * P["diam"])
+    got = sorted(zip(A["pid"].tolist(), A["alpha"].tolist(), A["j"].tolist(), A["i"].tolist()))
+    assert got == [tuple(int(v) for v in r) for r in ref]
+    assert np.array_equal(s.fields()["flag"], (owner >= 0).astype(np.uint8))
+    # per-particle bound 12N-12 and the geometric meaning of q: x_f + q e lies on the circle
+    for p in range(len(P["x"])):
+        r = 0.5 * P["diam"][p]
+        N = int(math.floor(P["x"][p] + r)) - int(math.floor(P["x"][p] - r)) + 3
+        Ny = int(math.floor(P["y"][p] + r)) - int(math.floor(P["y"][p] - r)) + 3
+        assert int((A["pid"] == p).sum()) <= 12 * max(N, Ny) - 12
+    xw = A["i"] + A["q"] * EX[A["alpha"]] - P["x"][A["pid"]]
+    yw = A["j"] + A["q"] * EY[A["alpha"]] - P["y"][A["pid"]]
+    assert np.all((A["q"] >= 0) & (A["q"] <= 1))
+    assert np.abs(np.hypot(xw, yw) - 0.5 * P["diam"][A["pid"]]).max() < 1e-12
+    del rng
+
+
+def test_rest_state_is_a_fixed_point_with_zero_force(ob, wl):
+    """Fluid at rest, particle at rest, no gravity, T_w = T0 = wall T: nothing may change and
+    the momentum-exchange force vanishes (each lattice line enters and leaves the body once)."""
+    p = params(wl, 1, T0=0.5)
+    p["wall_T_type"] = [1, 1, 1, 1]
+    p["wall_T"] = [0.5] * 4
+    s = ob.OracleSim(36, 34, p)
+    s.add_particles(x=[17.3], y=[16.6], diam=[11.4], rho_ratio=[1.5], T_w=[0.5])
+    s.step(25)
+    F = s.fields()
+    fl = F["flag"] == 0
+    assert np.abs(F["rho"][fl] - 1).max() < 1e-14
+    assert np.abs(F["T"][fl] - 0.5).max() < 1e-14
+    assert np.abs(F["ux"]).max() < 1e-15 and np.abs(F["uy"]).max() < 1e-15
+    P = s.particles()
+    assert abs(P["Fx"][0]) < 1e-13 and abs(P["Fy"][0]) < 1e-13 and abs(P["Tz"][0]) < 1e-12
+    assert P["x"][0] == pytest.approx(17.3, abs=1e-12) and P["y"][0] == pytest.approx(16.6, abs=1e-12)
+
+
+def test_zero_lift_on_symmetric_fixed_cylinder(ob, wl):
+    """Fixed cylinder centred on the centreline node row of a body-force channel (periodic_x):
+    |F_y|/|F_x| < 1e-10 and T_z ~ 0 by mirror symmetry; the drag is positive (along the flow)."""
+    nx, ny = 60, 41
+    p = params(wl, 1, dmax=10.0, periodic_x=1, body_ax=2e-6, nu=0.1)
+    s = ob.OracleSim(nx, ny, p)
+    s.add_particles(x=[30.0], y=[20.0], diam=[10.0], rho_ratio=[1.5], T_w=[0.0], fixed=[1])
+    s.step(1200)
+    P = s.particles()
+    assert P["Fx"][0] > 1e-6
+    assert abs(P["Fy"][0]) / abs(P["Fx"][0]) < 1e-10
+    assert abs(P["Tz"][0]) / (abs(P["Fx"][0]) * 5.0) < 1e-10
+    assert P["x"][0] == 30.0 and P["ux"][0] == 0.0           # fixed
+    F = s.fields()
+    assert np.abs(F["ux"] - F["ux"][::-1]).max() < 1e-13      # mirror-symmetric flow
+    assert np.abs(F["uy"] + F["uy"][::-1]).max() < 1e-13
+    # steady momentum balance: body force on the fluid = drag on cylinder + wall friction, so the
+    # drag cannot exceed the total body force
+    assert P["Fx"][0] < 2e-6 * (F["flag"] == 0).sum()
+
+
+def test_repulsion_and_gravity_enter_the_first_step_in_closed_form(ob, wl):
+    """At t = 0 the fluid is at rest, so F_hydro = 0 and U(1) = (weight + Eq. 15)/M exactly:
+    pair at gap 1.5 (s = 2, p = 1 -> a quarter of C/eps) and a particle at gap 1.5 from the bottom
+    wall.  (Gaps are chosen so that fluid nodes remain between the surfaces: with none, the
+    momentum-exchange sum loses the links of that side and F_hydro != 0 even at rest.)"""
+    g, ratio, r = 1.6e-4, 1.5, 4.75
+    p = params(wl, 3, dmax=10.0, g=g, rep_s=2.0, rep_eps=1e-3, rep_power=1)
+    s = ob.OracleSim(64, 48, p)
+    s.add_particles(x=[20.0, 31.0, 50.0], y=[30.0, 30.0, r + 1.0], diam=[2 * r] * 3,
+                    rho_ratio=[ratio] * 3, T_w=[0.0] * 3)
+    s.step(1)
+    P = s.particles()
+    area = math.pi * r * r
+    C = area * (ratio - 1) * g
+    M = ratio * area
+    a_g = -(ratio - 1) * area * g / M
+    a_pair = (C / 1e-3) * (2.0 - 1.5) / 2.0 / M
+    assert np.allclose([P["Fx"][0], P["Fy"][0]], 0, atol=1e-13)
+    assert P["ux"][0] == pytest.approx(-a_pair, rel=1e-12)
+    assert P["ux"][1] == pytest.approx(+a_pair, rel=1e-12)
+    assert P["uy"][0] == pytest.approx(a_g, rel=1e-10) and P["uy"][1] == pytest.approx(a_g, rel=1e-10)
+    a_wall = (C / 1e-3) * (2.0 - 1.5) / 2.0 / M
+    assert P["uy"][2] == pytest.approx(a_g + a_wall, rel=1e-12)
+    assert P["ux"][2] == pytest.approx(0.0, abs=1e-15)
+    assert P["x"][0] == pytest.approx(20.0 - 0.5 * a_pair, rel=1e-14)   # trapezoid position update
+    # quadratic variant of the paper (p = 2, s = 3): quarter of C/eps at half the range
+    p2 = params(wl, 2, dmax=10.0, g=g, rep_s=3.0, rep_eps=1e-3, rep_power=2)
+    s2 = ob.OracleSim(64, 48, p2)
+    s2.add_particles(x=[20.0, 31.0], y=[30.0, 30.0], diam=[2 * r] * 2, rho_ratio=[ratio] * 2, T_w=[0.0] * 2)
+    s2.step(1)
+    assert s2.particles()["ux"][1] == pytest.approx((C / 1e-3) * 0.25 / M, rel=1e-12)
+
+
+def test_argument_and_state_errors(ob, wl):
+    p = params(wl, 2)
+    s = ob.OracleSim(64, 64, p)
+    with pytest.raises(ob.OracleError) as e:
+        s.add_particles(x=[5.0], y=[30.0], diam=[20.0], rho_ratio=[1.5], T_w=[1.0])   # through W wall
+    assert e.value.code == -1
+    with pytest.raises(ob.OracleError) as e:
+        s.add_particles(x=[20.0, 30.0], y=[30.0, 30.0], diam=[20.0, 20.0], rho_ratio=[1.5] * 2, T_w=[1.0] * 2)
+    assert e.value.code == -1                                                            # overlap
+    with pytest.raises(ob.OracleError) as e:
+        s.add_particles(x=[20.0] * 3, y=[30.0] * 3, diam=[4.0] * 3, rho_ratio=[1.5] * 3, T_w=[1.0] * 3)
+    assert e.value.code == -3                                                            # capacity
+    s.add_particles(x=[20.0], y=[30.0], diam=[20.0], rho_ratio=[1.5], T_w=[1.0])
+    s.step(1)
+    with pytest.raises(ob.OracleError) as e:
+        s.add_particles(x=[45.0], y=[30.0], diam=[10.0], rho_ratio=[1.5], T_w=[1.0])
+    assert e.value.code == -2
+    p3 = params(wl, 1)
+    p3["max_links_per_particle"] = 100
+    s3 = ob.OracleSim(64, 64, p3)
+    with pytest.raises(ob.OracleError) as e:
+        s3.add_particles(x=[20.0], y=[30.0], diam=[20.0], rho_ratio=[1.5], T_w=[1.0])
+    assert e.value.code == -3
+
+
+def test_moving_particle_refill_keeps_fields_sane(ob, wl):
+    """A particle launched at |U| = 0.06 crosses ~5 lattice rows in 100 steps, so many nodes are
+    covered and uncovered (Eqs. 16-17).  Fields stay finite and bounded, the solid-node count stays
+    that of a radius-6 disc (113 +- a few), and the hot wake stays within [T0, T_w] (+-5 %)."""
+    p = params(wl, 1, dmax=12.0, g=0.0, gbeta=0.0)
+    p["wall_T_type"] = [1, 1, 1, 1]
+    s = ob.OracleSim(48, 64, p)
+    s.add_particles(x=[24.3], y=[44.2], diam=[12.0], rho_ratio=[4.0], T_w=[1.0], ux=[0.01], uy=[-0.06],
+                    omega=[0.002])
+    y_prev = 44.2
+    for _ in range(5):
+        s.step(20)
+        F = s.fields()
+        fl = F["flag"] == 0
+        assert np.isfinite(F["rho"]).all() and np.isfinite(F["T"]).all()
+        assert np.abs(F["rho"][fl] - 1).max() < 0.08
+        assert F["T"][fl].min() > -0.05 and F["T"][fl].max() < 1.05
+        assert abs(int(F["flag"].sum()) - 113) <= 6
+        y = s.particles()["y"][0]
+        assert y < y_prev
+        y_prev = y
+    assert 44.2 - y_prev > 3.0
+    # fluid next to the particle is dragged along: downward velocity just below it
+    P = s.particles()
+    j, i = int(round(P["y"][0] - 8)), int(round(P["x"][0]))
+    assert s.fields()["uy"][j, i] < -0.005
+
+
+def test_config0_physical_sanity(ob, wl):
+    """Config 0 (single hot particle): accelerates downward, stays below the reference velocity
+    U_ref = sqrt(g pi d (rho_p/rho_f - 1)/2), stays on the axis, heats the fluid."""
+    w = wl.config(0)
+    s = ob.OracleSim.from_workload(w)
+    v = []
+    for _ in range(3):
+        s.step(100)
+        v.append(s.particles()["uy"][0])
+    Uref = math.sqrt(w.params["g"] * math.pi * 20 * 0.5 / 2)
+    assert Uref == pytest.approx(0.050, abs=0.001)
+    assert v[0] < 0 and v[1] < v[0] and v[2] < v[1]
+    assert abs(v[2]) < Uref
+    P = s.particles()
+    # (64, 200) is half a spacing off the box axis x = 63.5, so a tiny lateral drift is physical
+    assert abs(P["x"][0] - 64.0) < 1e-2 and abs(P["omega"][0]) < 1e-4
+    F = s.fields()
+    fl = F["flag"] == 0
+    assert F["T"][fl].max() > 0.5 and F["T"][fl].min() > -0.02
+    jc, ic = int(round(P["y"][0])), 64
+    assert F["T"][jc + 13, ic] > F["T"][jc - 13, ic]                # the warm wake trails above
