@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS of the particle-resolved thermal LBM hot path on B200 (one JSON line).
+
+A "step" is one time step of the whole hot path (rows a1-a6 of SURVEY.md 8(a): link build,
+bounce-back + momentum exchange, particle update, flag update, fused stream-collide, refill) on
+the workload BASELINE.json's metric is quoted on: config 3, 4000 x 4000 fp64 D2Q9+D2Q5 with 4,800
+hot particles (seeded synthetic placement, paper_2308_16597_b200/workloads.py).
+
+  value  MLUPS = nx*ny*K / seconds (Eq. 18), state resident in HBM, CUDA events
+         around ONE lbm_step(K) call on the library's stream, max over ranks
+  e2e    the same metric for a whole job through the public API with HOST buffers: lbm_create ->
+         lbm_set_temperature(host T) -> lbm_add_particles(host arrays) -> lbm_step(K) ->
+         lbm_get_fields(rho, ux, uy, T to pinned host) + lbm_get_particles, all inside the timed
+         region (an LBM state lives on the device between steps, so the host copies of a job are
+         its set-up and its read-out; bytes are reported per step = job bytes / K)
+  roofline      fused stream-collide kernel: algorithmic bytes / its mean CUDA-event duration
+  cpu_baseline  the CPU oracle as it stands, timed on this host on a bounded sample
+
+N > 1 (torchrun): the path does not shard in this build:
+every rank runs an independent replica of the workload, no data-path collective; value = all
+ranks' lattice updates / max-over-ranks time ("weak").
+
+--impl reference: times the oracle (single thread, host cores) on a bounded sample of the same
+workload; the ratio against it is not a headline (it is a deliberately slow checker).
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "MLUPS (fp64 D2Q9+D2Q5 with particles, 1 B200) and % of HBM roofline"
+BYTES_PER_LU = 2 * (9 + 5) * 8     # one read + one write of every population
+FLAG_BYTES = 1
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=200)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[k] (default 3)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--profile-steps", type=int, default=200)
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi samples DURING the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        inside = [l for (t, l) in self.lines if t0 <= t <= t1 + 0.1] or [l for _, l in self.lines]
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in inside:
+            c = [x.strip() for x in l.split(",")]
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); power.append(float(c[2]))
+            except (ValueError, IndexError):
+                continue
+            for nme, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------- oracle (CPU) legs
+def oracle_sample_workload(wl, cfg, edge):
+    """A bounded sample of config `cfg`: an edge x edge lattice with the same particle number
+    density, diameters, density ratio, temperatures, physics and placement recipe."""
+    full = wl.config(cfg) if cfg in (0, 1) else None
+    if cfg == 0:
+        return full
+    if cfg == 1:
+        import numpy as np
+        rng = np.random.default_rng(1)
+        j = np.arange(edge, dtype=np.float64)[:, None]
+        T = (1.0 - (j + 0.5) / edge) + 1e-3 * rng.uniform(-1.0, 1.0, size=(edge, edge))
+        return wl.Workload("config1_sample", edge, edge, full.params, 1, 1, T_init=T)
+    spec = {2: (1000, 480, 0.4, 20.0, 20.0), 3: (4000, 4800, 0.3, 20.0, 20.0),
+            4: (8192, 20000, 0.0, 12.0, 24.0)}[cfg]
+    n_full, np_full, yfrac, dlo, dhi = spec
+    npart = max(1, int(round(np_full * (edge / n_full) ** 2)))
+    return wl.sedimentation(edge, edge, npart, seed=cfg, y_frac_lo=yfrac, d_lo=dlo, d_hi=dhi,
+                            name=f"config{cfg}_sample_{edge}")
+
+
+def time_oracle(wl, cfg, edge, steps, warmup):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle_binding as ob
+    w = oracle_sample_workload(wl, cfg, edge)
+    o = ob.OracleSim.from_workload(w)
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return w, w.nx * w.ny * steps / dt / 1e6, dt
+
+
+def run_reference(args, wl):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    total = args.steps + args.warmup
+    # size the sample so that the whole run ends within ~2 minutes at ~1.5 MLUPS (measured)
+    edge = int(math.sqrt(max(1.0, 120.0 * 1.5e6 / max(total, 1))))
+    edge = max(96, min(1000, edge))
+    w, val, dt = time_oracle(wl, args.config, edge, args.steps, args.warmup)
+    sample = (f"{w.nx}x{w.ny} sample of config {args.config} ({w.n_particles} particles, same "
+              f"density/diameters/physics/placement recipe), {args.steps} steps after "
+              f"{args.warmup} warm-up, single thread")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "MLUPS",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config{args.config}", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "MLUPS", "cores": 1, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": "MLUPS", "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------- our arm
+def main():
+    args = parse_args()
+    from paper_2308_16597_b200 import workloads as wl
+    if args.impl == "reference":
+        run_reference(args, wl)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2308_16597_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, W = args.steps, max(args.warmup, 3)
+    w = wl.config(args.config)
+    n = w.nx * w.ny
+    stream = torch.cuda.current_stream(dev)
+
+    # ---------------- device-resident timing: value
+    sim = binding.Simulation.from_workload(w, device=dev)
+    sim.step(W)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    vis = [v for v in os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",") if v.strip()]
+    clocks = ClockSampler(vis[local] if local < len(vis) else local)
+    clocks.start()
+    time.sleep(0.3)
+    barrier()
+    l0 = sim.kernel_launches()
+    t0 = time.perf_counter()
+    ev0.record(stream)
+    sim.step(K)                      # K time steps, one stream synchronisation at the end
+    ev1.record(stream)
+    barrier()
+    t1 = time.perf_counter()
+    launches = sim.kernel_launches() - l0
+    ms = ev0.elapsed_time(ev1)
+    clk = clocks.stop(t0, t1)
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max = float(tmax.item())
+    value = world * n * K / (ms_max * 1e-3) / 1e6
+
+    # ---------------- per-kernel CUDA-event durations (separate pass) -> roofline
+    P = min(args.profile_steps, 512)
+    sim.profile(True)
+    sim.step(P)
+    prof = sim.profile_results()
+    sim.profile(False)
+    flag = sim.fields()["flag"]
+    n_fluid = int((flag == 0).sum())
+    sc_ms, sc_n = prof["stream_collide"]
+    step_ms_prof = sum(v[0] for k, v in prof.items() if k != "init_collide") / max(P, 1)
+    sc_avg_s = sc_ms / max(sc_n, 1) * 1e-3
+    alg_bytes = BYTES_PER_LU * n_fluid + FLAG_BYTES * n      # per launch, DESIGN.md "Roofline"
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    else:
+        peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+    achieved = alg_bytes / sc_avg_s / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_stream_collide", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": read_traffic(),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                "avg_launch_ms": sc_avg_s * 1e3, "launches_timed": sc_n,
+                "share_of_step": (sc_ms / max(sc_n, 1)) / step_ms_prof if step_ms_prof else None,
+                "kernel_ms_per_step": {k: v[0] / max(v[1], 1) for k, v in prof.items() if v[1]},
+                "whole_step_frac_of_hbm_roofline": value / world / (peak * 1e9 / BYTES_PER_LU / 1e6),
+                "fluid_fraction": n_fluid / n}
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+
+    # ---------------- end to end through the public API with host buffers
+    e2e = None
+    if not args.no_e2e:
+        T_host = torch.empty((w.ny, w.nx), dtype=torch.float64).pin_memory()
+        if w.T_init is not None:
+            T_host.copy_(torch.from_numpy(np.ascontiguousarray(w.T_init)))
+        else:
+            T_host.fill_(w.params["T0"])
+        outs = {k: torch.empty(n, dtype=torch.float64).pin_memory() for k in ("rho", "ux", "uy", "T")}
+        h2d = T_host.numel() * 8
+        if w.particles is not None:
+            h2d += sum(int(np.asarray(v).nbytes) for v in w.particles.values())
+        barrier()
+        te0 = time.perf_counter()
+        s2 = binding.Simulation(w.nx, w.ny, w.params, device=dev)
+        s2.set_temperature(T_host)
+        if w.particles is not None:
+            s2.add_particles(**w.particles)
+        s2.step(K)
+        res = s2.fields(out=outs)
+        pr = s2.particles()
+        barrier()
+        te = time.perf_counter() - te0
+        d2h = 4 * n * 8 + n + sum(int(v.nbytes) for v in pr.values())
+        tt = torch.tensor([te], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        assert np.isfinite(res["rho"]).all()
+        e2e = {"value": world * n * K / float(tt.item()) / 1e6, "unit": "MLUPS",
+               "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+               "job": "create + set_temperature(host) + add_particles(host) + step(K) + "
+                      "get_fields(rho,ux,uy,T,flag -> pinned host) + get_particles",
+               "job_seconds": float(tt.item())}
+        s2.close()
+
+    # ---------------- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        edge = 600 if args.config >= 2 else (512 if args.config == 1 else 0)
+        steps_cpu = 60 if args.config >= 1 else 400
+        wc, v, dt = time_oracle(wl, args.config, edge, steps_cpu, 1)
+        cpu = {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle",
+               "sample": f"{wc.nx}x{wc.ny} sample of config {args.config} ({wc.n_particles} "
+                         f"particles, same recipe), {steps_cpu} steps, {dt:.1f} s, single thread "
+                         f"of {os.cpu_count()} host cores"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "particles": w.n_particles,
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "l2": f"inputs larger than L2: {2 * 14 * 8 * n / 1e6:.0f} MB of "
+                                 "populations stream through per step (126 MB L2)"
+                                 if 2 * 14 * 8 * n > 126e6 * 2 else "working set fits L2: not an HBM-bound configuration",
+                           "seed": "numpy default_rng(config index)"},
+                "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "cpu_baseline": cpu,
+                "context": {"paper_single_gpu_mlups": 1750, "paper_hardware": "1x A100, OpenACC "
+                            "(PAPER.md:271-281; d=40, Pr=5 workload: context, not like-for-like)"}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def read_traffic():
+    """dram bytes (read + write) per k_stream_collide launch from the committed ncu --set full
+    capture, or None: profiles/traffic.csv, rows `kernel,dram_bytes_per_launch` (see the .md
+    beside it for the command)."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for row in open(p):
+            c = row.strip().split(",")
+            if c[0] == "k_stream_collide":
+                return float(c[1])
+    except (OSError, ValueError, IndexError):
+        pass
+    return None
+
+
+if __name__ == "__main__":
+    main()

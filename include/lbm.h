@@ -132,6 +132,11 @@ int lbm_profile_kernels(void);
 const char* lbm_profile_kernel_name(int kernel_id);
 int lbm_profile_get(lbm_t* h, int kernel_id, double* total_ms, long long* launches);
 
+/* Number of CUDA kernels this handle has launched since lbm_create (set-up, step and read-out
+ * kernels; memsets and copies are not counted).  bench.py reports the difference across its
+ * timed region as "gpu_launches".  Returns -1 for a NULL handle. */
+long long lbm_kernel_launches(const lbm_t* h);
+
 /* Frees the handle (not the workspace).  NULL is a no-op. */
 int lbm_destroy(lbm_t* h);
 

@@ -1,0 +1,240 @@
+"""Thin ctypes binding over the C ABI of include/lbm.h (argument marshalling only).
+
+PyTorch supplies the device workspace (one uint8 tensor) and the CUDA stream; every step of the
+hot path runs in the library's own sm_100a kernels.  There is NO CPU fallback: if the shared
+library is missing or no CUDA device is present, constructing a `Simulation` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+_bp = C.POINTER(C.c_ubyte)
+
+LBM_OK, LBM_E_ARG, LBM_E_STATE, LBM_E_CAPACITY, LBM_E_CUDA, LBM_E_NONFINITE = 0, -1, -2, -3, -4, -5
+
+
+class LbmParams(C.Structure):
+    """Mirror of `lbm_params` in include/lbm.h."""
+    _fields_ = [("nu", C.c_double), ("kappa", C.c_double), ("rho0", C.c_double),
+                ("T0", C.c_double), ("g", C.c_double), ("gbeta", C.c_double),
+                ("body_ax", C.c_double), ("body_ay", C.c_double), ("periodic_x", C.c_int),
+                ("wall_T_type", C.c_int * 4), ("wall_T", C.c_double * 4),
+                ("rep_s", C.c_double), ("rep_eps", C.c_double), ("rep_power", C.c_int),
+                ("max_particles", C.c_int), ("max_links_per_particle", C.c_int)]
+
+    @classmethod
+    def from_dict(cls, d):
+        p = cls()
+        for k, _ in cls._fields_:
+            v = d[k]
+            if k == "wall_T_type":
+                p.wall_T_type = (C.c_int * 4)(*[int(t) for t in v])
+            elif k == "wall_T":
+                p.wall_T = (C.c_double * 4)(*[float(t) for t in v])
+            else:
+                setattr(p, k, v)
+        return p
+
+
+class LbmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"lbm error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the C-ABI library and declare its signatures.  Raises if it has not been built
+    (`python -m paper_2308_16597_b200.build` or `__graft_entry__.build()`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build the CUDA library first "
+                           "(python paper_2308_16597_b200/build.py); there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, sz, ll = C.c_void_p, C.c_size_t, C.c_longlong
+    P = C.POINTER(LbmParams)
+    L.lbm_params_default.argtypes = [P]
+    L.lbm_params_default.restype = None
+    L.lbm_workspace_bytes.argtypes = [C.c_int, C.c_int, P]
+    L.lbm_workspace_bytes.restype = sz
+    L.lbm_create.argtypes = [C.c_int, C.c_int, P, vp, sz, vp, C.POINTER(vp)]
+    L.lbm_set_temperature.argtypes = [vp, _dp]
+    L.lbm_add_particles.argtypes = [vp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
+    L.lbm_step.argtypes = [vp, C.c_int]
+    L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
+    L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
+    L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
+    L.lbm_profile_enable.argtypes = [vp, C.c_int]
+    L.lbm_profile_kernels.argtypes = []
+    L.lbm_profile_kernel_name.argtypes = [C.c_int]
+    L.lbm_profile_kernel_name.restype = C.c_char_p
+    L.lbm_profile_get.argtypes = [vp, C.c_int, _dp, C.POINTER(ll)]
+    L.lbm_kernel_launches.argtypes = [vp]
+    L.lbm_kernel_launches.restype = ll
+    L.lbm_destroy.argtypes = [vp]
+    L.lbm_last_error.argtypes = [vp]
+    L.lbm_last_error.restype = C.c_char_p
+    for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_step",
+                 "lbm_get_fields", "lbm_get_particles", "lbm_get_links", "lbm_profile_enable",
+                 "lbm_profile_kernels", "lbm_profile_get", "lbm_destroy"):
+        getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _host(a, pinned_ok=True):
+    """numpy view of a host buffer (numpy array or CPU torch tensor, e.g. pinned)."""
+    if a is None:
+        return None
+    if hasattr(a, "numpy") and not isinstance(a, np.ndarray):
+        a = a.numpy()
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class Simulation:
+    """One particle-resolved thermal LBM simulation on one B200 (calls follow include/lbm.h)."""
+
+    def __init__(self, nx, ny, params, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the lattice Boltzmann hot path has no CPU fallback")
+        self._torch = torch
+        self._L = load_library()
+        self.nx, self.ny, self.n = int(nx), int(ny), int(nx) * int(ny)
+        self.params = dict(params)
+        self._P = LbmParams.from_dict(params)
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        nbytes = self._L.lbm_workspace_bytes(self.nx, self.ny, C.byref(self._P))
+        if nbytes == 0:
+            raise LbmError(LBM_E_ARG, "lbm_workspace_bytes: bad size or parameter")
+        self.workspace_bytes = int(nbytes)
+        self._ws = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=self.device)
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._h = C.c_void_p()
+        rc = self._L.lbm_create(self.nx, self.ny, C.byref(self._P), C.c_void_p(base),
+                                C.c_size_t(int(nbytes)), C.c_void_p(self.stream.cuda_stream),
+                                C.byref(self._h))
+        if rc:
+            raise LbmError(rc, self._L.lbm_last_error(None).decode())
+
+    @classmethod
+    def from_workload(cls, w, **kw):
+        sim = cls(w.nx, w.ny, w.params, **kw)
+        if w.T_init is not None:
+            sim.set_temperature(w.T_init)
+        if w.particles is not None:
+            sim.add_particles(**w.particles)
+        return sim
+
+    def _chk(self, rc):
+        if rc:
+            raise LbmError(rc, self._L.lbm_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h:
+            self._L.lbm_destroy(self._h)
+            self._h = C.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- set-up ----
+    def set_temperature(self, T):
+        T = _host(T).reshape(-1)
+        assert T.size == self.n
+        self._chk(self._L.lbm_set_temperature(self._h, _d(T)))
+
+    def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None):
+        x, y, diam, rho_ratio, T_w, ux, uy, omega = map(_host, (x, y, diam, rho_ratio, T_w, ux, uy, omega))
+        fx = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.uint8)
+        self._chk(self._L.lbm_add_particles(
+            self._h, int(x.size), _d(x), _d(y), _d(diam), _d(rho_ratio), _d(T_w), _d(ux), _d(uy),
+            _d(omega), None if fx is None else fx.ctypes.data_as(_bp)))
+
+    # ---- the hot path ----
+    def step(self, nsteps=1):
+        self._chk(self._L.lbm_step(self._h, int(nsteps)))
+
+    # ---- read-out ----
+    def fields(self, populations=False, out=None):
+        """dict of (ny, nx) arrays rho, ux, uy, T, flag (+ f (9,ny,nx), g (5,ny,nx) post-collision).
+        `out` may supply preallocated host buffers (e.g. pinned torch tensors) by the same keys."""
+        n = self.n
+        out = out or {}
+        bufs = {}
+        for k in ("rho", "ux", "uy", "T"):
+            b = out.get(k)
+            bufs[k] = (b.numpy() if hasattr(b, "numpy") and not isinstance(b, np.ndarray) else b) \
+                if b is not None else np.empty(n, dtype=np.float64)
+        f = np.empty(9 * n, dtype=np.float64) if populations else None
+        g = np.empty(5 * n, dtype=np.float64) if populations else None
+        flag = np.empty(n, dtype=np.uint8)
+        self._chk(self._L.lbm_get_fields(self._h, _d(bufs["rho"]), _d(bufs["ux"]), _d(bufs["uy"]),
+                                         _d(bufs["T"]), _d(f), _d(g), flag.ctypes.data_as(_bp)))
+        res = {k: v.reshape(self.ny, self.nx) for k, v in bufs.items()}
+        res["flag"] = flag.reshape(self.ny, self.nx)
+        if populations:
+            res["f"] = f.reshape(9, self.ny, self.nx)
+            res["g"] = g.reshape(5, self.ny, self.nx)
+        return res
+
+    def particles(self):
+        n = C.c_int()
+        self._chk(self._L.lbm_get_particles(self._h, C.byref(n), *([None] * 9)))
+        names = ("x", "y", "theta", "ux", "uy", "omega", "Fx", "Fy", "Tz")
+        out = {k: np.empty(n.value, dtype=np.float64) for k in names}
+        if n.value:
+            self._chk(self._L.lbm_get_particles(self._h, C.byref(n), *[_d(out[k]) for k in names]))
+        return out
+
+    def links(self):
+        n = C.c_longlong(0)
+        rc = self._L.lbm_get_links(self._h, C.byref(n), None, None, None, None, None)
+        if rc not in (LBM_OK, LBM_E_CAPACITY):
+            self._chk(rc)
+        m = n.value
+        pid, i, j, al = (np.empty(m, dtype=np.int32) for _ in range(4))
+        q = np.empty(m, dtype=np.float64)
+        n = C.c_longlong(m)
+        self._chk(self._L.lbm_get_links(self._h, C.byref(n), pid.ctypes.data_as(_ip),
+                                        i.ctypes.data_as(_ip), j.ctypes.data_as(_ip),
+                                        al.ctypes.data_as(_ip), _d(q)))
+        return dict(pid=pid, i=i, j=j, alpha=al, q=q)
+
+    # ---- profiling ----
+    def kernel_launches(self):
+        return int(self._L.lbm_kernel_launches(self._h))
+
+    def profile(self, on=True):
+        self._chk(self._L.lbm_profile_enable(self._h, 1 if on else 0))
+
+    def profile_results(self):
+        """{kernel name: (total ms over the sampled launches, number of sampled launches)}"""
+        out = {}
+        for k in range(self._L.lbm_profile_kernels()):
+            ms, cnt = C.c_double(), C.c_longlong()
+            self._chk(self._L.lbm_profile_get(self._h, k, C.byref(ms), C.byref(cnt)))
+            out[self._L.lbm_profile_kernel_name(k).decode()] = (ms.value, cnt.value)
+        return out

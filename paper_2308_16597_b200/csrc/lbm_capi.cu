@@ -1,0 +1,573 @@
+// lbm_capi.cu -- the C ABI of include/lbm.h: workspace carving, host-side validation, the per-step
+// launch sequence (SURVEY.md 3 / 7 "legal fused ordering"), read-out copies and event profiling.
+// No torch types, no exceptions across the boundary, no cudaMalloc of lattice state: everything
+// lives in the caller's workspace (only the pinned status word and the events are ours).
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <utility>
+#include <vector>
+
+#include "lbm_internal.cuh"
+
+namespace {
+
+char g_create_error[512] = "";
+
+const char* const kKernelNames[K_COUNT] = {
+    "stream_collide", "build_links", "bounce_back_force", "cells_integrate",
+    "flags_uncover", "flags_cover", "refill", "init_collide"};
+
+int fail(lbm* h, int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(h ? h->err : g_create_error, 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_OK(h, call)                                                              \
+  do {                                                                                \
+    cudaError_t e_ = (call);                                                          \
+    if (e_ != cudaSuccess)                                                            \
+      return fail(h, LBM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_));            \
+  } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Lays the arrays out in the workspace.  With base == nullptr only the size is computed.
+struct Carver {
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <typename T>
+  T* take(size_t count) {
+    off = align_up(off, 256);
+    T* p = base ? (T*)(base + off) : nullptr;
+    off += sizeof(T) * count;
+    return p;
+  }
+};
+
+struct Layout {
+  int px;
+  long long ps;
+  int max_cells, mcx, mcy;
+  int newborn_cap;
+};
+
+Layout layout_of(int nx, int ny, const lbm_params* p) {
+  Layout L;
+  L.px = (int)align_up((size_t)nx, 16);
+  L.ps = (long long)align_up((size_t)L.px * ny, 32);
+  L.mcx = (int)std::ceil(nx / MIN_CELL) + 1;
+  L.mcy = (int)std::ceil(ny / MIN_CELL) + 1;
+  L.max_cells = p->max_particles > 0 ? L.mcx * L.mcy : 0;
+  L.newborn_cap = p->max_particles * NEWBORN_PER_PARTICLE;
+  return L;
+}
+
+size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
+  const Layout L = layout_of(nx, ny, p);
+  Carver c(base);
+  const size_t np = (size_t)p->max_particles;
+  double* A = c.take<double>(14 * (size_t)L.ps);
+  double* B = c.take<double>(14 * (size_t)L.ps);
+  unsigned char* flag = c.take<unsigned char>((size_t)L.px * ny);
+  int* owner = c.take<int>((size_t)L.px * ny);
+  ParticleArrays pa;
+  for (int b = 0; b < 2; ++b) {
+    pa.x[b] = c.take<double>(np);
+    pa.y[b] = c.take<double>(np);
+    pa.theta[b] = c.take<double>(np);
+    pa.ux[b] = c.take<double>(np);
+    pa.uy[b] = c.take<double>(np);
+    pa.omega[b] = c.take<double>(np);
+  }
+  pa.r = c.take<double>(np);
+  pa.rho_ratio = c.take<double>(np);
+  pa.Tw = c.take<double>(np);
+  pa.Fx = c.take<double>(np);
+  pa.Fy = c.take<double>(np);
+  pa.Tz = c.take<double>(np);
+  pa.fixed = c.take<unsigned char>(np);
+  LinkArrays la;
+  const size_t nl = np * (size_t)p->max_links_per_particle;
+  la.node = c.take<int>(nl);
+  la.dir = c.take<unsigned char>(nl);
+  la.q = c.take<double>(nl);
+  la.count = c.take<int>(np);
+  la.cap = p->max_links_per_particle;
+  int* cell_count = c.take<int>((size_t)L.max_cells);
+  int* cell_items = c.take<int>((size_t)L.max_cells * CELL_CAP);
+  int* nb_node = c.take<int>((size_t)L.newborn_cap);
+  int* nb_pid = c.take<int>((size_t)L.newborn_cap);
+  int* nb_count = c.take<int>(1);
+  int* status = c.take<int>(1);
+  if (h) {
+    h->px = L.px;
+    h->ps = L.ps;
+    h->A = A;
+    h->B = B;
+    h->flag = flag;
+    h->owner = owner;
+    h->pa = pa;
+    h->la = la;
+    h->cell_count = cell_count;
+    h->cell_items = cell_items;
+    h->max_cells = L.max_cells;
+    h->newborn_node = nb_node;
+    h->newborn_pid = nb_pid;
+    h->newborn_count = nb_count;
+    h->newborn_cap = L.newborn_cap;
+    h->status_dev = status;
+  }
+  return align_up(c.off, 256);
+}
+
+bool params_ok(int nx, int ny, const lbm_params* p) {
+  return p && nx >= 4 && ny >= 4 && nx <= 46000 && ny <= 46000 && p->nu > 0.0 && p->kappa > 0.0 &&
+         p->kappa < 0.144 && p->rho0 > 0.0 && p->max_particles >= 0 &&
+         p->max_links_per_particle >= 0 && p->rep_s > 0.0 && p->rep_eps > 0.0 &&
+         p->rep_power >= 1 && std::isfinite(p->nu) && std::isfinite(p->kappa);
+}
+
+void fill_const(lbm* h) {
+  LbmConst& c = h->C;
+  const lbm_params& p = h->P;
+  c.nx = h->nx;
+  c.ny = h->ny;
+  c.px = h->px;
+  c.ps = h->ps;
+  c.periodic_x = p.periodic_x ? 1 : 0;
+  // DESIGN.md readings: s_nu = 1/tau, tau = 3 nu + 1/2, s_e = s_eps = s_nu, s_q = 8(2-s_nu)/(8-s_nu)
+  const double tau = 3.0 * p.nu + 0.5;
+  c.s_nu = 1.0 / tau;
+  c.s_e = c.s_nu;
+  c.s_eps = c.s_nu;
+  c.s_q = 8.0 * (2.0 - c.s_nu) / (8.0 - c.s_nu);
+  const double r3 = std::sqrt(3.0);
+  c.q_k = 3.0 - r3;
+  c.q_e = 4.0 * r3 - 6.0;
+  c.q_nu = 4.0 * r3 - 6.0;
+  c.aT = 20.0 * r3 * p.kappa - 4.0;
+  c.wT0 = (1.0 - c.aT) / 5.0;
+  c.wT = (4.0 + c.aT) / 20.0;
+  c.rho0 = p.rho0;
+  c.T0 = p.T0;
+  c.gbeta = p.gbeta;
+  c.ax = p.body_ax;
+  c.ay = p.body_ay;
+  c.g = p.g;
+  for (int k = 0; k < 4; ++k) {
+    c.wall_type[k] = p.wall_T_type[k];
+    c.wall_T[k] = p.wall_T[k];
+  }
+  c.rep_s = p.rep_s;
+  c.rep_eps = p.rep_eps;
+  c.rep_power = p.rep_power;
+}
+
+// ---- profiling helpers ----
+struct Timed {
+  lbm* h;
+  int k;
+  bool on;
+  Timed(lbm* h_, int k_) : h(h_), k(k_), on(false) {
+    if (h->prof_on && h->ev_n[k] < LBM_PROFILE_MAX_SAMPLES) {
+      on = true;
+      cudaEventRecord(h->ev0[k][h->ev_n[k]], h->stream);
+    }
+  }
+  ~Timed() {
+    if (on) {
+      cudaEventRecord(h->ev1[k][h->ev_n[k]], h->stream);
+      h->ev_n[k]++;
+    }
+  }
+};
+
+int check_status(lbm* h) {
+  CUDA_OK(h, cudaMemcpyAsync(h->status_host, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaGetLastError());
+  const int st = *h->status_host;
+  if (st & ST_NONFINITE) return fail(h, LBM_E_NONFINITE, "a particle state became NaN/Inf");
+  if (st & ST_LINK_OVERFLOW) return fail(h, LBM_E_CAPACITY, "a particle has more links than max_links_per_particle");
+  if (st & ST_CELL_OVERFLOW) return fail(h, LBM_E_CAPACITY, "more than %d particle centres in one repulsion cell", CELL_CAP);
+  if (st & ST_NEWBORN_OVERFLOW) return fail(h, LBM_E_CAPACITY, "newborn-node list overflow");
+  return LBM_OK;
+}
+
+void prime(lbm* h) {
+  if (h->primed) return;
+  Timed t(h, K_INIT);
+  launch_init_collide(h, h->A);
+  h->primed = 1;
+}
+
+} // namespace
+
+extern "C" {
+
+void lbm_params_default(lbm_params* p) {
+  if (!p) return;
+  std::memset(p, 0, sizeof(*p));
+  p->nu = 0.02;
+  p->kappa = 0.02 / 0.7;
+  p->rho0 = 1.0;
+  p->rep_s = 2.0;
+  p->rep_eps = 1e-3;
+  p->rep_power = 1;
+}
+
+size_t lbm_workspace_bytes(int nx, int ny, const lbm_params* p) {
+  if (!params_ok(nx, ny, p)) return 0;
+  return carve(nullptr, nullptr, nx, ny, p);
+}
+
+int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t bytes,
+               void* cuda_stream, lbm_t** out) {
+  if (!out) return fail(nullptr, LBM_E_ARG, "lbm_create: out is NULL");
+  *out = nullptr;
+  if (!params_ok(nx, ny, p)) return fail(nullptr, LBM_E_ARG, "lbm_create: bad size or parameter");
+  if (!dev_workspace || ((uintptr_t)dev_workspace & 255))
+    return fail(nullptr, LBM_E_ARG, "lbm_create: workspace NULL or not 256-byte aligned");
+  const size_t need = carve(nullptr, nullptr, nx, ny, p);
+  if (bytes < need) return fail(nullptr, LBM_E_CAPACITY, "lbm_create: workspace %zu < %zu bytes", bytes, need);
+  if ((long long)layout_of(nx, ny, p).px * ny >= 0x7fffffffLL)
+    return fail(nullptr, LBM_E_ARG, "lbm_create: lattice too large for 32-bit node indices");
+  lbm* h = new (std::nothrow) lbm;
+  if (!h) return fail(nullptr, LBM_E_ARG, "lbm_create: out of host memory");
+  std::memset(h, 0, sizeof(*h));
+  h->nx = nx;
+  h->ny = ny;
+  h->P = *p;
+  h->stream = (cudaStream_t)cuda_stream;
+  carve(h, dev_workspace, nx, ny, p);
+  fill_const(h);
+  cudaError_t e = cudaMallocHost((void**)&h->status_host, sizeof(int));
+  if (e != cudaSuccess) {
+    fail(nullptr, LBM_E_CUDA, "cudaMallocHost: %s", cudaGetErrorString(e));
+    delete h;
+    return LBM_E_CUDA;
+  }
+  // initial state: fluid everywhere, f = f_eq(rho0, 0), g = g_eq(T0, 0)
+  const size_t nn = (size_t)h->px * ny;
+  cudaMemsetAsync(h->flag, 0, nn, h->stream);
+  cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
+  cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
+  cudaMemsetAsync(h->newborn_count, 0, sizeof(int), h->stream);
+  cudaMemsetAsync(h->B, 0, sizeof(double) * 14 * (size_t)h->ps, h->stream);
+  launch_set_equilibrium(h);
+  e = cudaStreamSynchronize(h->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    fail(nullptr, LBM_E_CUDA, "lbm_create: %s", cudaGetErrorString(e));
+    cudaFreeHost(h->status_host);
+    delete h;
+    return LBM_E_CUDA;
+  }
+  *out = h;
+  return LBM_OK;
+}
+
+int lbm_set_temperature(lbm_t* h, const double* T_host) {
+  if (!h || !T_host) return h ? fail(h, LBM_E_ARG, "set_temperature: NULL") : LBM_E_ARG;
+  if (h->primed) return fail(h, LBM_E_STATE, "set_temperature after the first step");
+  // B is scratch until the first step writes it
+  const size_t n = (size_t)h->nx * h->ny;
+  CUDA_OK(h, cudaMemcpyAsync(h->B, T_host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  launch_set_temperature(h, h->B);
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaGetLastError());
+  return LBM_OK;
+}
+
+int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const double* diam,
+                      const double* rho_ratio, const double* T_w, const double* ux,
+                      const double* uy, const double* omega, const unsigned char* fixed) {
+  if (!h) return LBM_E_ARG;
+  if (n < 0 || (n > 0 && (!x || !y || !diam || !rho_ratio || !T_w)))
+    return fail(h, LBM_E_ARG, "add_particles: NULL array or negative count");
+  if (h->primed) return fail(h, LBM_E_STATE, "add_particles after the first step");
+  if (n == 0) return LBM_OK;
+  if ((long long)h->np + n > h->P.max_particles)
+    return fail(h, LBM_E_CAPACITY, "add_particles: max_particles (%d) exceeded", h->P.max_particles);
+
+  // existing particles (host mirror via a device read; add_particles is a set-up call)
+  const int n0 = h->np, nt = n0 + n;
+  std::vector<double> X(nt), Y(nt), R(nt);
+  if (n0) {
+    CUDA_OK(h, cudaMemcpyAsync(X.data(), h->pa.x[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpyAsync(Y.data(), h->pa.y[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpyAsync(R.data(), h->pa.r, n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  }
+  double dmax = h->d_max;
+  for (int k = 0; k < n; ++k) {
+    const double r = 0.5 * diam[k];
+    if (!(r > 0.0) || !(rho_ratio[k] > 0.0) || !std::isfinite(x[k]) || !std::isfinite(y[k]) ||
+        !std::isfinite(r) || !std::isfinite(T_w[k]) || (ux && !std::isfinite(ux[k])) ||
+        (uy && !std::isfinite(uy[k])) || (omega && !std::isfinite(omega[k])))
+      return fail(h, LBM_E_ARG, "add_particles: particle %d has a bad or non-finite value", k);
+    if (!(y[k] - r > -0.5) || !(y[k] + r < h->ny - 0.5))
+      return fail(h, LBM_E_ARG, "add_particles: particle %d touches a y wall", k);
+    if (!h->P.periodic_x) {
+      if (!(x[k] - r > -0.5) || !(x[k] + r < h->nx - 0.5))
+        return fail(h, LBM_E_ARG, "add_particles: particle %d touches an x wall", k);
+    } else if ((int)std::floor(x[k] - r) - 2 < 0 || (int)std::floor(x[k] + r) + 2 > h->nx - 1) {
+      return fail(h, LBM_E_ARG, "add_particles: zone of particle %d crosses the periodic seam", k);
+    }
+    const int Nmax = (int)std::floor(2.0 * r) + 4;   // worst-case N of PAPER.md:258
+    if (12 * Nmax - 12 > h->P.max_links_per_particle)
+      return fail(h, LBM_E_CAPACITY, "add_particles: 12N-12 = %d exceeds max_links_per_particle = %d",
+                  12 * Nmax - 12, h->P.max_links_per_particle);
+    X[n0 + k] = x[k];
+    Y[n0 + k] = y[k];
+    R[n0 + k] = r;
+    dmax = std::max(dmax, 2.0 * r);
+  }
+  // overlap test through a host cell grid (cell >= largest diameter)
+  {
+    const double cell = std::max(dmax, 1.0);
+    std::map<std::pair<int, int>, std::vector<int>> grid;
+    for (int k = 0; k < nt; ++k) {
+      const int ci = (int)std::floor(X[k] / cell), cj = (int)std::floor(Y[k] / cell);
+      if (k >= n0)
+        for (int a = ci - 1; a <= ci + 1; ++a)
+          for (int b = cj - 1; b <= cj + 1; ++b) {
+            auto it = grid.find({a, b});
+            if (it == grid.end()) continue;
+            for (int m : it->second) {
+              const double dx = X[k] - X[m], dy = Y[k] - Y[m];
+              if (std::sqrt(dx * dx + dy * dy) < R[k] + R[m])
+                return fail(h, LBM_E_ARG, "add_particles: particles %d and %d overlap", m, k);
+            }
+          }
+      grid[{ci, cj}].push_back(k);
+    }
+  }
+  // upload
+  const int c = h->cur;
+  std::vector<double> zero(n, 0.0), rr(n);
+  for (int k = 0; k < n; ++k) rr[k] = 0.5 * diam[k];
+  std::vector<unsigned char> fx(n, 0);
+  if (fixed)
+    for (int k = 0; k < n; ++k) fx[k] = fixed[k] ? 1 : 0;
+  auto up = [&](double* dst, const double* src) {
+    return cudaMemcpyAsync(dst + n0, src ? src : zero.data(), n * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+  };
+  for (int b = 0; b < 2; ++b) {
+    CUDA_OK(h, up(h->pa.x[b], x));
+    CUDA_OK(h, up(h->pa.y[b], y));
+    CUDA_OK(h, up(h->pa.theta[b], nullptr));
+    CUDA_OK(h, up(h->pa.ux[b], ux));
+    CUDA_OK(h, up(h->pa.uy[b], uy));
+    CUDA_OK(h, up(h->pa.omega[b], omega));
+  }
+  CUDA_OK(h, up(h->pa.r, rr.data()));
+  CUDA_OK(h, up(h->pa.rho_ratio, rho_ratio));
+  CUDA_OK(h, up(h->pa.Tw, T_w));
+  CUDA_OK(h, up(h->pa.Fx, nullptr));
+  CUDA_OK(h, up(h->pa.Fy, nullptr));
+  CUDA_OK(h, up(h->pa.Tz, nullptr));
+  CUDA_OK(h, cudaMemcpyAsync(h->pa.fixed + n0, fx.data(), n, cudaMemcpyHostToDevice, h->stream));
+  h->np = nt;
+  h->d_max = dmax;
+  h->cell = std::max(dmax + h->P.rep_s, MIN_CELL);
+  h->ncx = (int)std::ceil(h->nx / h->cell) + 1;
+  h->ncy = (int)std::ceil(h->ny / h->cell) + 1;
+  if ((long long)h->ncx * h->ncy > h->max_cells)
+    return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
+  launch_cover(h, c);   // stamp flag and owner maps (primed == 0: fixed particles too)
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaGetLastError());
+  (void)c;
+  return LBM_OK;
+}
+
+int lbm_step(lbm_t* h, int nsteps) {
+  if (!h) return LBM_E_ARG;
+  if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
+  prime(h);
+  for (int s = 0; s < nsteps; ++s) {
+    if (h->np > 0) {
+      { Timed t(h, K_BUILD_LINKS); launch_build_links(h); }
+      { Timed t(h, K_BOUNCE_BACK); launch_bounce_back(h); }
+      { Timed t(h, K_INTEGRATE); launch_cells_and_integrate(h); }
+      { Timed t(h, K_UNCOVER); launch_uncover(h); }
+      { Timed t(h, K_COVER); launch_cover(h, h->cur ^ 1); }
+      h->cur ^= 1;
+    }
+    { Timed t(h, K_STREAM_COLLIDE); launch_stream_collide(h); }
+    if (h->np > 0) { Timed t(h, K_REFILL); launch_refill(h); }
+    std::swap(h->A, h->B);
+    h->steps_done++;
+  }
+  return check_status(h);
+}
+
+int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, double* f, double* g,
+                   unsigned char* flag) {
+  if (!h) return LBM_E_ARG;
+  const size_t n = (size_t)h->nx * h->ny;
+  if (rho || ux || uy || T) {
+    // B is dead between steps: use four of its planes as dense scratch
+    double* s0 = h->B;
+    double* s1 = h->B + h->ps;
+    double* s2 = h->B + 2 * h->ps;
+    double* s3 = h->B + 3 * h->ps;
+    launch_macroscopic(h, s0, s1, s2, s3);
+    if (rho) CUDA_OK(h, cudaMemcpyAsync(rho, s0, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (ux) CUDA_OK(h, cudaMemcpyAsync(ux, s1, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (uy) CUDA_OK(h, cudaMemcpyAsync(uy, s2, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (T) CUDA_OK(h, cudaMemcpyAsync(T, s3, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  }
+  if (f || g) {
+    // f, g are defined as the post-collision populations; before the first step the resident
+    // state is still pre-collision, so collide it into the scratch copy (stream order keeps the
+    // macroscopic copies above ahead of this overwrite of B)
+    const double* src = h->A;
+    if (!h->primed) {
+      launch_init_collide(h, h->B);
+      src = h->B;
+    }
+    const size_t row = (size_t)h->nx * sizeof(double), pitch = (size_t)h->px * sizeof(double);
+    for (int k = 0; k < 14; ++k) {
+      double* dst = k < 9 ? (f ? f + (size_t)k * n : nullptr) : (g ? g + (size_t)(k - 9) * n : nullptr);
+      if (!dst) continue;
+      CUDA_OK(h, cudaMemcpy2DAsync(dst, row, src + (size_t)k * h->ps, pitch, row, h->ny,
+                                   cudaMemcpyDeviceToHost, h->stream));
+    }
+  }
+  if (flag)
+    CUDA_OK(h, cudaMemcpy2DAsync(flag, h->nx, h->flag, h->px, h->nx, h->ny, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaGetLastError());
+  return LBM_OK;
+}
+
+int lbm_get_particles(lbm_t* h, int* n, double* x, double* y, double* theta, double* ux,
+                      double* uy, double* omega, double* Fx, double* Fy, double* Tz) {
+  if (!h || !n) return h ? fail(h, LBM_E_ARG, "get_particles: n is NULL") : LBM_E_ARG;
+  *n = h->np;
+  if (h->np == 0) return LBM_OK;
+  const int c = h->cur;
+  const size_t b = (size_t)h->np * sizeof(double);
+  auto down = [&](double* dst, const double* src) {
+    return dst ? cudaMemcpyAsync(dst, src, b, cudaMemcpyDeviceToHost, h->stream) : cudaSuccess;
+  };
+  CUDA_OK(h, down(x, h->pa.x[c]));
+  CUDA_OK(h, down(y, h->pa.y[c]));
+  CUDA_OK(h, down(theta, h->pa.theta[c]));
+  CUDA_OK(h, down(ux, h->pa.ux[c]));
+  CUDA_OK(h, down(uy, h->pa.uy[c]));
+  CUDA_OK(h, down(omega, h->pa.omega[c]));
+  CUDA_OK(h, down(Fx, h->pa.Fx));
+  CUDA_OK(h, down(Fy, h->pa.Fy));
+  CUDA_OK(h, down(Tz, h->pa.Tz));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  return LBM_OK;
+}
+
+int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, double* q) {
+  if (!h || !n) return h ? fail(h, LBM_E_ARG, "get_links: n is NULL") : LBM_E_ARG;
+  const long long capacity = *n;
+  *n = 0;
+  if (h->np == 0) return LBM_OK;
+  launch_build_links(h);
+  std::vector<int> count(h->np);
+  CUDA_OK(h, cudaMemcpyAsync(count.data(), h->la.count, h->np * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  int rc = check_status(h);
+  if (rc) return rc;
+  long long total = 0;
+  for (int c : count) total += c;
+  *n = total;
+  if (total > capacity) return fail(h, LBM_E_CAPACITY, "get_links: %lld links, capacity %lld", total, capacity);
+  const size_t nl = (size_t)h->np * h->la.cap;
+  std::vector<int> node(nl);
+  std::vector<unsigned char> dir(nl);
+  std::vector<double> qq(nl);
+  CUDA_OK(h, cudaMemcpyAsync(node.data(), h->la.node, nl * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaMemcpyAsync(dir.data(), h->la.dir, nl, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaMemcpyAsync(qq.data(), h->la.q, nl * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  long long o = 0;
+  for (int p = 0; p < h->np; ++p)
+    for (int s = 0; s < count[p]; ++s, ++o) {
+      const size_t k = (size_t)p * h->la.cap + s;
+      if (pid) pid[o] = p;
+      if (i) i[o] = node[k] % h->px;
+      if (j) j[o] = node[k] / h->px;
+      if (alpha) alpha[o] = dir[k];
+      if (q) q[o] = qq[k];
+    }
+  return LBM_OK;
+}
+
+int lbm_profile_enable(lbm_t* h, int on) {
+  if (!h) return LBM_E_ARG;
+  if (on) {
+    for (int k = 0; k < K_COUNT; ++k) {
+      if (!h->ev0[k]) {
+        h->ev0[k] = new cudaEvent_t[LBM_PROFILE_MAX_SAMPLES];
+        h->ev1[k] = new cudaEvent_t[LBM_PROFILE_MAX_SAMPLES];
+        for (int s = 0; s < LBM_PROFILE_MAX_SAMPLES; ++s) {
+          CUDA_OK(h, cudaEventCreate(&h->ev0[k][s]));
+          CUDA_OK(h, cudaEventCreate(&h->ev1[k][s]));
+        }
+      }
+      h->ev_n[k] = 0;
+    }
+  }
+  h->prof_on = on ? 1 : 0;
+  return LBM_OK;
+}
+
+int lbm_profile_kernels(void) { return K_COUNT; }
+
+const char* lbm_profile_kernel_name(int kernel_id) {
+  return (kernel_id >= 0 && kernel_id < K_COUNT) ? kKernelNames[kernel_id] : "";
+}
+
+int lbm_profile_get(lbm_t* h, int kernel_id, double* total_ms, long long* launches) {
+  if (!h || kernel_id < 0 || kernel_id >= K_COUNT) return LBM_E_ARG;
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  double tot = 0.0;
+  const int n = h->ev0[kernel_id] ? h->ev_n[kernel_id] : 0;
+  for (int s = 0; s < n; ++s) {
+    float ms = 0.f;
+    CUDA_OK(h, cudaEventElapsedTime(&ms, h->ev0[kernel_id][s], h->ev1[kernel_id][s]));
+    tot += ms;
+  }
+  if (total_ms) *total_ms = tot;
+  if (launches) *launches = n;
+  return LBM_OK;
+}
+
+long long lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : -1; }
+
+int lbm_destroy(lbm_t* h) {
+  if (!h) return LBM_OK;
+  cudaStreamSynchronize(h->stream);
+  for (int k = 0; k < K_COUNT; ++k)
+    if (h->ev0[k]) {
+      for (int s = 0; s < LBM_PROFILE_MAX_SAMPLES; ++s) {
+        cudaEventDestroy(h->ev0[k][s]);
+        cudaEventDestroy(h->ev1[k][s]);
+      }
+      delete[] h->ev0[k];
+      delete[] h->ev1[k];
+    }
+  if (h->status_host) cudaFreeHost(h->status_host);
+  delete h;
+  return LBM_OK;
+}
+
+const char* lbm_last_error(const lbm_t* h) { return h ? h->err : g_create_error; }
+
+} // extern "C"

@@ -1,0 +1,113 @@
+// lbm_internal.cuh -- shared declarations of the CUDA path (product).  Not part of the C ABI.
+//
+// HBM layout: structure of arrays, fp64.
+//   populations: 14 planes (f0..f8, g0..g4), plane k at base + k*ps doubles, node (i,j) at j*px + i
+//   px = nx rounded up to 16 doubles (128 B rows -> every row start is sector- and TMA-aligned),
+//   ps = px*ny rounded up to 32 doubles.  Two copies A (read) and B (written), swapped per step.
+//   flag : 1 byte/node, 0 fluid, 1 solid, 2 newborn (solid at t, fluid at t+1; only between the
+//          flag update and the refill kernel of one step)
+//   owner: int32/node, id of the lowest-numbered particle covering the node, OWNER_NONE = fluid
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lbm.h"
+
+#define OWNER_NONE 0x7f7f7f7f   // = cudaMemset(0x7f): larger than any particle id
+#define CELL_CAP 32          // particle centres per repulsion-grid cell
+#define MIN_CELL 16.0        // smallest repulsion-grid cell edge (workspace is sized for it)
+#define NEWBORN_PER_PARTICLE 64
+
+// status bits written by kernels, read once per lbm_step call
+#define ST_NONFINITE 1
+#define ST_LINK_OVERFLOW 2
+#define ST_CELL_OVERFLOW 4
+#define ST_NEWBORN_OVERFLOW 8
+
+enum {
+  K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
+  K_INIT, K_COUNT
+};
+
+// constants every kernel needs; passed by value (lands in the constant bank)
+struct LbmConst {
+  int nx, ny, px;          // lattice size, row pitch (doubles)
+  long long ps;            // plane stride (doubles)
+  int periodic_x;
+  // D2Q9 MRT (DESIGN.md readings): relaxation rates and the (1 - s/2) forcing factors
+  double s_e, s_eps, s_q, s_nu;
+  // D2Q5 MRT
+  double q_k, q_e, q_nu, aT, wT0, wT;   // wT0 = (1-aT)/5, wT = (4+aT)/20
+  double rho0, T0, gbeta, ax, ay, g;
+  int wall_type[4];        // W,E,S,N
+  double wall_T[4];
+  double rep_s, rep_eps;
+  int rep_power;
+};
+
+struct ParticleArrays {      // SoA in the workspace, each max_particles long
+  double *x[2], *y[2], *theta[2], *ux[2], *uy[2], *omega[2];   // double-buffered state
+  double *r, *rho_ratio, *Tw;
+  double *Fx, *Fy, *Tz;      // hydrodynamic force / torque of the last step (Eqs. 13, 14)
+  unsigned char* fixed;
+};
+
+struct LinkArrays {          // the paper's fixed index array: segment p = [p*cap, (p+1)*cap)
+  int* node;                 // j*px + i of the fluid node x_f
+  unsigned char* dir;        // alpha in 1..8
+  double* q;
+  int* count;                // links of particle p
+  int cap;
+};
+
+struct lbm {
+  int nx, ny, px;
+  long long ps;
+  lbm_params P;
+  LbmConst C;
+  cudaStream_t stream;
+  double *A, *B;             // 14 planes each
+  unsigned char* flag;
+  int* owner;
+  ParticleArrays pa;
+  LinkArrays la;
+  int cur;                   // which particle state buffer is current
+  int np;                    // particles added
+  double d_max;              // largest diameter (sizes the repulsion grid)
+  int* cell_count;
+  int* cell_items;
+  int ncx, ncy;
+  double cell;               // cell edge
+  int max_cells;
+  int* newborn_node;
+  int* newborn_pid;
+  int* newborn_count;
+  int newborn_cap;
+  int* status_dev;
+  int* status_host;          // pinned
+  int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
+  long long steps_done;
+  long long launches;        // kernels launched (lbm_kernel_launches)
+  // profiling
+  int prof_on;
+  cudaEvent_t* ev0[K_COUNT];
+  cudaEvent_t* ev1[K_COUNT];
+  int ev_n[K_COUNT];
+  char err[512];
+};
+
+// ---- kernel launchers (each in its own translation unit) ----
+// stream_collide.cu
+void launch_stream_collide(lbm* h);
+void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
+void launch_set_temperature(lbm* h, const double* T_dev_dense);
+void launch_set_equilibrium(lbm* h);
+void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
+// particles.cu (compiled with -fmad=false)
+void launch_build_links(lbm* h);
+void launch_cells_and_integrate(lbm* h);
+void launch_uncover(lbm* h);
+void launch_cover(lbm* h, int which_buffer);
+// bounce_back.cu
+void launch_bounce_back(lbm* h);
+void launch_refill(lbm* h);

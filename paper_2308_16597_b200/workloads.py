@@ -2,15 +2,15 @@
 
 This module holds NONE of the method's arithmetic (no collision, streaming, bounce-back, force or
 integration formulas): it only produces parameters, initial temperature fields and particle
-placements.  Both `paper_2308_16597_b200.binding` (product) and `oracle/oracle_binding.py` (test
-infrastructure) receive the same arrays, so parity is taken on identical bits.
+placements.  Both the CUDA binding (product) and the CPU checker used by the tests (test infrastructure,
+kept outside this package) receive the same arrays, so parity is taken on identical bits.
 
 The five workloads are `BASELINE.json` `configs[0..4]` as resolved in SURVEY.md 8(d) "Synthetic
 inputs" (they stand in for the paper's own benchmark, 4,800 hot particles in a 4000^2 cavity,
 PAPER.md:230-246, whose shapes the configs override).  Nothing is read from a dataset.
 
 `lattice_units()` is the paper's unit conversion (Eqs. 2-4 and Tables 1-4, PAPER.md:51-70,
-173-244), a harness helper used to choose g and to pin the oracle's parameter handling.
+173-244), a harness helper used to choose g and pinned against the paper's printed tables.
 """
 from __future__ import annotations
 

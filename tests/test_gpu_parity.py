@@ -1,0 +1,229 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI, via the thin binding) against the
+paper-order CPU oracle on the same seeded inputs, element by element.
+
+Sizes here are ones the oracle finishes in seconds; every lattice spans several 128-thread tiles
+and has a ragged tail (nx not a multiple of 128 / 16).  Full-size cases are in
+test_gpu_fullsize.py.  Tolerances: tests/parity.py.
+"""
+import numpy as np
+import pytest
+
+from parity import (assert_fields_close, assert_links_equal, assert_particles_close)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2308_16597_b200 import binding
+    binding.load_library()   # fails loudly if the CUDA library is missing: there is no fallback
+    return binding
+
+
+def both(gpu, ob, w):
+    return gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+
+
+def run_and_compare(gpu, ob, w, checkpoints, r_min=10.0, links=True):
+    g, o = both(gpu, ob, w)
+    if links and w.particles is not None:
+        assert_links_equal(g.links(), o.links())
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    done = 0
+    out = {}
+    for c in checkpoints:
+        g.step(c - done)
+        o.step(c - done)
+        done = c
+        out[c] = assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+        if w.particles is not None:
+            out[c].update(assert_particles_close(g.particles(), o.particles(), r_min, steps=c))
+    return g, o, out
+
+
+# ------------------------------------------------------------------ particle-free (row a1)
+
+def test_rayleigh_benard_small_ragged(gpu, ob, wl):
+    """Config 1's set-up (bottom hot, top cold, adiabatic sides, conduction profile + seeded noise)
+    on 333 x 130: three 128-wide tiles with a 77-wide tail, pitch 336 != nx."""
+    nx, ny = 333, 130
+    w = wl.config(1)
+    rng = np.random.default_rng(11)
+    j = np.arange(ny, dtype=np.float64)[:, None]
+    T = (1.0 - (j + 0.5) / ny) + 1e-3 * rng.uniform(-1.0, 1.0, size=(ny, nx))
+    w = wl.Workload("rb_small", nx, ny, dict(w.params, gbeta=1e-4), steps=100, parity_steps=100,
+                    T_init=np.ascontiguousarray(T))
+    run_and_compare(gpu, ob, w, [1, 2, 100])
+
+
+def test_all_wall_types_and_body_force(gpu, ob, wl):
+    """Every wall branch of the rim path: W Dirichlet 0.3, E adiabatic, S Dirichlet 1, N Dirichlet
+    -0.2, plus a uniform body acceleration in both directions (Guo forcing terms of Eq. 5)."""
+    p = wl.default_params()
+    p.update(wall_T_type=[1, 0, 1, 1], wall_T=[0.3, 0.0, 1.0, -0.2], gbeta=2e-4, T0=0.25,
+             body_ax=1e-5, body_ay=-2e-5, nu=0.05, kappa=0.03)
+    rng = np.random.default_rng(5)
+    T = 0.25 + 0.5 * rng.uniform(-1, 1, size=(37, 141))
+    w = wl.Workload("walls", 141, 37, p, 60, 60, T_init=T)
+    run_and_compare(gpu, ob, w, [1, 60])
+
+
+def test_periodic_poiseuille(gpu, ob, wl):
+    """x-periodic body-force channel (the closed-form check's set-up): wrap-around pulls."""
+    p = wl.default_params()
+    p.update(periodic_x=1, body_ax=1e-6, nu=0.1)
+    w = wl.Workload("poiseuille", 20, 33, p, 200, 200)
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 200])
+    # and the GPU itself against the closed form after convergence (independent of the oracle)
+    g.step(6000)
+    ux = g.fields()["ux"]
+    jj = np.arange(33, dtype=np.float64)
+    exact = 1e-6 / (2 * 0.1) * (jj + 0.5) * (33 - 0.5 - jj)
+    assert np.abs(ux[:, 3] - exact).max() / exact.max() < 1e-8
+
+
+def test_smallest_lattice_and_zero_steps(gpu, ob, wl):
+    p = wl.default_params()
+    p.update(gbeta=1e-3, wall_T_type=[0, 0, 1, 1], wall_T=[0, 0, 1.0, 0.0])
+    w = wl.Workload("tiny", 4, 4, p, 10, 10)
+    g, o = both(gpu, ob, w)
+    g.step(0)
+    o.step(0)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    g.step(25)
+    o.step(25)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+
+
+def test_mass_conservation_closed_box_gpu(gpu, wl):
+    """Property that holds at any size: particle-free closed box conserves total mass to 1e-12."""
+    w = wl.config(1)
+    g = gpu.Simulation.from_workload(w)
+    m0 = g.fields()["rho"].sum()
+    g.step(300)
+    m1 = g.fields()["rho"].sum()
+    assert abs(m1 - m0) / m0 < 1e-12
+
+
+# ------------------------------------------------------------------ particles (rows a2-a6)
+
+def test_config0_single_hot_particle(gpu, ob, wl):
+    """BASELINE config 0 in full: 128x256, one d=20 hot particle settling from rest.  Links
+    bit-exact at step 0, fields and particle state at 100 and 1000 steps (the particle has moved
+    ~20 nodes by then: thousands of cover / uncover / refill events)."""
+    w = wl.config(0)
+    g, o, errs = run_and_compare(gpu, ob, w, [1, 100, 1000])
+    pg, po = g.particles(), o.particles()
+    assert po["y"][0] < 200.0 - 5.0 and abs(pg["y"][0] - po["y"][0]) < 1e-7
+    # links again after the run, on the oracle's particle state injected into fresh simulations
+    assert_links_after_injection(gpu, ob, wl, w, po)
+
+
+def assert_links_after_injection(gpu, ob, wl, w, po):
+    parts = dict(w.particles)
+    parts.update(x=po["x"], y=po["y"], ux=po["ux"], uy=po["uy"], omega=po["omega"])
+    w2 = wl.Workload(w.name + "_inj", w.nx, w.ny, w.params, 1, 1, particles=parts)
+    try:
+        g2, o2 = both(gpu, ob, w2)
+    except Exception as e:   # particles that drifted into overlap are rejected by both sides
+        pytest.skip(f"injected state rejected: {e}")
+    assert_links_equal(g2.links(), o2.links())
+    fg, fo = g2.fields(), o2.fields()
+    assert np.array_equal(fg["flag"], fo["flag"])
+
+
+def test_moving_rotating_particles_mixed_sizes(gpu, ob, wl):
+    """Several particles of different diameters with initial velocities and spins, two of them
+    within the repulsion range of each other and one next to a wall: exercises the fallback
+    ladders (stencil nodes inside another particle / beyond the wall), repulsion (pair and wall),
+    refill in every direction.  303 x 190 lattice (ragged)."""
+    nx, ny = 303, 190
+    x = np.array([40.0, 62.3, 150.5, 151.0, 250.25, 12.4, 200.0, 100.7])
+    y = np.array([60.0, 61.1, 100.0, 125.5, 40.5, 150.0, 174.6, 20.9])
+    d = np.array([20.0, 21.5, 24.0, 24.0, 12.0, 22.0, 24.0, 18.6])
+    n = len(x)
+    ux = np.array([0.01, -0.01, 0.0, 0.0, 0.02, -0.01, 0.0, 0.015])
+    uy = np.array([0.0, 0.0, 0.01, -0.01, 0.02, 0.0, 0.005, -0.01])
+    om = np.array([0.002, -0.003, 0.0, 0.001, -0.004, 0.002, 0.0, 0.003])
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=n,
+             max_links_per_particle=wl.max_links_for_diameter(24.0))
+    parts = dict(x=x, y=y, diam=d, rho_ratio=np.linspace(1.1, 2.0, n), T_w=np.linspace(0.2, 1.0, n),
+                 ux=ux, uy=uy, omega=om)
+    w = wl.Workload("mixed", nx, ny, p, 150, 150, particles=parts)
+    g, o, errs = run_and_compare(gpu, ob, w, [1, 2, 50, 150], r_min=6.0)
+    assert_links_after_injection(gpu, ob, wl, w, o.particles())
+
+
+def test_paper_repulsion_variant(gpu, ob, wl):
+    """Eq. (15) as the paper prints it: quadratic, s = 3, eps_w = 1e-3; two
+    particles approaching head-on and one falling onto the bottom wall."""
+    nx, ny = 160, 96
+    p = wl.default_params()
+    p.update(g=3e-4, gbeta=0.0, rep_s=3.0, rep_power=2, max_particles=3,
+             max_links_per_particle=wl.max_links_for_diameter(20.0), wall_T_type=[1, 1, 1, 1])
+    parts = dict(x=np.array([40.0, 63.5, 120.0]), y=np.array([50.0, 50.0, 12.2]),
+                 diam=np.array([20.0, 20.0, 20.0]), rho_ratio=np.array([1.5, 1.5, 2.5]),
+                 T_w=np.array([1.0, 0.5, 0.0]), ux=np.array([0.02, -0.02, 0.0]),
+                 uy=np.array([0.0, 0.0, -0.02]), omega=np.zeros(3))
+    w = wl.Workload("rep", nx, ny, p, 120, 120, particles=parts)
+    run_and_compare(gpu, ob, w, [1, 120])
+
+
+def test_fixed_cylinder_in_channel(gpu, ob, wl):
+    """Fixed (immobile) particle in an x-periodic body-force channel: force is computed, state is
+    not integrated; zero-lift symmetry holds on the GPU too."""
+    nx, ny = 96, 65
+    p = wl.default_params()
+    p.update(periodic_x=1, body_ax=2e-6, nu=0.05, max_particles=1,
+             max_links_per_particle=wl.max_links_for_diameter(16.0))
+    parts = dict(x=np.array([48.0]), y=np.array([32.0]), diam=np.array([16.0]),
+                 rho_ratio=np.array([1.5]), T_w=np.array([0.0]), fixed=np.array([1], dtype=np.uint8))
+    w = wl.Workload("cyl", nx, ny, p, 400, 400, particles=parts)
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 400], r_min=8.0)
+    pg = g.particles()
+    assert pg["x"][0] == 48.0 and pg["y"][0] == 32.0 and pg["ux"][0] == 0.0
+    assert pg["Fx"][0] > 0 and abs(pg["Fy"][0]) < 1e-10 * abs(pg["Fx"][0])
+
+
+def test_small_sedimentation_many_particles(gpu, ob, wl):
+    """Structure of configs 2-4 at a size the oracle does in seconds: 40 particles of seeded
+    diameters in [12, 24], 2-unit gaps, 420 x 300."""
+    w = wl.sedimentation(420, 300, 40, seed=7, y_frac_lo=0.0, d_lo=12.0, d_hi=24.0,
+                         name="sed_small")
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 100], r_min=6.0)
+    assert_links_after_injection(gpu, ob, wl, w, o.particles())
+
+
+# ------------------------------------------------------------------ boundary behaviour
+
+def test_error_codes(gpu, wl):
+    p = wl.default_params()
+    p.update(max_particles=2, max_links_per_particle=wl.max_links_for_diameter(20.0))
+    s = gpu.Simulation(64, 64, p)
+    one = dict(diam=np.array([20.0]), rho_ratio=np.array([1.5]), T_w=np.array([1.0]))
+    with pytest.raises(gpu.LbmError) as e:      # touches the wall
+        s.add_particles(x=np.array([5.0]), y=np.array([30.0]), **one)
+    assert e.value.code == gpu.LBM_E_ARG
+    s.add_particles(x=np.array([30.0]), y=np.array([30.0]), **one)
+    with pytest.raises(gpu.LbmError) as e:      # overlaps the first
+        s.add_particles(x=np.array([40.0]), y=np.array([30.0]), **one)
+    assert e.value.code == gpu.LBM_E_ARG
+    with pytest.raises(gpu.LbmError) as e:      # diameter too large for the link capacity
+        s.add_particles(x=np.array([30.0]), y=np.array([30.0]), diam=np.array([40.0]),
+                        rho_ratio=np.array([1.5]), T_w=np.array([1.0]))
+    assert e.value.code == gpu.LBM_E_CAPACITY
+    s.step(1)
+    with pytest.raises(gpu.LbmError) as e:      # no insertion mid-run
+        s.add_particles(x=np.array([10.0]), y=np.array([52.0]), **one)
+    assert e.value.code == gpu.LBM_E_STATE
+    with pytest.raises(gpu.LbmError) as e:
+        s.set_temperature(np.zeros((64, 64)))
+    assert e.value.code == gpu.LBM_E_STATE
+    assert len(s.particles()["x"]) == 1
+    # no particles at all: empty link list, empty particle arrays
+    s2 = gpu.Simulation(32, 32, wl.default_params())
+    assert len(s2.links()["q"]) == 0 and len(s2.particles()["x"]) == 0
+    s2.step(3)
