@@ -79,7 +79,10 @@ def assert_particles_close(gpu, ora, r_min, tol=PARTICLE_TOL, steps=1):
     # rim speed U / r, not the noise itself
     om_scale = max(float(np.abs(ora["omega"]).max()), vel_scale / r_min)
     th_scale = max(float(np.abs(ora["theta"]).max()), om_scale * max(steps, 1))
-    f_scale = max(float(np.abs(ora["Fx"]).max()), float(np.abs(ora["Fy"]).max()), 1e-30)
+    # the hydrodynamic force is a cancelling sum of ~20 r link terms of size ~ w_i rho0 ~ 0.1; on a
+    # particle at rest in fluid at rest it is pure round-off (1e-18), which has no scale of its
+    # own: floor = 1e-6 r (lattice units, rho0 = 1), i.e. an absolute tolerance of 1e-15 r
+    f_scale = max(float(np.abs(ora["Fx"]).max()), float(np.abs(ora["Fy"]).max()), 1e-6 * r_min)
     t_scale = max(float(np.abs(ora["Tz"]).max()), f_scale * r_min)
     for k, s in (("x", pos_scale), ("y", pos_scale), ("ux", vel_scale), ("uy", vel_scale),
                  ("omega", om_scale), ("theta", th_scale), ("Fx", f_scale), ("Fy", f_scale),

@@ -77,7 +77,7 @@ def test_periodic_poiseuille(gpu, ob, wl):
     w = wl.Workload("poiseuille", 20, 33, p, 200, 200)
     g, o, _ = run_and_compare(gpu, ob, w, [1, 200])
     # and the GPU itself against the closed form after convergence (independent of the oracle)
-    g.step(6000)
+    g.step(40000)
     ux = g.fields()["ux"]
     jj = np.arange(33, dtype=np.float64)
     exact = 1e-6 / (2 * 0.1) * (jj + 0.5) * (33 - 0.5 - jj)
