@@ -240,7 +240,7 @@ def main():
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    achieved = alg_bytes / sc_avg_s / 1e9
+    achieved = alg_bytes / sc_avg_s / 1e9 if sc_avg_s > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": "k_stream_collide", "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": read_traffic(),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
