@@ -250,7 +250,7 @@ __global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __r
 void launch_bounce_back(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->flag, h->la, h->pa, h->cur, h->C);
+  k_bounce_back<<<h->np, BT, 0, h->chain>>>(h->A, h->flag, h->la, h->pa, h->cur, h->C);
 }
 
 void launch_refill(lbm* h) {
@@ -258,9 +258,9 @@ void launch_refill(lbm* h) {
   int blocks = (h->np * 4 + 127) / 128;   // a handful of newborn nodes per particle and step
   if (blocks > 1184) blocks = 1184;
   h->launches++;
-  k_refill<<<blocks, 128, 0, h->stream>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
+  k_refill<<<blocks, 128, 0, h->chain>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
                                           h->newborn_count, h->newborn_cap, h->pa, h->cur, h->C);
   h->launches++;
-  k_newborn_clear<<<blocks, 128, 0, h->stream>>>(h->flag, h->newborn_node, h->newborn_count,
+  k_newborn_clear<<<blocks, 128, 0, h->chain>>>(h->flag, h->newborn_node, h->newborn_count,
                                                  h->newborn_cap);
 }

@@ -19,7 +19,7 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "cells_integrate",
-    "flags_uncover", "flags_cover", "refill", "init_collide"};
+    "flags_uncover", "flags_cover", "refill", "init_collide", "stream_collide_near"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -77,6 +77,8 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   double* A = c.take<double>(14 * (size_t)L.ps);
   double* B = c.take<double>(14 * (size_t)L.ps);
   unsigned char* flag = c.take<unsigned char>((size_t)L.px * ny);
+  unsigned char* zs0 = c.take<unsigned char>((size_t)L.px * ny);
+  unsigned char* zs1 = c.take<unsigned char>((size_t)L.px * ny);
   int* owner = c.take<int>((size_t)L.px * ny);
   ParticleArrays pa;
   for (int b = 0; b < 2; ++b) {
@@ -113,6 +115,8 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
     h->A = A;
     h->B = B;
     h->flag = flag;
+    h->zstamp[0] = zs0;
+    h->zstamp[1] = zs1;
     h->owner = owner;
     h->pa = pa;
     h->la = la;
@@ -175,22 +179,24 @@ void fill_const(lbm* h) {
 struct Timed {
   lbm* h;
   int k;
+  cudaStream_t st;
   bool on;
-  Timed(lbm* h_, int k_) : h(h_), k(k_), on(false) {
+  Timed(lbm* h_, int k_, cudaStream_t st_) : h(h_), k(k_), st(st_), on(false) {
     if (h->prof_on && h->ev_n[k] < LBM_PROFILE_MAX_SAMPLES) {
       on = true;
-      cudaEventRecord(h->ev0[k][h->ev_n[k]], h->stream);
+      cudaEventRecord(h->ev0[k][h->ev_n[k]], st);
     }
   }
   ~Timed() {
     if (on) {
-      cudaEventRecord(h->ev1[k][h->ev_n[k]], h->stream);
+      cudaEventRecord(h->ev1[k][h->ev_n[k]], st);
       h->ev_n[k]++;
     }
   }
 };
 
 int check_status(lbm* h) {
+  if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
   CUDA_OK(h, cudaMemcpyAsync(h->status_host, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
@@ -204,7 +210,7 @@ int check_status(lbm* h) {
 
 void prime(lbm* h) {
   if (h->primed) return;
-  Timed t(h, K_INIT);
+  Timed t(h, K_INIT, h->stream);
   launch_init_collide(h, h->A);
   h->primed = 1;
 }
@@ -255,12 +261,31 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     delete h;
     return LBM_E_CUDA;
   }
+  // second stream for the particle chain: highest priority, so
+  // that its short latency-bound kernels get SM slots as CTAs of the far pass retire
+  h->chain = h->stream;
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
+        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess) {
+      h->overlap = 1;
+      h->chain = h->chain_own;
+    } else {
+      cudaGetLastError();
+      h->chain_own = nullptr;
+    }
+  }
   // initial state: fluid everywhere, f = f_eq(rho0, 0), g = g_eq(T0, 0)
   const size_t nn = (size_t)h->px * ny;
   cudaMemsetAsync(h->flag, 0, nn, h->stream);
+  cudaMemsetAsync(h->zstamp[0], 0, nn, h->stream);
+  cudaMemsetAsync(h->zstamp[1], 0, nn, h->stream);
   cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
   cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
   cudaMemsetAsync(h->newborn_count, 0, sizeof(int), h->stream);
+  if (h->max_cells) cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->max_cells, h->stream);
   cudaMemsetAsync(h->B, 0, sizeof(double) * 14 * (size_t)h->ps, h->stream);
   launch_set_equilibrium(h);
   e = cudaStreamSynchronize(h->stream);
@@ -383,10 +408,10 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   h->ncy = (int)std::ceil(h->ny / h->cell) + 1;
   if ((long long)h->ncx * h->ncy > h->max_cells)
     return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
-  launch_cover(h, c);   // stamp flag and owner maps (primed == 0: fixed particles too)
-  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));   // uploads done before the chain stream reads them
+  launch_cover(h, c);   // flag, owner and zone maps of step 0 (primed == 0: fixed particles too)
+  CUDA_OK(h, cudaStreamSynchronize(h->chain));
   CUDA_OK(h, cudaGetLastError());
-  (void)c;
   return LBM_OK;
 }
 
@@ -394,21 +419,49 @@ int lbm_step(lbm_t* h, int nsteps) {
   if (!h) return LBM_E_ARG;
   if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
   prime(h);
+  cudaStream_t S0 = h->stream, S1 = h->chain;
   for (int s = 0; s < nsteps; ++s) {
+    const long long t = h->steps_done;
     if (h->np > 0) {
-      { Timed t(h, K_BUILD_LINKS); launch_build_links(h); }
-      { Timed t(h, K_BOUNCE_BACK); launch_bounce_back(h); }
-      { Timed t(h, K_INTEGRATE); launch_cells_and_integrate(h); }
-      { Timed t(h, K_UNCOVER); launch_uncover(h); }
-      { Timed t(h, K_COVER); launch_cover(h, h->cur ^ 1); }
-      h->cur ^= 1;
+      // zone map of this step's parity: its stamp value wraps every 510 steps -> clear + re-mark
+      if (t >= 2 && ((t >> 1) % 255) == 0) {
+        cudaMemsetAsync(h->zstamp[t & 1], 0, (size_t)h->px * h->ny, S0);
+        launch_mark_zones(h, h->cur, t, S0);
+      }
+      if (S1 != S0) {
+        cudaEventRecord(h->ev_fork, S0);
+        cudaStreamWaitEvent(S1, h->ev_fork, 0);
+      }
     }
-    { Timed t(h, K_STREAM_COLLIDE); launch_stream_collide(h); }
-    if (h->np > 0) { Timed t(h, K_REFILL); launch_refill(h); }
+    // far pass: independent of the particle chain, runs concurrently with it
+    { Timed tm(h, K_STREAM_COLLIDE, S0); launch_stream_collide_far(h); }
+    if (h->np > 0) {
+      { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h); }
+      { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h); }
+      { Timed tm(h, K_INTEGRATE, S1); launch_cells_and_integrate(h); }
+      { Timed tm(h, K_UNCOVER, S1); launch_uncover(h); }
+      { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1); }
+      h->cur ^= 1;
+      { Timed tm(h, K_STREAM_COLLIDE_NEAR, S1); launch_stream_collide_near(h); }
+      { Timed tm(h, K_REFILL, S1); launch_refill(h); }
+      if (S1 != S0) {
+        cudaEventRecord(h->ev_join, S1);
+        cudaStreamWaitEvent(S0, h->ev_join, 0);
+      }
+    }
     std::swap(h->A, h->B);
     h->steps_done++;
   }
   return check_status(h);
+}
+
+int lbm_set_overlap(lbm_t* h, int on) {
+  if (!h) return LBM_E_ARG;
+  cudaStreamSynchronize(h->stream);
+  if (h->chain_own) cudaStreamSynchronize(h->chain_own);
+  h->overlap = (on && h->chain_own) ? 1 : 0;
+  h->chain = h->overlap ? h->chain_own : h->stream;
+  return LBM_OK;
 }
 
 int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, double* f, double* g,
@@ -480,6 +533,7 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
   *n = 0;
   if (h->np == 0) return LBM_OK;
   launch_build_links(h);
+  if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
   std::vector<int> count(h->np);
   CUDA_OK(h, cudaMemcpyAsync(count.data(), h->la.count, h->np * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   int rc = check_status(h);
@@ -537,6 +591,7 @@ const char* lbm_profile_kernel_name(int kernel_id) {
 int lbm_profile_get(lbm_t* h, int kernel_id, double* total_ms, long long* launches) {
   if (!h || kernel_id < 0 || kernel_id >= K_COUNT) return LBM_E_ARG;
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
   double tot = 0.0;
   const int n = h->ev0[kernel_id] ? h->ev_n[kernel_id] : 0;
   for (int s = 0; s < n; ++s) {
@@ -554,6 +609,12 @@ long long lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : -1; }
 int lbm_destroy(lbm_t* h) {
   if (!h) return LBM_OK;
   cudaStreamSynchronize(h->stream);
+  if (h->chain_own) {
+    cudaStreamSynchronize(h->chain_own);
+    cudaStreamDestroy(h->chain_own);
+    cudaEventDestroy(h->ev_fork);
+    cudaEventDestroy(h->ev_join);
+  }
   for (int k = 0; k < K_COUNT; ++k)
     if (h->ev0[k]) {
       for (int s = 0; s < LBM_PROFILE_MAX_SAMPLES; ++s) {

@@ -7,6 +7,11 @@
 //   flag : 1 byte/node, 0 fluid, 1 solid, 2 newborn (solid at t, fluid at t+1; only between the
 //          flag update and the refill kernel of one step)
 //   owner: int32/node, id of the lowest-numbered particle covering the node, OWNER_NONE = fluid
+//   zstamp[2]: 1 byte/node each, double-buffered by step parity: node x lies in some particle's
+//          effective zone at step t  <=>  zstamp[t&1][x] == zone_stamp(t).  Nodes outside every
+//          zone ("far") cannot be solid, cannot change flag and do not pull from a solid slot, so
+//          the far pass of the lattice kernel is independent of the whole particle chain of the
+//          step and overlaps with it on a second stream.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -26,8 +31,15 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
-  K_INIT, K_COUNT
+  K_INIT, K_STREAM_COLLIDE_NEAR, K_COUNT
 };
+
+// stamp of step t in zstamp[t&1]: 1..255, each value used once per array and epoch of 510 steps;
+// the array is cleared and re-marked when the value wraps (lbm_capi.cu), so a stale stamp never
+// equals the current one
+__host__ __device__ inline unsigned char zone_stamp(long long t) {
+  return (unsigned char)(((t >> 1) % 255) + 1);
+}
 
 // constants every kernel needs; passed by value (lands in the constant bank)
 struct LbmConst {
@@ -65,9 +77,14 @@ struct lbm {
   long long ps;
   lbm_params P;
   LbmConst C;
-  cudaStream_t stream;
+  cudaStream_t stream;       // the caller's stream: far pass of the lattice kernel, set-up, read-out
+  cudaStream_t chain;        // particle chain + near pass (own high-priority stream when overlapping)
+  cudaStream_t chain_own;    // the stream we created (NULL if creation failed)
+  cudaEvent_t ev_fork, ev_join;
+  int overlap;               // 1: chain runs on `chain_own` concurrently with the far pass
   double *A, *B;             // 14 planes each
   unsigned char* flag;
+  unsigned char* zstamp[2];
   int* owner;
   ParticleArrays pa;
   LinkArrays la;
@@ -98,7 +115,8 @@ struct lbm {
 
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
-void launch_stream_collide(lbm* h);
+void launch_stream_collide_far(lbm* h);    // on h->stream
+void launch_stream_collide_near(lbm* h);   // on h->chain; zones of the positions in buffer cur^1
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
 void launch_set_equilibrium(lbm* h);
@@ -108,6 +126,7 @@ void launch_build_links(lbm* h);
 void launch_cells_and_integrate(lbm* h);
 void launch_uncover(lbm* h);
 void launch_cover(lbm* h, int which_buffer);
+void launch_mark_zones(lbm* h, int which_buffer, long long step, cudaStream_t st);
 // bounce_back.cu
 void launch_bounce_back(lbm* h);
 void launch_refill(lbm* h);

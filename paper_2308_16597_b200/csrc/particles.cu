@@ -25,6 +25,14 @@ __device__ __forceinline__ bool inside_disc(double xi, double yj, double xc, dou
   return dx * dx + dy * dy <= r * r;
 }
 
+// "Near" nodes of a particle: the disc itself plus every node that can have a solid node of it
+// among its 8 neighbours (|x - x_c| <= r + sqrt2 < r + 1.5).  Only these depend on the particle
+// chain within a step; all other nodes are left to the far pass of the lattice kernel.
+__device__ __forceinline__ bool near_disc(double xi, double yj, double xc, double yc, double r) {
+  const double dx = xi - xc, dy = yj - yc, rr = r + 1.5;
+  return dx * dx + dy * dy <= rr * rr;
+}
+
 // q = |x_f - x_w|/|x_f - x_b|: smaller root of |x_f + t e - x_c|^2 = r^2
 __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc, double yc, double r) {
   const double ex = (double)p_ex[al], ey = (double)p_ey[al];
@@ -53,7 +61,7 @@ __global__ void __launch_bounds__(PT)
 k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
               const double* __restrict__ pr, const unsigned char* __restrict__ flag,
               const int* __restrict__ owner, LinkArrays la, int* __restrict__ status,
-              const LbmConst c) {
+              int* __restrict__ nb_count, const LbmConst c) {
   const int p = blockIdx.x;
   const double xc = px_[p], yc = py_[p], r = pr[p];
   int i0, i1, j0, j1;
@@ -62,7 +70,10 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   __shared__ int s_warp[PT / 32];
   __shared__ int s_running;
-  if (threadIdx.x == 0) s_running = 0;
+  if (threadIdx.x == 0) {
+    s_running = 0;
+    if (p == 0) *nb_count = 0;   // the newborn list of the previous step has been consumed
+  }
   __syncthreads();
   const long long base = (long long)p * la.cap;
   const double rfar = (r + 1.5) * (r + 1.5);   // beyond this no neighbour can be inside the disc
@@ -107,14 +118,14 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
     int off = s_running + woff + incl - cnt;
     if (cnt) {
       if (off + cnt <= la.cap) {
-#pragma unroll
-        for (int al = 1; al <= 8; ++al)
-          if (mask & (1u << al)) {
-            la.node[base + off] = j * c.px + i;
-            la.dir[base + off] = (unsigned char)al;
-            la.q[base + off] = link_q((double)i, (double)j, al, xc, yc, r);
-            ++off;
-          }
+        const int node = j * c.px + i;
+        while (mask) {                         // compaction only; q follows in a balanced pass
+          const int al = __ffs(mask) - 1;
+          mask &= mask - 1;
+          la.node[base + off] = node;
+          la.dir[base + off] = (unsigned char)al;
+          ++off;
+        }
       } else {
         atomicOr(status, ST_LINK_OVERFLOW);
       }
@@ -123,7 +134,14 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
     if (threadIdx.x == 0) s_running += btotal;
     __syncthreads();
   }
-  if (threadIdx.x == 0) la.count[p] = min(s_running, la.cap);
+  // q for the compacted links, one link per thread (no divergence over directions)
+  const int nl = min(s_running, la.cap);
+  for (int s = threadIdx.x; s < nl; s += PT) {
+    const int node = la.node[base + s];
+    const int al = la.dir[base + s];
+    la.q[base + s] = link_q((double)(node % c.px), (double)(node / c.px), al, xc, yc, r);
+  }
+  if (threadIdx.x == 0) la.count[p] = nl;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -240,8 +258,10 @@ __global__ void k_integrate(ParticleArrays pa, int cur, int np, double cell, int
 __global__ void __launch_bounds__(PT)
 k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __restrict__ owner,
           int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
-          int* __restrict__ status, const LbmConst c) {
+          int* __restrict__ status, int* __restrict__ cell_count, int ncells, const LbmConst c) {
   const int p = blockIdx.x;
+  // the repulsion grid of this step has been consumed by k_integrate: zero it for the next step
+  for (int k = p * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count[k] = 0;
   if (pa.fixed[p]) return;
   const int nxt = cur ^ 1;
   const double xo = pa.x[cur][p], yo = pa.y[cur][p], r = pa.r[p];
@@ -269,12 +289,14 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
 }
 
 // Phase B: every node inside the disc at the position in buffer `buf` is solid; the lowest
-// particle id wins the owner map (same rule as a from-scratch recomputation).
+// particle id wins the owner map (same rule as a from-scratch recomputation).  Also stamps the
+// particle's effective zone at that position into the zone map of the step that will use it.
 __global__ void __launch_bounds__(PT)
 k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ flag,
-        int* __restrict__ owner, const LbmConst c) {
+        int* __restrict__ owner, unsigned char* __restrict__ zs, unsigned char stamp,
+        const LbmConst c) {
   const int p = blockIdx.x;
-  if (skip_fixed && pa.fixed[p]) return;
+  const bool stamp_only = skip_fixed && pa.fixed[p];
   const double xn = pa.x[buf][p], yn = pa.y[buf][p], r = pa.r[p];
   int i0, i1, j0, j1;
   zone_of(xn, yn, r, i0, i1, j0, j1);
@@ -282,11 +304,30 @@ k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ 
   for (int t = threadIdx.x; t < total; t += PT) {
     const int i = i0 + t % W, j = j0 + t / W;
     if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    if (!inside_disc((double)i, (double)j, xn, yn, r)) continue;
     const long long x = (long long)j * c.px + i;
+    if (!near_disc((double)i, (double)j, xn, yn, r)) continue;
+    zs[x] = stamp;
+    if (stamp_only || !inside_disc((double)i, (double)j, xn, yn, r)) continue;
     if (owner[x] == p) continue;
     const int prev = atomicMin(&owner[x], p);
     if (prev != p) flag[x] = 1;
+  }
+}
+
+// zone stamps only (epoch reset of a zone map, see zone_stamp())
+__global__ void __launch_bounds__(PT)
+k_mark_zones(const double* __restrict__ px_, const double* __restrict__ py_,
+             const double* __restrict__ pr, unsigned char* __restrict__ zs, unsigned char stamp,
+             const LbmConst c) {
+  const int p = blockIdx.x;
+  const double xc = px_[p], yc = py_[p], r = pr[p];
+  int i0, i1, j0, j1;
+  zone_of(xc, yc, r, i0, i1, j0, j1);
+  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
+  for (int t = threadIdx.x; t < total; t += PT) {
+    const int i = i0 + t % W, j = j0 + t / W;
+    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
+    if (near_disc((double)i, (double)j, xc, yc, r)) zs[(long long)j * c.px + i] = stamp;
   }
 }
 
@@ -295,37 +336,46 @@ k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ 
 void launch_build_links(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_build_links<<<h->np, PT, 0, h->stream>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->pa.r, h->flag,
-                                             h->owner, h->la, h->status_dev, h->C);
+  k_build_links<<<h->np, PT, 0, h->chain>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->pa.r, h->flag,
+                                             h->owner, h->la, h->status_dev, h->newborn_count, h->C);
 }
 
 void launch_cells_and_integrate(lbm* h) {
   if (h->np == 0) return;
-  cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->ncx * h->ncy, h->stream);
   const int blocks = (h->np + 127) / 128;
   h->launches++;
-  k_cells_build<<<blocks, 128, 0, h->stream>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->np, h->cell,
+  k_cells_build<<<blocks, 128, 0, h->chain>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->np, h->cell,
                                                h->ncx, h->ncy, h->cell_count, h->cell_items,
                                                h->status_dev);
   h->launches++;
-  k_integrate<<<blocks, 128, 0, h->stream>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
+  k_integrate<<<blocks, 128, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
                                              h->cell_count, h->cell_items, h->status_dev, h->C);
 }
 
 void launch_uncover(lbm* h) {
   if (h->np == 0) return;
-  cudaMemsetAsync(h->newborn_count, 0, sizeof(int), h->stream);
   h->launches++;
-  k_uncover<<<h->np, PT, 0, h->stream>>>(h->pa, h->cur, h->flag, h->owner, h->newborn_node,
+  k_uncover<<<h->np, PT, 0, h->chain>>>(h->pa, h->cur, h->flag, h->owner, h->newborn_node,
                                          h->newborn_pid, h->newborn_count, h->newborn_cap,
-                                         h->status_dev, h->C);
+                                         h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
 }
 
 void launch_cover(lbm* h, int which_buffer) {
   if (h->np == 0) return;
   // after add_particles every particle (fixed ones too) must be stamped; during stepping the
   // fixed ones never move
+  // The positions in `which_buffer` are those of step `next`: during stepping next = steps_done+1
+  // (called before steps_done is incremented), at set-up next = steps_done (= 0).
   const int skip_fixed = h->primed ? 1 : 0;
+  const long long next = h->primed ? h->steps_done + 1 : h->steps_done;
   h->launches++;
-  k_cover<<<h->np, PT, 0, h->stream>>>(h->pa, which_buffer, skip_fixed, h->flag, h->owner, h->C);
+  k_cover<<<h->np, PT, 0, h->chain>>>(h->pa, which_buffer, skip_fixed, h->flag, h->owner,
+                                      h->zstamp[next & 1], zone_stamp(next), h->C);
+}
+
+void launch_mark_zones(lbm* h, int which_buffer, long long step, cudaStream_t st) {
+  if (h->np == 0) return;
+  h->launches++;
+  k_mark_zones<<<h->np, PT, 0, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r,
+                                     h->zstamp[step & 1], zone_stamp(step), h->C);
 }

@@ -55,14 +55,10 @@ __device__ __forceinline__ void pull_boundary(const double* __restrict__ A, cons
   }
 }
 
-__global__ void __launch_bounds__(SC_THREADS)
-k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
-                 const unsigned char* __restrict__ flag, const LbmConst c) {
-  const int i = blockIdx.x * SC_THREADS + threadIdx.x;
-  const int j = blockIdx.y;
-  if (i >= c.nx) return;
+// one lattice update of node (i, j): pull, collide, store
+__device__ __forceinline__ void update_node(const double* __restrict__ A, double* __restrict__ B,
+                                            const LbmConst& c, int i, int j) {
   const long long x = (long long)j * c.px + i;
-  if (flag[x] != 0) return;   // solid or newborn: not touched here
   double f[9], g[5];
   if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
     const double* __restrict__ F = A + x;
@@ -91,6 +87,45 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   for (int k = 0; k < 9; ++k) O[k * c.ps] = f[k];
 #pragma unroll
   for (int k = 0; k < 5; ++k) O[(9 + k) * c.ps] = g[k];
+}
+
+// FAR pass: every node outside all particle zones of this step (zstamp != stamp).  Such a node is
+// fluid, stays fluid, and none of its upstream neighbours is a solid slot, so this kernel depends
+// on nothing the particle chain of the step produces and runs concurrently with it.
+__global__ void __launch_bounds__(SC_THREADS)
+k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
+                 const unsigned char* __restrict__ zstamp, const unsigned char stamp,
+                 const LbmConst c) {
+  const int i = blockIdx.x * SC_THREADS + threadIdx.x;
+  const int j = blockIdx.y;
+  if (i >= c.nx) return;
+  if (zstamp[(long long)j * c.px + i] == stamp) return;   // near: left to k_stream_collide_near
+  update_node(A, B, c, i, j);
+}
+
+// NEAR pass: one CTA per particle over its effective zone [INT(xc-r)-1, INT(xc+r)+1]^2 at the
+// positions of time t, after the flag update: near nodes (zone stamp of this step) that are fluid
+// (flag 0) are updated; solid and newborn nodes are not.  Near sets of neighbouring particles may
+// overlap: both CTAs then compute and store bit-identical values (same inputs, same code), which
+// is benign.
+__global__ void __launch_bounds__(SC_THREADS)
+k_stream_collide_near(const double* __restrict__ A, double* __restrict__ B,
+                      const unsigned char* __restrict__ flag,
+                      const unsigned char* __restrict__ zstamp, const unsigned char stamp,
+                      const double* __restrict__ px_, const double* __restrict__ py_,
+                      const double* __restrict__ pr, const LbmConst c) {
+  const int p = blockIdx.x;
+  const double xc = px_[p], yc = py_[p], r = pr[p];
+  const int i0 = (int)floor(xc - r) - 1, i1 = (int)floor(xc + r) + 1;
+  const int j0 = (int)floor(yc - r) - 1, j1 = (int)floor(yc + r) + 1;
+  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
+  for (int t = threadIdx.x; t < total; t += SC_THREADS) {
+    const int i = i0 + t % W, j = j0 + t / W;
+    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
+    const long long x = (long long)j * c.px + i;
+    if (zstamp[x] != stamp || flag[x] != 0) continue;
+    update_node(A, B, c, i, j);
+  }
 }
 
 // first step only: A holds the PRE-collision initial state f(x,0); collide it (in place when
@@ -178,10 +213,19 @@ inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1
 
 } // namespace
 
-void launch_stream_collide(lbm* h) {
+void launch_stream_collide_far(lbm* h) {
   h->launches++;
   k_stream_collide<<<grid_rows(h->nx, h->ny, SC_THREADS), SC_THREADS, 0, h->stream>>>(
-      h->A, h->B, h->flag, h->C);
+      h->A, h->B, h->zstamp[h->steps_done & 1], zone_stamp(h->steps_done), h->C);
+}
+
+void launch_stream_collide_near(lbm* h) {
+  if (h->np == 0) return;
+  const int old = h->cur ^ 1;   // positions at time t (the integrator has already flipped cur)
+  h->launches++;
+  k_stream_collide_near<<<h->np, SC_THREADS, 0, h->chain>>>(
+      h->A, h->B, h->flag, h->zstamp[h->steps_done & 1], zone_stamp(h->steps_done), h->pa.x[old],
+      h->pa.y[old], h->pa.r, h->C);
 }
 
 void launch_init_collide(lbm* h, double* dst) {

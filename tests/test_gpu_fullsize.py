@@ -1,0 +1,144 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(Simulation.from_workload(config(k)), lbm_step on the current torch stream).
+
+* configs 1 and 2: the full 100-step parity horizon against the oracle (SURVEY 8(c) protocol).
+* config 3 (the benched workload): links bit-exact on the full 4,800-particle set, full-field and
+  particle parity over a short horizon the oracle can afford (3.6 s per step), and a sampled
+  one-step check deep into the run: for sampled nodes the oracle's per-node collision is applied
+  to the populations pulled from the GPU state at step s and compared with the GPU state at s+1.
+* config 4 (8192^2, 20,000 particles): links bit-exact, flag map against an independent numpy
+  rasterisation of the discs, 2-step macroscopic + particle parity, sampled one-step check.
+"""
+import numpy as np
+import pytest
+
+from parity import (FIELD_TOL, assert_fields_close, assert_links_equal, assert_particles_close)
+
+pytestmark = pytest.mark.gpu
+
+EX = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1])
+EY = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1])
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2308_16597_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def host_gb_free():
+    import psutil
+    return psutil.virtual_memory().available / 2 ** 30
+
+
+def sampled_one_step_check(g, ob, w, nsamples=1500, seed=0):
+    """State s -> s+1 on sampled nodes whose whole pull stencil is plain fluid at both times (no
+    wall, no particle within 2 nodes): f_k(x, s+1) must equal collide(pull of f+(., s))."""
+    a = g.fields(populations=True)
+    g.step(1)
+    b = g.fields(populations=True)
+    ny, nx = a["flag"].shape
+    solid = (a["flag"] != 0) | (b["flag"] != 0)
+    near = solid.copy()
+    for dy in (-2, -1, 0, 1, 2):          # dilate by 2 (np.roll wraps; the rim is excluded below)
+        for dx in (-2, -1, 0, 1, 2):
+            near |= np.roll(np.roll(solid, dy, axis=0), dx, axis=1)
+    near[:2, :] = near[-2:, :] = True
+    near[:, :2] = near[:, -2:] = True
+    jj, ii = np.nonzero(~near)
+    rng = np.random.default_rng(seed)
+    pick = rng.choice(len(jj), size=min(nsamples, len(jj)), replace=False)
+    worst_f = worst_g = 0.0
+    fs = float(np.abs(b["f"]).max())
+    gs = max(float(np.abs(b["g"]).max()), 1e-30)
+    for t in pick:
+        j, i = int(jj[t]), int(ii[t])
+        f = np.array([a["f"][k, j - EY[k], i - EX[k]] for k in range(9)])
+        gg = np.array([a["g"][k, j - EY[k], i - EX[k]] for k in range(5)])
+        fo, go = ob.collide_node(w.params, f, gg)
+        worst_f = max(worst_f, float(np.abs(fo - b["f"][:, j, i]).max()) / fs)
+        worst_g = max(worst_g, float(np.abs(go - b["g"][:, j, i]).max()) / gs)
+    assert worst_f <= FIELD_TOL and worst_g <= FIELD_TOL, (worst_f, worst_g)
+    return len(pick)
+
+
+def numpy_flags(w):
+    """Independent rasterisation: node solid iff dx*dx + dy*dy <= r*r for some particle."""
+    flag = np.zeros((w.ny, w.nx), dtype=np.uint8)
+    P = w.particles
+    for x, y, d in zip(P["x"], P["y"], P["diam"]):
+        r = 0.5 * d
+        i0, i1 = max(int(np.floor(x - r)) - 1, 0), min(int(np.floor(x + r)) + 1, w.nx - 1)
+        j0, j1 = max(int(np.floor(y - r)) - 1, 0), min(int(np.floor(y + r)) + 1, w.ny - 1)
+        I, J = np.meshgrid(np.arange(i0, i1 + 1, dtype=np.float64),
+                           np.arange(j0, j1 + 1, dtype=np.float64))
+        dx, dy = I - x, J - y
+        flag[j0:j1 + 1, i0:i1 + 1] |= (dx * dx + dy * dy <= r * r).astype(np.uint8)
+    return flag
+
+
+def test_config1_full_parity_100_steps(gpu, ob, wl):
+    w = wl.config(1)
+    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+    g.step(w.parity_steps)
+    o.step(w.parity_steps)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    assert sampled_one_step_check(g, ob, w, 500) == 500
+
+
+def test_config2_full_parity_100_steps(gpu, ob, wl):
+    w = wl.config(2)
+    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+    assert_links_equal(g.links(), o.links())
+    g.step(w.parity_steps)
+    o.step(w.parity_steps)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    assert_particles_close(g.particles(), o.particles(), r_min=10.0, steps=w.parity_steps)
+    # links on the oracle's state after the run, injected into fresh simulations
+    po = o.particles()
+    parts = dict(w.particles)
+    parts.update(x=po["x"], y=po["y"], ux=po["ux"], uy=po["uy"], omega=po["omega"])
+    w2 = wl.Workload("config2_inj", w.nx, w.ny, w.params, 1, 1, particles=parts)
+    assert_links_equal(gpu.Simulation.from_workload(w2).links(),
+                       ob.OracleSim.from_workload(w2).links())
+
+
+def test_config3_full_size(gpu, ob, wl):
+    if host_gb_free() < 24:
+        pytest.skip("needs ~20 GB of host memory for the oracle's 4000^2 arrays")
+    w = wl.config(3)
+    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+    Lg = g.links()
+    assert_links_equal(Lg, o.links())
+    assert len(Lg["q"]) > 4800 * 150
+    assert np.array_equal(g.fields()["flag"], numpy_flags(w))
+    g.step(6)
+    o.step(6)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    assert_particles_close(g.particles(), o.particles(), r_min=10.0, steps=6)
+    del o
+    # deep into the run, in bench.py's regime
+    g.step(300)
+    assert sampled_one_step_check(g, ob, w, 1500) == 1500
+    p = g.particles()
+    assert all(np.isfinite(v).all() for v in p.values())
+    assert (p["uy"] < 0).mean() > 0.9          # they are settling
+
+
+def test_config4_full_size(gpu, ob, wl):
+    if host_gb_free() < 90:
+        pytest.skip("needs ~70 GB of host memory for the oracle's 8192^2 arrays")
+    w = wl.config(4)
+    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+    assert_links_equal(g.links(), o.links())
+    assert np.array_equal(g.fields()["flag"], numpy_flags(w))
+    g.step(2)
+    o.step(2)
+    assert_fields_close(g.fields(), o.fields(), populations=False)
+    assert_particles_close(g.particles(), o.particles(), r_min=6.0, steps=2)
+    del o
+    g.step(50)
+    assert sampled_one_step_check(g, ob, w, 800) == 800
