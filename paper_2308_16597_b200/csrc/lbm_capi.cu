@@ -135,7 +135,7 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
 bool params_ok(int nx, int ny, const lbm_params* p) {
   return p && nx >= 4 && ny >= 4 && nx <= 46000 && ny <= 46000 && p->nu > 0.0 && p->kappa > 0.0 &&
          p->kappa < 0.144 && p->rho0 > 0.0 && p->max_particles >= 0 &&
-         p->max_links_per_particle >= 0 && p->rep_s > 0.0 && p->rep_eps > 0.0 &&
+         p->max_links_per_particle >= 0 && p->max_links_per_particle <= 12000 && p->rep_s > 0.0 && p->rep_eps > 0.0 &&
          p->rep_power >= 1 && std::isfinite(p->nu) && std::isfinite(p->kappa);
 }
 

@@ -41,6 +41,23 @@ __host__ __device__ inline unsigned char zone_stamp(long long t) {
   return (unsigned char)(((t >> 1) % 255) + 1);
 }
 
+// "Near" nodes of a particle: the disc itself plus every node that can have one of its solid nodes
+// among its 8 neighbours (|x - x_c| <= r + sqrt2 < r + 1.5).  Written with explicit round-to-nearest
+// intrinsics so that every translation unit (with or without -fmad) takes the same decision: the
+// zone-stamp writer (particles.cu) and the near pass (stream_collide.cu) must agree node by node.
+__device__ __forceinline__ bool near_disc(double xi, double yj, double xc, double yc, double r) {
+  const double dx = __dsub_rn(xi, xc), dy = __dsub_rn(yj, yc), rr = __dadd_rn(r, 1.5);
+  return __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)) <= __dmul_rn(rr, rr);
+}
+
+// effective zone of PAPER.md:258 (the narrower reading of DESIGN.md): [INT(xc-r)-1, INT(xc+r)+1]^2
+__device__ __forceinline__ void zone_of(double xc, double yc, double r, int& i0, int& i1, int& j0, int& j1) {
+  i0 = (int)floor(__dsub_rn(xc, r)) - 1;
+  i1 = (int)floor(__dadd_rn(xc, r)) + 1;
+  j0 = (int)floor(__dsub_rn(yc, r)) - 1;
+  j1 = (int)floor(__dadd_rn(yc, r)) + 1;
+}
+
 // constants every kernel needs; passed by value (lands in the constant bank)
 struct LbmConst {
   int nx, ny, px;          // lattice size, row pitch (doubles)

@@ -25,14 +25,6 @@ __device__ __forceinline__ bool inside_disc(double xi, double yj, double xc, dou
   return dx * dx + dy * dy <= r * r;
 }
 
-// "Near" nodes of a particle: the disc itself plus every node that can have a solid node of it
-// among its 8 neighbours (|x - x_c| <= r + sqrt2 < r + 1.5).  Only these depend on the particle
-// chain within a step; all other nodes are left to the far pass of the lattice kernel.
-__device__ __forceinline__ bool near_disc(double xi, double yj, double xc, double yc, double r) {
-  const double dx = xi - xc, dy = yj - yc, rr = r + 1.5;
-  return dx * dx + dy * dy <= rr * rr;
-}
-
 // q = |x_f - x_w|/|x_f - x_b|: smaller root of |x_f + t e - x_c|^2 = r^2
 __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc, double yc, double r) {
   const double ex = (double)p_ex[al], ey = (double)p_ey[al];
@@ -46,13 +38,6 @@ __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc
   if (t < 0.0) t = 0.0;
   if (t > 1.0) t = 1.0;
   return t;
-}
-
-__device__ __forceinline__ void zone_of(double xc, double yc, double r, int& i0, int& i1, int& j0, int& j1) {
-  i0 = (int)floor(xc - r) - 1;
-  i1 = (int)floor(xc + r) + 1;
-  j0 = (int)floor(yc - r) - 1;
-  j1 = (int)floor(yc + r) + 1;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -174,48 +159,87 @@ __device__ __forceinline__ double repulsion_mag(double C, const LbmConst& c, dou
 
 // Eqs. (7), (8), (15): total force = hydrodynamic + weight - buoyancy + repulsion; one step of
 // U' = U + F/M, x' = x + (U + U')/2 (DESIGN.md reading), same for Omega, theta.
-__global__ void k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
-                            const int* __restrict__ cell_count, const int* __restrict__ cell_items,
-                            int* __restrict__ status, const LbmConst c) {
-  const int ia = blockIdx.x * blockDim.x + threadIdx.x;
+// One WARP per particle: the lanes fetch the candidates of the 3 x 3 cell neighbourhood in
+// parallel (one round of dependent loads instead of a serial walk), each lane evaluates one pair,
+// and the non-zero contributions are added in ascending particle id (warp min-reduction picks the
+// next one), so the sum order is fixed whatever order the cell slots were filled in.
+constexpr int IW = 4;   // warps (particles) per CTA
+__global__ void __launch_bounds__(IW * 32)
+k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
+            const int* __restrict__ cell_count, const int* __restrict__ cell_items,
+            int* __restrict__ status, const LbmConst c) {
+  const int lane = threadIdx.x & 31;
+  const int ia = blockIdx.x * IW + (threadIdx.x >> 5);
   if (ia >= np) return;
+  const unsigned FULL = 0xffffffffu;
   const int nxt = cur ^ 1;
   const double PI = 3.14159265358979323846;
   const double ax = pa.x[cur][ia], ay = pa.y[cur][ia], ar = pa.r[ia], ratio = pa.rho_ratio[ia];
   const double Ca = PI * ar * ar * (ratio * c.rho0 - c.rho0) * c.g;
   double Fx = pa.Fx[ia], Fy = pa.Fy[ia];
   Fy += -(ratio * c.rho0 - c.rho0) * PI * ar * ar * c.g;
-  // neighbours in ascending id: repeatedly pick the smallest id above the last one handled
   int ci = (int)floor(ax / cell), cj = (int)floor(ay / cell);
   ci = min(max(ci, 0), ncx - 1);
   cj = min(max(cj, 0), ncy - 1);
-  int last = -1;
-  while (true) {
-    int best = 0x7fffffff;
-    for (int b = max(cj - 1, 0); b <= min(cj + 1, ncy - 1); ++b)
-      for (int a = max(ci - 1, 0); a <= min(ci + 1, ncx - 1); ++a) {
-        const int cidx = b * ncx + a;
-        const int n = min(cell_count[cidx], CELL_CAP);
-        for (int k = 0; k < n; ++k) {
-          const int id = cell_items[cidx * CELL_CAP + k];
-          if (id > last && id < best) best = id;
+  // lanes 0..8: one cell of the neighbourhood each
+  int cidx = -1, cnt = 0;
+  if (lane < 9) {
+    const int a = ci + lane % 3 - 1, b = cj + lane / 3 - 1;
+    if (a >= 0 && a < ncx && b >= 0 && b < ncy) {
+      cidx = b * ncx + a;
+      cnt = min(cell_count[cidx], CELL_CAP);
+    }
+  }
+  int incl = cnt;   // inclusive prefix over lanes 0..8
+#pragma unroll
+  for (int d = 1; d < 16; d <<= 1) {
+    const int v = __shfl_up_sync(FULL, incl, d);
+    if (lane >= d) incl += v;
+  }
+  const int total = __shfl_sync(FULL, incl, 8);
+  for (int base = 0; base < total; base += 32) {
+    const int k = base + lane;   // candidate number k lives in the cell whose prefix range holds it
+    int id = 0x7fffffff;
+    double fx = 0.0, fy = 0.0;
+    int my_cell = -1, my_slot = 0;
+#pragma unroll
+    for (int s = 0; s < 9; ++s) {
+      const int hi = __shfl_sync(FULL, incl, s), n = __shfl_sync(FULL, cnt, s);
+      const int cc = __shfl_sync(FULL, cidx, s);
+      if (my_cell < 0 && k < hi && k >= hi - n) { my_cell = cc; my_slot = k - (hi - n); }
+    }
+    bool has = false;
+    if (k < total && my_cell >= 0) {
+      const int best = cell_items[my_cell * CELL_CAP + my_slot];
+      if (best != ia) {
+        const double bx = pa.x[cur][best], by = pa.y[cur][best], br = pa.r[best];
+        const double dx = ax - bx, dy = ay - by;
+        const double reach = ar + br + c.rep_s;
+        if (!(fabs(dx) > reach || fabs(dy) > reach)) {
+          const double dist = sqrt(dx * dx + dy * dy);
+          const double delta = dist - ar - br;
+          if (delta <= c.rep_s && dist > 0.0) {
+            const double Cb = PI * br * br * (pa.rho_ratio[best] * c.rho0 - c.rho0) * c.g;
+            const double mag = repulsion_mag(0.5 * (Ca + Cb), c, delta);
+            fx = mag * (dx / dist);
+            fy = mag * (dy / dist);
+            id = best;
+            has = true;
+          }
         }
       }
-    if (best == 0x7fffffff) break;
-    last = best;
-    if (best == ia) continue;
-    const double bx = pa.x[cur][best], by = pa.y[cur][best], br = pa.r[best];
-    const double dx = ax - bx, dy = ay - by;
-    const double reach = ar + br + c.rep_s;
-    if (fabs(dx) > reach || fabs(dy) > reach) continue;
-    const double dist = sqrt(dx * dx + dy * dy);
-    const double delta = dist - ar - br;
-    if (!(delta <= c.rep_s) || !(dist > 0.0)) continue;
-    const double Cb = PI * br * br * (pa.rho_ratio[best] * c.rho0 - c.rho0) * c.g;
-    const double mag = repulsion_mag(0.5 * (Ca + Cb), c, delta);
-    Fx += mag * (dx / dist);
-    Fy += mag * (dy / dist);
+    }
+    // contributions of this batch in ascending id (batches themselves are rare beyond the first:
+    // 32 candidates already cover 9 cells of edge >= d_max + s)
+    while (__any_sync(FULL, has)) {
+      const int m = __reduce_min_sync(FULL, has ? id : 0x7fffffff);
+      const int src = __ffs(__ballot_sync(FULL, has && id == m)) - 1;
+      Fx += __shfl_sync(FULL, fx, src);
+      Fy += __shfl_sync(FULL, fy, src);
+      if (lane == src) has = false;
+    }
   }
+  if (lane != 0) return;
   if (!c.periodic_x) {
     const double dW = (ax + 0.5) - ar;
     if (dW <= c.rep_s) Fx += repulsion_mag(Ca, c, dW);
@@ -348,7 +372,7 @@ void launch_cells_and_integrate(lbm* h) {
                                                h->ncx, h->ncy, h->cell_count, h->cell_items,
                                                h->status_dev);
   h->launches++;
-  k_integrate<<<blocks, 128, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
+  k_integrate<<<(h->np + IW - 1) / IW, IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
                                              h->cell_count, h->cell_items, h->status_dev, h->C);
 }
 

@@ -103,28 +103,46 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   update_node(A, B, c, i, j);
 }
 
-// NEAR pass: one CTA per particle over its effective zone [INT(xc-r)-1, INT(xc+r)+1]^2 at the
-// positions of time t, after the flag update: near nodes (zone stamp of this step) that are fluid
-// (flag 0) are updated; solid and newborn nodes are not.  Near sets of neighbouring particles may
-// overlap: both CTAs then compute and store bit-identical values (same inputs, same code), which
-// is benign.
+// NEAR pass: one CTA per particle, after the flag update, at the positions of time t.  Phase 1
+// scans the particle's effective zone [INT(xc-r)-1, INT(xc+r)+1]^2 with arithmetic only (the
+// same near_disc() predicate that stamped the zone map, so far and near pass partition the
+// lattice exactly), reads the flag of the candidates and compacts the nodes that are fluid at t
+// and t+1 (flag 0; solid = 1 and newborn = 2 are skipped) into shared memory.  Phase 2 updates
+// the compacted nodes, one per thread: ~100 of the 23 x 23 zone nodes at d = 20, so the heavy
+// per-node code runs with full warps instead of a 5-pass sweep with 80 % idle lanes.
+// Near sets of neighbouring particles may overlap: both CTAs then compute and store
+// bit-identical values (same inputs, same code), which is benign.
 __global__ void __launch_bounds__(SC_THREADS)
 k_stream_collide_near(const double* __restrict__ A, double* __restrict__ B,
-                      const unsigned char* __restrict__ flag,
-                      const unsigned char* __restrict__ zstamp, const unsigned char stamp,
-                      const double* __restrict__ px_, const double* __restrict__ py_,
-                      const double* __restrict__ pr, const LbmConst c) {
+                      const unsigned char* __restrict__ flag, const double* __restrict__ px_,
+                      const double* __restrict__ py_, const double* __restrict__ pr, int cap,
+                      const LbmConst c) {
+  extern __shared__ unsigned s_list[];   // cap entries: i | j << 16
+  __shared__ int s_n;
   const int p = blockIdx.x;
   const double xc = px_[p], yc = py_[p], r = pr[p];
-  const int i0 = (int)floor(xc - r) - 1, i1 = (int)floor(xc + r) + 1;
-  const int j0 = (int)floor(yc - r) - 1, j1 = (int)floor(yc + r) + 1;
+  int i0, i1, j0, j1;
+  zone_of(xc, yc, r, i0, i1, j0, j1);
   const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
+  if (threadIdx.x == 0) s_n = 0;
+  __syncthreads();
+  // nodes closer than r - 1 to the centre are inside the disc under any rounding: never flag 0
+  const double rin = r > 1.0 ? (r - 1.0) * (r - 1.0) : -1.0;
   for (int t = threadIdx.x; t < total; t += SC_THREADS) {
     const int i = i0 + t % W, j = j0 + t / W;
     if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    const long long x = (long long)j * c.px + i;
-    if (zstamp[x] != stamp || flag[x] != 0) continue;
-    update_node(A, B, c, i, j);
+    const double dx = (double)i - xc, dy = (double)j - yc;
+    if (dx * dx + dy * dy < rin) continue;
+    if (!near_disc((double)i, (double)j, xc, yc, r)) continue;
+    if (flag[(long long)j * c.px + i] != 0) continue;
+    const int e = atomicAdd(&s_n, 1);
+    if (e < cap) s_list[e] = (unsigned)i | ((unsigned)j << 16);
+  }
+  __syncthreads();
+  const int n = min(s_n, cap);
+  for (int e = threadIdx.x; e < n; e += SC_THREADS) {
+    const unsigned v = s_list[e];
+    update_node(A, B, c, (int)(v & 0xffffu), (int)(v >> 16));
   }
 }
 
@@ -223,9 +241,8 @@ void launch_stream_collide_near(lbm* h) {
   if (h->np == 0) return;
   const int old = h->cur ^ 1;   // positions at time t (the integrator has already flipped cur)
   h->launches++;
-  k_stream_collide_near<<<h->np, SC_THREADS, 0, h->chain>>>(
-      h->A, h->B, h->flag, h->zstamp[h->steps_done & 1], zone_stamp(h->steps_done), h->pa.x[old],
-      h->pa.y[old], h->pa.r, h->C);
+  k_stream_collide_near<<<h->np, SC_THREADS, h->la.cap * sizeof(unsigned), h->chain>>>(
+      h->A, h->B, h->flag, h->pa.x[old], h->pa.y[old], h->pa.r, h->la.cap, h->C);
 }
 
 void launch_init_collide(lbm* h, double* dst) {
