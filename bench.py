@@ -224,8 +224,8 @@ def main():
     value = world * n * K / (ms_max * 1e-3) / 1e6
 
     # ---------------- per-kernel CUDA-event durations -> roofline.  Two separate passes after the
-    # timed region: (a) as benched (particle chain overlapping the far pass of the lattice
-    # kernel), (b) strictly sequential on one stream (each kernel alone on the GPU).
+    # timed region: (a) strictly sequential on one stream (each kernel alone on the GPU), (b) as
+    # benched (particle update chain on its own stream, concurrent with the lattice kernel).
     P = min(args.profile_steps, 512)
 
     def profile_pass(overlap):
@@ -242,19 +242,18 @@ def main():
     st = sim.fields()
     flag = st["flag"]
     n_fluid = int((flag == 0).sum())
-    n_far = n - zone_nodes(w, sim.particles()) if w.particles is not None else n
     far_s = seq["stream_collide"] * 1e-3
     far_ovl_s = ovl["stream_collide"] * 1e-3
     step_ms_seq = sum(seq.values())
-    # far pass: 14 doubles read + 14 written per far node + 1 zone-stamp byte per node
-    alg_bytes = BYTES_PER_LU * n_far + FLAG_BYTES * n
+    # 14 doubles read + 14 written per fluid node + 1 flag byte per node
+    alg_bytes = BYTES_PER_LU * n_fluid + FLAG_BYTES * n
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
     achieved = alg_bytes / far_s / 1e9 if far_s > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_stream_collide (far pass)", "achieved": achieved,
+    roofline = {"bound": "hbm", "kernel": "k_stream_collide", "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": read_traffic(),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                 "avg_launch_ms": far_s * 1e3, "launches_timed": P,
@@ -263,7 +262,7 @@ def main():
                 "share_of_sequential_step": seq["stream_collide"] / step_ms_seq if step_ms_seq else None,
                 "kernel_ms_per_step_sequential": seq, "kernel_ms_per_step_overlapped": ovl,
                 "whole_step_frac_of_hbm_roofline": value / world / (peak * 1e9 / BYTES_PER_LU / 1e6),
-                "fluid_fraction": n_fluid / n, "far_fraction": n_far / n}
+                "fluid_fraction": n_fluid / n}
     sim.close()
     del sim
     torch.cuda.empty_cache()
@@ -331,22 +330,6 @@ def main():
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-
-
-def zone_nodes(w, parts):
-    """Number of lattice nodes the far pass skips: nodes within r + 1.5 of a particle centre
-    (the disc and every node that can have one of its solid nodes as a neighbour), inside the
-    effective zone of PAPER.md:258.  Harness-side count for the roofline's algorithmic bytes."""
-    import numpy as np
-    m = np.zeros((w.ny, w.nx), dtype=bool)
-    R = 0.5 * np.asarray(w.particles["diam"])
-    for x, y, r in zip(parts["x"], parts["y"], R):
-        i0, i1 = max(int(np.floor(x - r)) - 1, 0), min(int(np.floor(x + r)) + 1, w.nx - 1)
-        j0, j1 = max(int(np.floor(y - r)) - 1, 0), min(int(np.floor(y + r)) + 1, w.ny - 1)
-        I, J = np.meshgrid(np.arange(i0, i1 + 1, dtype=np.float64),
-                           np.arange(j0, j1 + 1, dtype=np.float64))
-        m[j0:j1 + 1, i0:i1 + 1] |= (I - x) ** 2 + (J - y) ** 2 <= (r + 1.5) ** 2
-    return int(m.sum())
 
 
 def read_traffic():

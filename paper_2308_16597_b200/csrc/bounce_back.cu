@@ -37,8 +37,7 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
 }
 
 __global__ void __launch_bounds__(BT)
-k_bounce_back(double* __restrict__ A, const unsigned char* __restrict__ flag, LinkArrays la,
-              ParticleArrays pa, int cur, const LbmConst c) {
+k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, const LbmConst c) {
   const int p = blockIdx.x;
   const int n = la.count[p];
   const long long base = (long long)p * la.cap;
@@ -47,23 +46,32 @@ k_bounce_back(double* __restrict__ A, const unsigned char* __restrict__ flag, Li
   double Fx = 0.0, Fy = 0.0, Tz = 0.0;
   for (int s = threadIdx.x; s < n; s += BT) {
     const int xf = la.node[base + s];
-    const int al = la.dir[base + s];
+    const int db = la.dir[base + s];
     const double q = la.q[base + s];
+    const int al = db & LINK_DIR_MASK;
+    const int nbehind = db >> LINK_BEHIND_SHIFT;   // fluid nodes behind x_f (link builder)
     const int ab = b_opp[al];
     const int i = xf % c.px, j = xf / c.px;
     const int ex = b_ex[al], ey = b_ey[al];
-    const long long x1 = node_at(c, i, j, -ex, -ey);
-    int nbehind = 0;
-    long long x2 = -1;
-    if (x1 >= 0 && flag[x1] == 0) {
-      nbehind = 1;
-      x2 = node_at(c, i, j, -2 * ex, -2 * ey);
-      if (x2 >= 0 && flag[x2] == 0) nbehind = 2;
-    }
+    // every population the ladder can ask for is fetched up front (independent loads in flight
+    // together); a node that is not there is replaced by x_f and its value is not used
+    const long long x1 = nbehind >= 1 ? node_at(c, i, j, -ex, -ey) : (long long)xf;
+    const long long x2 = nbehind == 2 ? node_at(c, i, j, -2 * ex, -2 * ey) : (long long)xf;
     const double* Fi = A + (long long)al * c.ps;
     const double* Fb = A + (long long)ab * c.ps;
     const double fi0 = Fi[xf];
     const double fb0 = Fb[xf];
+    const double fi1 = Fi[x1];
+    const double fi2 = Fi[x2];
+    const double fb1 = Fb[x1];
+    double gi0 = 0.0, gb0 = 0.0, gi1 = 0.0;
+    if (al <= 4) {
+      const double* Gi = A + (long long)(9 + al) * c.ps;
+      const double* Gb = A + (long long)(9 + ab) * c.ps;
+      gi0 = Gi[xf];
+      gb0 = Gb[xf];
+      gi1 = Gi[x1];
+    }
     // wall point and wall velocity u_w = U_c + Omega x (x_w - x_c)
     const double rwx = ((double)i + q * ex) - xc;
     const double rwy = ((double)j + q * ey) - yc;
@@ -73,15 +81,15 @@ k_bounce_back(double* __restrict__ A, const unsigned char* __restrict__ flag, Li
     double fbb;
     if (q <= 0.5) {
       if (nbehind == 2)
-        fbb = q * (2.0 * q + 1.0) * fi0 + (1.0 - 4.0 * q * q) * Fi[x1] - q * (1.0 - 2.0 * q) * Fi[x2] + wall;
+        fbb = q * (2.0 * q + 1.0) * fi0 + (1.0 - 4.0 * q * q) * fi1 - q * (1.0 - 2.0 * q) * fi2 + wall;
       else if (nbehind == 1)
-        fbb = 2.0 * q * fi0 + (1.0 - 2.0 * q) * Fi[x1] + wall;
+        fbb = 2.0 * q * fi0 + (1.0 - 2.0 * q) * fi1 + wall;
       else
         fbb = fi0 + wall;
     } else {
       if (nbehind >= 1) {
         const double cq = 1.0 / (q * (2.0 * q + 1.0));
-        fbb = cq * fi0 + ((2.0 * q - 1.0) / q) * fb0 - ((2.0 * q - 1.0) / (2.0 * q + 1.0)) * Fb[x1] + cq * wall;
+        fbb = cq * fi0 + ((2.0 * q - 1.0) / q) * fb0 - ((2.0 * q - 1.0) / (2.0 * q + 1.0)) * fb1 + cq * wall;
       } else {
         fbb = (fi0 + (2.0 * q - 1.0) * fb0) / (2.0 * q) + wall / (2.0 * q);
       }
@@ -89,15 +97,14 @@ k_bounce_back(double* __restrict__ A, const unsigned char* __restrict__ flag, Li
     const long long xb = (long long)(j + ey) * c.px + (i + ex);   // solid node of the link
     A[(long long)ab * c.ps + xb] = fbb;                           // parked for the pull at x_f
     if (al <= 4) {
-      const double* Gi = A + (long long)(9 + al) * c.ps;
-      const double* Gb = A + (long long)(9 + ab) * c.ps;
-      double cd2 = 0.0, cd4 = 1.0, gi1 = 0.0;
+      double cd2 = 0.0, cd4 = 1.0;
       if (nbehind >= 1) {
         cd2 = (2.0 * q - 1.0) / (2.0 * q + 1.0);
         cd4 = 2.0 / (2.0 * q + 1.0);
-        gi1 = Gi[x1];
+      } else {
+        gi1 = 0.0;
       }
-      const double gbb = (-Gi[xf] + cd2 * gi1 + cd2 * Gb[xf]) + cd4 * (2.0 * c.wT * Tw);
+      const double gbb = (-gi0 + cd2 * gi1 + cd2 * gb0) + cd4 * (2.0 * c.wT * Tw);
       A[(long long)(9 + ab) * c.ps + xb] = gbb;
     }
     // Eqs. (13), (14)
@@ -250,7 +257,7 @@ __global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __r
 void launch_bounce_back(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_bounce_back<<<h->np, BT, 0, h->chain>>>(h->A, h->flag, h->la, h->pa, h->cur, h->C);
+  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->C);
 }
 
 void launch_refill(lbm* h) {
@@ -258,9 +265,9 @@ void launch_refill(lbm* h) {
   int blocks = (h->np * 4 + 127) / 128;   // a handful of newborn nodes per particle and step
   if (blocks > 1184) blocks = 1184;
   h->launches++;
-  k_refill<<<blocks, 128, 0, h->chain>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
+  k_refill<<<blocks, 128, 0, h->stream>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
                                           h->newborn_count, h->newborn_cap, h->pa, h->cur, h->C);
   h->launches++;
-  k_newborn_clear<<<blocks, 128, 0, h->chain>>>(h->flag, h->newborn_node, h->newborn_count,
+  k_newborn_clear<<<blocks, 128, 0, h->stream>>>(h->flag, h->newborn_node, h->newborn_count,
                                                  h->newborn_cap);
 }

@@ -19,7 +19,7 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "cells_integrate",
-    "flags_uncover", "flags_cover", "refill", "init_collide", "stream_collide_near"};
+    "flags_uncover", "flags_cover", "refill", "init_collide"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -77,8 +77,6 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   double* A = c.take<double>(14 * (size_t)L.ps);
   double* B = c.take<double>(14 * (size_t)L.ps);
   unsigned char* flag = c.take<unsigned char>((size_t)L.px * ny);
-  unsigned char* zs0 = c.take<unsigned char>((size_t)L.px * ny);
-  unsigned char* zs1 = c.take<unsigned char>((size_t)L.px * ny);
   int* owner = c.take<int>((size_t)L.px * ny);
   ParticleArrays pa;
   for (int b = 0; b < 2; ++b) {
@@ -115,8 +113,6 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
     h->A = A;
     h->B = B;
     h->flag = flag;
-    h->zstamp[0] = zs0;
-    h->zstamp[1] = zs1;
     h->owner = owner;
     h->pa = pa;
     h->la = la;
@@ -215,6 +211,13 @@ void prime(lbm* h) {
   h->primed = 1;
 }
 
+// links of the current positions (the first step's; afterwards every step builds the next one's)
+void ensure_links(lbm* h) {
+  if (h->links_ready || h->np == 0) return;
+  launch_build_links(h, h->cur, h->stream);
+  h->links_ready = 1;
+}
+
 } // namespace
 
 extern "C" {
@@ -261,8 +264,8 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     delete h;
     return LBM_E_CUDA;
   }
-  // second stream for the particle chain: highest priority, so
-  // that its short latency-bound kernels get SM slots as CTAs of the far pass retire
+  // second stream for the particle update chain: highest priority, so
+  // that its short latency-bound kernels get SM slots as CTAs of the lattice kernel retire
   h->chain = h->stream;
   {
     int lo = 0, hi = 0;
@@ -280,8 +283,6 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   // initial state: fluid everywhere, f = f_eq(rho0, 0), g = g_eq(T0, 0)
   const size_t nn = (size_t)h->px * ny;
   cudaMemsetAsync(h->flag, 0, nn, h->stream);
-  cudaMemsetAsync(h->zstamp[0], 0, nn, h->stream);
-  cudaMemsetAsync(h->zstamp[1], 0, nn, h->stream);
   cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
   cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
   cudaMemsetAsync(h->newborn_count, 0, sizeof(int), h->stream);
@@ -408,46 +409,46 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   h->ncy = (int)std::ceil(h->ny / h->cell) + 1;
   if ((long long)h->ncx * h->ncy > h->max_cells)
     return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
-  CUDA_OK(h, cudaStreamSynchronize(h->stream));   // uploads done before the chain stream reads them
-  launch_cover(h, c);   // flag, owner and zone maps of step 0 (primed == 0: fixed particles too)
-  CUDA_OK(h, cudaStreamSynchronize(h->chain));
+  launch_cover(h, c, h->stream);   // flag and owner maps of step 0 (primed == 0: fixed particles too)
+  h->links_ready = 0;
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
   return LBM_OK;
 }
 
+// Step schedule: the resident state A is f+(x,t), g+(x,t), the index array holds
+// the links of x_p(t).
+//   S0: bounce-back + momentum exchange (parks f_ibar(x_f,t+1) in solid slots of A, sums F, T_z)
+//   S1:   after it: integrate -> uncover -> cover -> links of x_p(t+1)      } concurrent with
+//   S0: fused pull-stream-collide A -> B over every node fluid at t          } each other
+//   S0: after both: refill of the nodes uncovered this step (A -> B), newborn flags cleared
+// Only the lattice kernel, the bounce-back kernel and the refill are on the critical path.
 int lbm_step(lbm_t* h, int nsteps) {
   if (!h) return LBM_E_ARG;
   if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
-  prime(h);
+  if (nsteps > 0) {
+    prime(h);
+    ensure_links(h);
+  }
   cudaStream_t S0 = h->stream, S1 = h->chain;
   for (int s = 0; s < nsteps; ++s) {
-    const long long t = h->steps_done;
     if (h->np > 0) {
-      // zone map of this step's parity: its stamp value wraps every 510 steps -> clear + re-mark
-      if (t >= 2 && ((t >> 1) % 255) == 0) {
-        cudaMemsetAsync(h->zstamp[t & 1], 0, (size_t)h->px * h->ny, S0);
-        launch_mark_zones(h, h->cur, t, S0);
-      }
+      { Timed tm(h, K_BOUNCE_BACK, S0); launch_bounce_back(h); }
       if (S1 != S0) {
         cudaEventRecord(h->ev_fork, S0);
         cudaStreamWaitEvent(S1, h->ev_fork, 0);
       }
-    }
-    // far pass: independent of the particle chain, runs concurrently with it
-    { Timed tm(h, K_STREAM_COLLIDE, S0); launch_stream_collide_far(h); }
-    if (h->np > 0) {
-      { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h); }
-      { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h); }
       { Timed tm(h, K_INTEGRATE, S1); launch_cells_and_integrate(h); }
       { Timed tm(h, K_UNCOVER, S1); launch_uncover(h); }
-      { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1); }
+      { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1, S1); }
+      { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h, h->cur ^ 1, S1); }
       h->cur ^= 1;
-      { Timed tm(h, K_STREAM_COLLIDE_NEAR, S1); launch_stream_collide_near(h); }
-      { Timed tm(h, K_REFILL, S1); launch_refill(h); }
-      if (S1 != S0) {
-        cudaEventRecord(h->ev_join, S1);
-        cudaStreamWaitEvent(S0, h->ev_join, 0);
-      }
+      if (S1 != S0) cudaEventRecord(h->ev_join, S1);
+    }
+    { Timed tm(h, K_STREAM_COLLIDE, S0); launch_stream_collide(h); }
+    if (h->np > 0) {
+      if (S1 != S0) cudaStreamWaitEvent(S0, h->ev_join, 0);
+      { Timed tm(h, K_REFILL, S0); launch_refill(h); }
     }
     std::swap(h->A, h->B);
     h->steps_done++;
@@ -532,8 +533,7 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
   const long long capacity = *n;
   *n = 0;
   if (h->np == 0) return LBM_OK;
-  launch_build_links(h);
-  if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
+  ensure_links(h);
   std::vector<int> count(h->np);
   CUDA_OK(h, cudaMemcpyAsync(count.data(), h->la.count, h->np * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   int rc = check_status(h);
@@ -557,7 +557,7 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
       if (pid) pid[o] = p;
       if (i) i[o] = node[k] % h->px;
       if (j) j[o] = node[k] / h->px;
-      if (alpha) alpha[o] = dir[k];
+      if (alpha) alpha[o] = dir[k] & LINK_DIR_MASK;
       if (q) q[o] = qq[k];
     }
   return LBM_OK;

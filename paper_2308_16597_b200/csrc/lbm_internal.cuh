@@ -7,11 +7,6 @@
 //   flag : 1 byte/node, 0 fluid, 1 solid, 2 newborn (solid at t, fluid at t+1; only between the
 //          flag update and the refill kernel of one step)
 //   owner: int32/node, id of the lowest-numbered particle covering the node, OWNER_NONE = fluid
-//   zstamp[2]: 1 byte/node each, double-buffered by step parity: node x lies in some particle's
-//          effective zone at step t  <=>  zstamp[t&1][x] == zone_stamp(t).  Nodes outside every
-//          zone ("far") cannot be solid, cannot change flag and do not pull from a solid slot, so
-//          the far pass of the lattice kernel is independent of the whole particle chain of the
-//          step and overlaps with it on a second stream.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -31,24 +26,15 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
-  K_INIT, K_STREAM_COLLIDE_NEAR, K_COUNT
+  K_INIT, K_COUNT
 };
 
-// stamp of step t in zstamp[t&1]: 1..255, each value used once per array and epoch of 510 steps;
-// the array is cleared and re-marked when the value wraps (lbm_capi.cu), so a stale stamp never
-// equals the current one
-__host__ __device__ inline unsigned char zone_stamp(long long t) {
-  return (unsigned char)(((t >> 1) % 255) + 1);
-}
-
-// "Near" nodes of a particle: the disc itself plus every node that can have one of its solid nodes
-// among its 8 neighbours (|x - x_c| <= r + sqrt2 < r + 1.5).  Written with explicit round-to-nearest
-// intrinsics so that every translation unit (with or without -fmad) takes the same decision: the
-// zone-stamp writer (particles.cu) and the near pass (stream_collide.cu) must agree node by node.
-__device__ __forceinline__ bool near_disc(double xi, double yj, double xc, double yc, double r) {
-  const double dx = __dsub_rn(xi, xc), dy = __dsub_rn(yj, yc), rr = __dadd_rn(r, 1.5);
-  return __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)) <= __dmul_rn(rr, rr);
-}
+// link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along
+// -e_alpha (0, 1 or 2: which rung of the interpolation ladder of DESIGN.md reading 6 applies).
+// The link builder fills it from the flag map of the step the links belong to, so that the
+// bounce-back kernel needs no dependent flag loads.
+#define LINK_DIR_MASK 0x0f
+#define LINK_BEHIND_SHIFT 4
 
 // effective zone of PAPER.md:258 (the narrower reading of DESIGN.md): [INT(xc-r)-1, INT(xc+r)+1]^2
 __device__ __forceinline__ void zone_of(double xc, double yc, double r, int& i0, int& i1, int& j0, int& j1) {
@@ -94,14 +80,14 @@ struct lbm {
   long long ps;
   lbm_params P;
   LbmConst C;
-  cudaStream_t stream;       // the caller's stream: far pass of the lattice kernel, set-up, read-out
-  cudaStream_t chain;        // particle chain + near pass (own high-priority stream when overlapping)
+  cudaStream_t stream;       // the caller's stream: bounce-back, lattice kernel, refill, set-up, read-out
+  cudaStream_t chain;        // particle update chain (integrator, flags, next step's links)
   cudaStream_t chain_own;    // the stream we created (NULL if creation failed)
   cudaEvent_t ev_fork, ev_join;
-  int overlap;               // 1: chain runs on `chain_own` concurrently with the far pass
+  int overlap;               // 1: chain runs on `chain_own` concurrently with the lattice kernel
+  int links_ready;           // the index array holds the links of the current particle positions
   double *A, *B;             // 14 planes each
   unsigned char* flag;
-  unsigned char* zstamp[2];
   int* owner;
   ParticleArrays pa;
   LinkArrays la;
@@ -132,18 +118,16 @@ struct lbm {
 
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
-void launch_stream_collide_far(lbm* h);    // on h->stream
-void launch_stream_collide_near(lbm* h);   // on h->chain; zones of the positions in buffer cur^1
+void launch_stream_collide(lbm* h);        // on h->stream
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
 void launch_set_equilibrium(lbm* h);
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
 // particles.cu (compiled with -fmad=false)
-void launch_build_links(lbm* h);
-void launch_cells_and_integrate(lbm* h);
-void launch_uncover(lbm* h);
-void launch_cover(lbm* h, int which_buffer);
-void launch_mark_zones(lbm* h, int which_buffer, long long step, cudaStream_t st);
+void launch_build_links(lbm* h, int which_buffer, cudaStream_t st);
+void launch_cells_and_integrate(lbm* h);   // on h->chain
+void launch_uncover(lbm* h);               // on h->chain
+void launch_cover(lbm* h, int which_buffer, cudaStream_t st);
 // bounce_back.cu
-void launch_bounce_back(lbm* h);
-void launch_refill(lbm* h);
+void launch_bounce_back(lbm* h);            // on h->stream
+void launch_refill(lbm* h);                 // on h->stream

@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(PT)
 k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
               const double* __restrict__ pr, const unsigned char* __restrict__ flag,
               const int* __restrict__ owner, LinkArrays la, int* __restrict__ status,
-              int* __restrict__ nb_count, const LbmConst c) {
+              const LbmConst c) {
   const int p = blockIdx.x;
   const double xc = px_[p], yc = py_[p], r = pr[p];
   int i0, i1, j0, j1;
@@ -55,10 +55,7 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   __shared__ int s_warp[PT / 32];
   __shared__ int s_running;
-  if (threadIdx.x == 0) {
-    s_running = 0;
-    if (p == 0) *nb_count = 0;   // the newborn list of the previous step has been consumed
-  }
+  if (threadIdx.x == 0) s_running = 0;
   __syncthreads();
   const long long base = (long long)p * la.cap;
   const double rfar = (r + 1.5) * (r + 1.5);   // beyond this no neighbour can be inside the disc
@@ -72,7 +69,8 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
       j = j0 + t / W;
       if (i >= 0 && i < c.nx && j >= 0 && j < c.ny) {
         const double dx = (double)i - xc, dy = (double)j - yc;
-        if (dx * dx + dy * dy <= rfar && flag[(long long)j * c.px + i] == 0) {
+        // flag 2 = newborn: a fluid node of the step these links belong to
+        if (dx * dx + dy * dy <= rfar && flag[(long long)j * c.px + i] != 1) {
 #pragma unroll
           for (int al = 1; al <= 8; ++al) {
             const int bi = i + p_ex[al], bj = j + p_ey[al];
@@ -119,12 +117,25 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
     if (threadIdx.x == 0) s_running += btotal;
     __syncthreads();
   }
-  // q for the compacted links, one link per thread (no divergence over directions)
+  // q and the ladder rung for the compacted links, one link per thread (no divergence over
+  // directions): how many of x_f - e, x_f - 2e are fluid nodes inside the cavity
   const int nl = min(s_running, la.cap);
   for (int s = threadIdx.x; s < nl; s += PT) {
     const int node = la.node[base + s];
     const int al = la.dir[base + s];
-    la.q[base + s] = link_q((double)(node % c.px), (double)(node / c.px), al, xc, yc, r);
+    const int i = node % c.px, j = node / c.px;
+    la.q[base + s] = link_q((double)i, (double)j, al, xc, yc, r);
+    int behind = 0;
+    int a1 = i - p_ex[al], b1 = j - p_ey[al];
+    if (c.periodic_x) a1 = (a1 + c.nx) % c.nx;
+    if (a1 >= 0 && a1 < c.nx && b1 >= 0 && b1 < c.ny && flag[(long long)b1 * c.px + a1] != 1) {
+      behind = 1;
+      int a2 = i - 2 * p_ex[al], b2 = j - 2 * p_ey[al];
+      if (c.periodic_x) a2 = (a2 + c.nx) % c.nx;
+      if (a2 >= 0 && a2 < c.nx && b2 >= 0 && b2 < c.ny && flag[(long long)b2 * c.px + a2] != 1)
+        behind = 2;
+    }
+    la.dir[base + s] = (unsigned char)(al | (behind << LINK_BEHIND_SHIFT));
   }
   if (threadIdx.x == 0) la.count[p] = nl;
 }
@@ -133,9 +144,11 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
 // a5: repulsion grid
 __global__ void k_cells_build(const double* __restrict__ px_, const double* __restrict__ py_, int np,
                               double cell, int ncx, int ncy, int* __restrict__ cell_count,
-                              int* __restrict__ cell_items, int* __restrict__ status) {
+                              int* __restrict__ cell_items, int* __restrict__ status,
+                              int* __restrict__ nb_count) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np) return;
+  if (p == 0) *nb_count = 0;   // the newborn list of the previous step has been consumed
   int ci = (int)floor(px_[p] / cell), cj = (int)floor(py_[p] / cell);
   ci = min(max(ci, 0), ncx - 1);
   cj = min(max(cj, 0), ncy - 1);
@@ -313,14 +326,12 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
 }
 
 // Phase B: every node inside the disc at the position in buffer `buf` is solid; the lowest
-// particle id wins the owner map (same rule as a from-scratch recomputation).  Also stamps the
-// particle's effective zone at that position into the zone map of the step that will use it.
+// particle id wins the owner map (same rule as a from-scratch recomputation).
 __global__ void __launch_bounds__(PT)
 k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ flag,
-        int* __restrict__ owner, unsigned char* __restrict__ zs, unsigned char stamp,
-        const LbmConst c) {
+        int* __restrict__ owner, const LbmConst c) {
   const int p = blockIdx.x;
-  const bool stamp_only = skip_fixed && pa.fixed[p];
+  if (skip_fixed && pa.fixed[p]) return;
   const double xn = pa.x[buf][p], yn = pa.y[buf][p], r = pa.r[p];
   int i0, i1, j0, j1;
   zone_of(xn, yn, r, i0, i1, j0, j1);
@@ -328,40 +339,21 @@ k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ 
   for (int t = threadIdx.x; t < total; t += PT) {
     const int i = i0 + t % W, j = j0 + t / W;
     if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
+    if (!inside_disc((double)i, (double)j, xn, yn, r)) continue;
     const long long x = (long long)j * c.px + i;
-    if (!near_disc((double)i, (double)j, xn, yn, r)) continue;
-    zs[x] = stamp;
-    if (stamp_only || !inside_disc((double)i, (double)j, xn, yn, r)) continue;
     if (owner[x] == p) continue;
     const int prev = atomicMin(&owner[x], p);
     if (prev != p) flag[x] = 1;
   }
 }
 
-// zone stamps only (epoch reset of a zone map, see zone_stamp())
-__global__ void __launch_bounds__(PT)
-k_mark_zones(const double* __restrict__ px_, const double* __restrict__ py_,
-             const double* __restrict__ pr, unsigned char* __restrict__ zs, unsigned char stamp,
-             const LbmConst c) {
-  const int p = blockIdx.x;
-  const double xc = px_[p], yc = py_[p], r = pr[p];
-  int i0, i1, j0, j1;
-  zone_of(xc, yc, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
-  for (int t = threadIdx.x; t < total; t += PT) {
-    const int i = i0 + t % W, j = j0 + t / W;
-    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    if (near_disc((double)i, (double)j, xc, yc, r)) zs[(long long)j * c.px + i] = stamp;
-  }
-}
-
 } // namespace
 
-void launch_build_links(lbm* h) {
+void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_build_links<<<h->np, PT, 0, h->chain>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->pa.r, h->flag,
-                                             h->owner, h->la, h->status_dev, h->newborn_count, h->C);
+  k_build_links<<<h->np, PT, 0, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r,
+                                      h->flag, h->owner, h->la, h->status_dev, h->C);
 }
 
 void launch_cells_and_integrate(lbm* h) {
@@ -370,7 +362,7 @@ void launch_cells_and_integrate(lbm* h) {
   h->launches++;
   k_cells_build<<<blocks, 128, 0, h->chain>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->np, h->cell,
                                                h->ncx, h->ncy, h->cell_count, h->cell_items,
-                                               h->status_dev);
+                                               h->status_dev, h->newborn_count);
   h->launches++;
   k_integrate<<<(h->np + IW - 1) / IW, IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
                                              h->cell_count, h->cell_items, h->status_dev, h->C);
@@ -384,22 +376,10 @@ void launch_uncover(lbm* h) {
                                          h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
 }
 
-void launch_cover(lbm* h, int which_buffer) {
-  if (h->np == 0) return;
-  // after add_particles every particle (fixed ones too) must be stamped; during stepping the
-  // fixed ones never move
-  // The positions in `which_buffer` are those of step `next`: during stepping next = steps_done+1
-  // (called before steps_done is incremented), at set-up next = steps_done (= 0).
-  const int skip_fixed = h->primed ? 1 : 0;
-  const long long next = h->primed ? h->steps_done + 1 : h->steps_done;
-  h->launches++;
-  k_cover<<<h->np, PT, 0, h->chain>>>(h->pa, which_buffer, skip_fixed, h->flag, h->owner,
-                                      h->zstamp[next & 1], zone_stamp(next), h->C);
-}
-
-void launch_mark_zones(lbm* h, int which_buffer, long long step, cudaStream_t st) {
+// after add_particles every particle (fixed ones too) is rasterised; during stepping the fixed
+// ones never move
+void launch_cover(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_mark_zones<<<h->np, PT, 0, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r,
-                                     h->zstamp[step & 1], zone_stamp(step), h->C);
+  k_cover<<<h->np, PT, 0, st>>>(h->pa, which_buffer, h->primed ? 1 : 0, h->flag, h->owner, h->C);
 }

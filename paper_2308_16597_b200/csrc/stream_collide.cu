@@ -89,61 +89,35 @@ __device__ __forceinline__ void update_node(const double* __restrict__ A, double
   for (int k = 0; k < 5; ++k) O[(9 + k) * c.ps] = g[k];
 }
 
-// FAR pass: every node outside all particle zones of this step (zstamp != stamp).  Such a node is
-// fluid, stays fluid, and none of its upstream neighbours is a solid slot, so this kernel depends
-// on nothing the particle chain of the step produces and runs concurrently with it.
+// One thread per node, 128-thread CTAs along x.  Solid (1) and newborn (2) nodes do no lattice
+// update.  DRAM moves whole 32-byte sectors, and a partially written sector costs a read-modify-
+// write there, so a non-fluid lane whose aligned group of SC_FILL lanes (= SC_FILL * 8 bytes of
+// every plane) holds at least one fluid lane stores zeros: slots of non-fluid nodes in B are
+// don't-care (a parked value is written by the NEXT step's bounce-back kernel, a newborn node by
+// this step's refill kernel, both ordered after this kernel), and every store of the kernel then
+// covers complete sectors.
+//
+// The flag update of this step (k_uncover / k_cover on the chain stream) may run concurrently:
+// a node it covers (0 -> 1) was fluid at t, so updating it or not are both fine (its B slot is
+// don't-care from t+1 on); a node it uncovers (1 -> 2) is skipped under either value.
+constexpr int SC_FILL = 8;
 __global__ void __launch_bounds__(SC_THREADS)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
-                 const unsigned char* __restrict__ zstamp, const unsigned char stamp,
-                 const LbmConst c) {
+                 const unsigned char* __restrict__ flag, const LbmConst c) {
   const int i = blockIdx.x * SC_THREADS + threadIdx.x;
   const int j = blockIdx.y;
-  if (i >= c.nx) return;
-  if (zstamp[(long long)j * c.px + i] == stamp) return;   // near: left to k_stream_collide_near
-  update_node(A, B, c, i, j);
-}
-
-// NEAR pass: one CTA per particle, after the flag update, at the positions of time t.  Phase 1
-// scans the particle's effective zone [INT(xc-r)-1, INT(xc+r)+1]^2 with arithmetic only (the
-// same near_disc() predicate that stamped the zone map, so far and near pass partition the
-// lattice exactly), reads the flag of the candidates and compacts the nodes that are fluid at t
-// and t+1 (flag 0; solid = 1 and newborn = 2 are skipped) into shared memory.  Phase 2 updates
-// the compacted nodes, one per thread: ~100 of the 23 x 23 zone nodes at d = 20, so the heavy
-// per-node code runs with full warps instead of a 5-pass sweep with 80 % idle lanes.
-// Near sets of neighbouring particles may overlap: both CTAs then compute and store
-// bit-identical values (same inputs, same code), which is benign.
-__global__ void __launch_bounds__(SC_THREADS)
-k_stream_collide_near(const double* __restrict__ A, double* __restrict__ B,
-                      const unsigned char* __restrict__ flag, const double* __restrict__ px_,
-                      const double* __restrict__ py_, const double* __restrict__ pr, int cap,
-                      const LbmConst c) {
-  extern __shared__ unsigned s_list[];   // cap entries: i | j << 16
-  __shared__ int s_n;
-  const int p = blockIdx.x;
-  const double xc = px_[p], yc = py_[p], r = pr[p];
-  int i0, i1, j0, j1;
-  zone_of(xc, yc, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
-  if (threadIdx.x == 0) s_n = 0;
-  __syncthreads();
-  // nodes closer than r - 1 to the centre are inside the disc under any rounding: never flag 0
-  const double rin = r > 1.0 ? (r - 1.0) * (r - 1.0) : -1.0;
-  for (int t = threadIdx.x; t < total; t += SC_THREADS) {
-    const int i = i0 + t % W, j = j0 + t / W;
-    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    const double dx = (double)i - xc, dy = (double)j - yc;
-    if (dx * dx + dy * dy < rin) continue;
-    if (!near_disc((double)i, (double)j, xc, yc, r)) continue;
-    if (flag[(long long)j * c.px + i] != 0) continue;
-    const int e = atomicAdd(&s_n, 1);
-    if (e < cap) s_list[e] = (unsigned)i | ((unsigned)j << 16);
+  const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
+  const unsigned m = __ballot_sync(0xffffffffu, fluid);
+  if (fluid) {
+    update_node(A, B, c, i, j);
+    return;
   }
-  __syncthreads();
-  const int n = min(s_n, cap);
-  for (int e = threadIdx.x; e < n; e += SC_THREADS) {
-    const unsigned v = s_list[e];
-    update_node(A, B, c, (int)(v & 0xffffu), (int)(v >> 16));
-  }
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned grp = (m >> (lane & ~(unsigned)(SC_FILL - 1))) & ((1u << SC_FILL) - 1u);
+  if (grp == 0u || i >= c.px) return;
+  double* __restrict__ O = B + (long long)j * c.px + i;
+#pragma unroll
+  for (int k = 0; k < 14; ++k) O[k * c.ps] = 0.0;
 }
 
 // first step only: A holds the PRE-collision initial state f(x,0); collide it (in place when
@@ -231,18 +205,10 @@ inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1
 
 } // namespace
 
-void launch_stream_collide_far(lbm* h) {
+void launch_stream_collide(lbm* h) {
   h->launches++;
-  k_stream_collide<<<grid_rows(h->nx, h->ny, SC_THREADS), SC_THREADS, 0, h->stream>>>(
-      h->A, h->B, h->zstamp[h->steps_done & 1], zone_stamp(h->steps_done), h->C);
-}
-
-void launch_stream_collide_near(lbm* h) {
-  if (h->np == 0) return;
-  const int old = h->cur ^ 1;   // positions at time t (the integrator has already flipped cur)
-  h->launches++;
-  k_stream_collide_near<<<h->np, SC_THREADS, h->la.cap * sizeof(unsigned), h->chain>>>(
-      h->A, h->B, h->flag, h->pa.x[old], h->pa.y[old], h->pa.r, h->la.cap, h->C);
+  k_stream_collide<<<grid_rows(h->px, h->ny, SC_THREADS), SC_THREADS, 0, h->stream>>>(
+      h->A, h->B, h->flag, h->C);
 }
 
 void launch_init_collide(lbm* h, double* dst) {

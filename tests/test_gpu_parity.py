@@ -198,9 +198,8 @@ def test_small_sedimentation_many_particles(gpu, ob, wl):
 
 
 def test_overlap_and_sequential_modes_agree_bitwise(gpu, wl):
-    """The far/near split with the particle chain on its own stream must give the same bits as
-    the strictly sequential single-stream schedule (also crosses two zone-map epoch resets at
-    steps 510/511 and 1020/1021)."""
+    """The schedule with the particle update chain on its own stream, concurrent with the lattice
+    kernel, must give the same bits as the strictly sequential single-stream schedule."""
     w = wl.sedimentation(300, 260, 14, seed=9, y_frac_lo=0.2, d_lo=12.0, d_hi=24.0, name="ovl")
     a = gpu.Simulation.from_workload(w)
     b = gpu.Simulation.from_workload(w)
