@@ -36,9 +36,20 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
   return (long long)b * c.px + a;
 }
 
-__global__ void __launch_bounds__(BT)
-k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, const LbmConst c) {
+__global__ void __launch_bounds__(BT, 6)
+k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
+              unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
+              const int* __restrict__ nb_count, int nb_cap, const LbmConst c) {
   const int p = blockIdx.x;
+  // the nodes refilled by the previous step are ordinary fluid nodes from now on (this kernel
+  // reads no flags; the lattice kernel and the flag update of this step run after it)
+  {
+    const int nn = min(*nb_count, nb_cap);
+    for (int e = p * BT + threadIdx.x; e < nn; e += gridDim.x * BT) {
+      const int x = nb_node[e];
+      if (flag[x] == 2) flag[x] = 0;
+    }
+  }
   const int n = la.count[p];
   const long long base = (long long)p * la.cap;
   const double xc = pa.x[cur][p], yc = pa.y[cur][p];
@@ -53,17 +64,17 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     const int ab = b_opp[al];
     const int i = xf % c.px, j = xf / c.px;
     const int ex = b_ex[al], ey = b_ey[al];
-    // every population the ladder can ask for is fetched up front (independent loads in flight
-    // together); a node that is not there is replaced by x_f and its value is not used
+    // the populations this link's rung of the ladder needs, all requested before the first use
+    // (independent loads in flight together); q <= 1/2 interpolates upstream of x_f in plane
+    // alpha, q > 1/2 downstream of the wall in plane alpha-bar
+    const bool lo = q <= 0.5;
     const long long x1 = nbehind >= 1 ? node_at(c, i, j, -ex, -ey) : (long long)xf;
     const long long x2 = nbehind == 2 ? node_at(c, i, j, -2 * ex, -2 * ey) : (long long)xf;
     const double* Fi = A + (long long)al * c.ps;
     const double* Fb = A + (long long)ab * c.ps;
     const double fi0 = Fi[xf];
-    const double fb0 = Fb[xf];
-    const double fi1 = Fi[x1];
-    const double fi2 = Fi[x2];
-    const double fb1 = Fb[x1];
+    const double fa = lo ? Fi[x1] : Fb[xf];      // f_i(x_f - e_i)    | f_ibar(x_f)
+    const double fc = lo ? Fi[x2] : Fb[x1];      // f_i(x_f - 2 e_i)  | f_ibar(x_f - e_i)
     double gi0 = 0.0, gb0 = 0.0, gi1 = 0.0;
     if (al <= 4) {
       const double* Gi = A + (long long)(9 + al) * c.ps;
@@ -79,19 +90,19 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     const double uwy = Uy + Om * rwx;
     const double wall = 6.0 * b_w[al] * c.rho0 * ((double)b_ex[ab] * uwx + (double)b_ey[ab] * uwy);
     double fbb;
-    if (q <= 0.5) {
+    if (lo) {
       if (nbehind == 2)
-        fbb = q * (2.0 * q + 1.0) * fi0 + (1.0 - 4.0 * q * q) * fi1 - q * (1.0 - 2.0 * q) * fi2 + wall;
+        fbb = q * (2.0 * q + 1.0) * fi0 + (1.0 - 4.0 * q * q) * fa - q * (1.0 - 2.0 * q) * fc + wall;
       else if (nbehind == 1)
-        fbb = 2.0 * q * fi0 + (1.0 - 2.0 * q) * fi1 + wall;
+        fbb = 2.0 * q * fi0 + (1.0 - 2.0 * q) * fa + wall;
       else
         fbb = fi0 + wall;
     } else {
       if (nbehind >= 1) {
         const double cq = 1.0 / (q * (2.0 * q + 1.0));
-        fbb = cq * fi0 + ((2.0 * q - 1.0) / q) * fb0 - ((2.0 * q - 1.0) / (2.0 * q + 1.0)) * fb1 + cq * wall;
+        fbb = cq * fi0 + ((2.0 * q - 1.0) / q) * fa - ((2.0 * q - 1.0) / (2.0 * q + 1.0)) * fc + cq * wall;
       } else {
-        fbb = (fi0 + (2.0 * q - 1.0) * fb0) / (2.0 * q) + wall / (2.0 * q);
+        fbb = (fi0 + (2.0 * q - 1.0) * fa) / (2.0 * q) + wall / (2.0 * q);
       }
     }
     const long long xb = (long long)(j + ey) * c.px + (i + ex);   // solid node of the link
@@ -143,23 +154,22 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
   }
 }
 
-// f_k(y, t+1) for every k at a node y that was fluid at t: the same pull the lattice kernel does
-__device__ __forceinline__ void pull_f(const double* __restrict__ A, const LbmConst& c, int i, int j,
-                                       double (&f)[9]) {
-  const long long y = (long long)j * c.px + i;
-#pragma unroll
-  for (int k = 0; k < 9; ++k) {
-    const long long s = node_at(c, i, j, -b_ex[k], -b_ey[k]);
-    f[k] = s >= 0 ? A[(long long)k * c.ps + s] : A[(long long)b_opp[k] * c.ps + y];
-  }
-}
-
-__global__ void k_refill(const double* __restrict__ A, double* __restrict__ B,
-                         const unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
-                         const int* __restrict__ nb_pid, const int* __restrict__ nb_count, int nb_cap,
-                         ParticleArrays pa, int cur, const LbmConst c) {
+// a6: one WARP per newborn node.  Lane l < 27 fetches population k = l % 9 of stencil node
+// s = l / 9, i.e. f_k(x_new + (s+1) e_c, t+1) = the same pull the lattice kernel does at a node
+// that was fluid at t (upstream slot of A, which holds a parked value where the upstream node is
+// solid; the node's own opposite slot at a cavity wall), so the 27 gathers are in flight
+// together; the extrapolation, the momentum constraint, Eq. (17) and the collision are then
+// evaluated redundantly by every lane and lane k < 14 stores plane k.
+constexpr int RW = 8;   // warps (newborn nodes) per CTA
+__global__ void __launch_bounds__(RW * 32)
+k_refill(const double* __restrict__ A, double* __restrict__ B,
+         const unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
+         const int* __restrict__ nb_pid, const int* __restrict__ nb_count, int nb_cap,
+         ParticleArrays pa, int cur, const LbmConst c) {
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
   const int n = min(*nb_count, nb_cap);
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+  for (int e = blockIdx.x * RW + (threadIdx.x >> 5); e < n; e += gridDim.x * RW) {
     const int x = nb_node[e];
     if (flag[x] != 2) continue;   // covered again by another particle in the same step
     const int p = nb_pid[e];
@@ -177,72 +187,70 @@ __global__ void k_refill(const double* __restrict__ A, double* __restrict__ B,
     }
     const double uwx = pa.ux[cur][p] - pa.omega[cur][p] * dyn;
     const double uwy = pa.uy[cur][p] + pa.omega[cur][p] * dxn;
-    int nvalid = 0;
-    int si[3], sj[3];
-    for (int k = 1; k <= 3; ++k) {
-      const long long s = node_at(c, i, j, k * b_ex[ec], k * b_ey[ec]);
-      if (s < 0 || flag[s] != 0) break;   // must be fluid at t and at t+1
-      si[k - 1] = (int)(s % c.px);
-      sj[k - 1] = (int)(s / c.px);
-      nvalid = k;
+    const double Tw = pa.Tw[p];
+    // stencil node of this lane and whether it is fluid at t and at t+1 (flag 0)
+    const int st = lane / 9, k = lane % 9;
+    const long long snode = lane < 27 ? node_at(c, i, j, (st + 1) * b_ex[ec], (st + 1) * b_ey[ec]) : -1;
+    const bool ok = snode >= 0 && flag[snode] == 0;
+    const unsigned okm = __ballot_sync(FULL, ok);
+    int nvalid = 0;                                   // leading run of valid stencil nodes
+    if (okm & 1u) { nvalid = 1; if (okm & (1u << 9)) { nvalid = 2; if (okm & (1u << 18)) nvalid = 3; } }
+    double v = 0.0;
+    if (lane < 27 && st < nvalid) {
+      const int ci = (int)(snode % c.px), cj = (int)(snode / c.px);
+      const long long src = node_at(c, ci, cj, -b_ex[k], -b_ey[k]);
+      v = src >= 0 ? A[(long long)k * c.ps + src] : A[(long long)b_opp[k] * c.ps + snode];
     }
     double f[9], g[5];
+#pragma unroll
+    for (int kk = 0; kk < 9; ++kk) {
+      const double f1 = __shfl_sync(FULL, v, kk);
+      const double f2 = __shfl_sync(FULL, v, 9 + kk);
+      const double f3 = __shfl_sync(FULL, v, 18 + kk);
+      if (nvalid == 3) f[kk] = 3.0 * f1 - 3.0 * f2 + f3;   // Eq. (16)
+      else if (nvalid == 2) f[kk] = 2.0 * f1 - f2;
+      else f[kk] = f1;
+    }
     if (nvalid == 0) {
       const double u2 = uwx * uwx + uwy * uwy;
 #pragma unroll
-      for (int k = 0; k < 9; ++k) {
-        const double eu = (double)b_ex[k] * uwx + (double)b_ey[k] * uwy;
-        f[k] = b_w[k] * c.rho0 * (1.0 + 3.0 * eu + 4.5 * eu * eu - 1.5 * u2);
-      }
-    } else {
-      double f1[9];
-      pull_f(A, c, si[0], sj[0], f1);
-      if (nvalid == 1) {
-#pragma unroll
-        for (int k = 0; k < 9; ++k) f[k] = f1[k];
-      } else {
-        double f2[9];
-        pull_f(A, c, si[1], sj[1], f2);
-        if (nvalid == 2) {
-#pragma unroll
-          for (int k = 0; k < 9; ++k) f[k] = 2.0 * f1[k] - f2[k];
-        } else {
-          double f3[9];
-          pull_f(A, c, si[2], sj[2], f3);
-#pragma unroll
-          for (int k = 0; k < 9; ++k) f[k] = 3.0 * f1[k] - 3.0 * f2[k] + f3[k];   // Eq. (16)
-        }
+      for (int kk = 0; kk < 9; ++kk) {
+        const double eu = (double)b_ex[kk] * uwx + (double)b_ey[kk] * uwy;
+        f[kk] = b_w[kk] * c.rho0 * (1.0 + 3.0 * eu + 4.5 * eu * eu - 1.5 * u2);
       }
     }
     // MRT velocity constraint: set j = rho_new u_w, all other moments unchanged:
     // f += M^-1 (dj_x e_jx + dj_y e_jy), rows j_x, j_y of M have norm^2 6
     double rho = 0.0, jx = 0.0, jy = 0.0;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) {
-      rho += f[k];
-      jx += (double)b_ex[k] * f[k];
-      jy += (double)b_ey[k] * f[k];
+    for (int kk = 0; kk < 9; ++kk) {
+      rho += f[kk];
+      jx += (double)b_ex[kk] * f[kk];
+      jy += (double)b_ey[kk] * f[kk];
     }
     const double djx = (rho * uwx - jx) * (1.0 / 6.0), djy = (rho * uwy - jy) * (1.0 / 6.0);
 #pragma unroll
-    for (int k = 1; k < 9; ++k) f[k] += (double)b_ex[k] * djx + (double)b_ey[k] * djy;
+    for (int kk = 1; kk < 9; ++kk) f[kk] += (double)b_ex[kk] * djx + (double)b_ey[kk] * djy;
     // Eq. (17): g = g_eq(T_w, u_w)
-    const double Tw = pa.Tw[p];
     g[0] = c.wT0 * Tw;
 #pragma unroll
-    for (int k = 1; k < 5; ++k) g[k] = c.wT * Tw + 0.5 * ((double)b_ex[k] * uwx + (double)b_ey[k] * uwy) * Tw;
+    for (int kk = 1; kk < 5; ++kk)
+      g[kk] = c.wT * Tw + 0.5 * ((double)b_ex[kk] * uwx + (double)b_ey[kk] * uwy) * Tw;
     // the resident state is post-collision: collide the refilled node now
     mrt_collide(f, g, c);
+    double out = 0.0;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) B[(long long)k * c.ps + x] = f[k];
+    for (int kk = 0; kk < 9; ++kk) if (lane == kk) out = f[kk];
 #pragma unroll
-    for (int k = 0; k < 5; ++k) B[(long long)(9 + k) * c.ps + x] = g[k];
-    // flag[x] stays 2 until k_newborn_clear: other threads of this kernel still test their
-    // stencil nodes against it
+    for (int kk = 0; kk < 5; ++kk) if (lane == 9 + kk) out = g[kk];
+    if (lane < 14) B[(long long)lane * c.ps + x] = out;
+    // flag[x] stays 2 until the newborn flags are cleared (next step's bounce-back kernel or a
+    // read-out): other warps of this kernel still test their stencil nodes against it
   }
 }
 
-// newborn nodes are ordinary fluid nodes from the next step on
+// newborn nodes are ordinary fluid nodes from the next step on: done by the next step's
+// bounce-back kernel, and by this kernel at the end of an lbm_step call (before any read-out)
 __global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
                                 const int* __restrict__ nb_count, int nb_cap) {
   const int n = min(*nb_count, nb_cap);
@@ -257,16 +265,23 @@ __global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __r
 void launch_bounce_back(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->C);
+  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->flag, h->newborn_node,
+                                              h->newborn_count, h->newborn_cap, h->C);
 }
 
 void launch_refill(lbm* h) {
   if (h->np == 0) return;
-  int blocks = (h->np * 4 + 127) / 128;   // a handful of newborn nodes per particle and step
+  int blocks = (h->np + RW - 1) / RW;   // a handful of newborn nodes per particle and step
   if (blocks > 1184) blocks = 1184;
   h->launches++;
-  k_refill<<<blocks, 128, 0, h->stream>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
-                                          h->newborn_count, h->newborn_cap, h->pa, h->cur, h->C);
+  k_refill<<<blocks, RW * 32, 0, h->stream>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
+                                               h->newborn_count, h->newborn_cap, h->pa, h->cur, h->C);
+}
+
+void launch_newborn_clear(lbm* h) {
+  if (h->np == 0) return;
+  int blocks = (h->np * 4 + 127) / 128;
+  if (blocks > 1184) blocks = 1184;
   h->launches++;
   k_newborn_clear<<<blocks, 128, 0, h->stream>>>(h->flag, h->newborn_node, h->newborn_count,
                                                  h->newborn_cap);

@@ -453,6 +453,7 @@ int lbm_step(lbm_t* h, int nsteps) {
     std::swap(h->A, h->B);
     h->steps_done++;
   }
+  if (nsteps > 0) launch_newborn_clear(h);   // read-outs see flags 0/1 only
   return check_status(h);
 }
 

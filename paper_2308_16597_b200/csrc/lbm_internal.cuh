@@ -131,3 +131,4 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st);
 // bounce_back.cu
 void launch_bounce_back(lbm* h);            // on h->stream
 void launch_refill(lbm* h);                 // on h->stream
+void launch_newborn_clear(lbm* h);          // on h->stream
