@@ -56,13 +56,14 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
   const double Ux = pa.ux[cur][p], Uy = pa.uy[cur][p], Om = pa.omega[cur][p], Tw = pa.Tw[p];
   double Fx = 0.0, Fy = 0.0, Tz = 0.0;
   for (int s = threadIdx.x; s < n; s += BT) {
-    const int xf = la.node[base + s];
+    const int nd = la.node[base + s];
     const int db = la.dir[base + s];
     const double q = la.q[base + s];
     const int al = db & LINK_DIR_MASK;
     const int nbehind = db >> LINK_BEHIND_SHIFT;   // fluid nodes behind x_f (link builder)
     const int ab = b_opp[al];
-    const int i = xf % c.px, j = xf / c.px;
+    const int i = nd & 0xffff, j = (int)((unsigned)nd >> 16);
+    const int xf = j * c.px + i;
     const int ex = b_ex[al], ey = b_ey[al];
     // the populations this link's rung of the ladder needs, all requested before the first use
     // (independent loads in flight together); q <= 1/2 interpolates upstream of x_f in plane

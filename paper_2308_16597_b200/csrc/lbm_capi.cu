@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -18,7 +19,7 @@ namespace {
 char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
-    "stream_collide", "build_links", "bounce_back_force", "cells_integrate",
+    "stream_collide", "build_links", "bounce_back_force", "integrate",
     "flags_uncover", "flags_cover", "refill", "init_collide"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
@@ -94,6 +95,7 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   pa.Fy = c.take<double>(np);
   pa.Tz = c.take<double>(np);
   pa.fixed = c.take<unsigned char>(np);
+  pa.ovl = c.take<unsigned char>(np);
   LinkArrays la;
   const size_t nl = np * (size_t)p->max_links_per_particle;
   la.node = c.take<int>(nl);
@@ -258,6 +260,10 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   h->stream = (cudaStream_t)cuda_stream;
   carve(h, dev_workspace, nx, ny, p);
   fill_const(h);
+  if (particles_configure(h) != 0) {
+    delete h;
+    return fail(nullptr, LBM_E_CUDA, "lbm_create: max_links_per_particle needs more shared memory than the device has");
+  }
   cudaError_t e = cudaMallocHost((void**)&h->status_host, sizeof(int));
   if (e != cudaSuccess) {
     fail(nullptr, LBM_E_CUDA, "cudaMallocHost: %s", cudaGetErrorString(e));
@@ -270,7 +276,9 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);
-    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
+    int prio = hi;
+    if (const char* e = getenv("LBM_CHAIN_PRIO")) prio = (e[0] == 'l') ? lo : (e[0] == 's' ? 0 : hi);
+    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, prio) == cudaSuccess &&
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess) {
       h->overlap = 1;
@@ -402,6 +410,7 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   CUDA_OK(h, up(h->pa.Fy, nullptr));
   CUDA_OK(h, up(h->pa.Tz, nullptr));
   CUDA_OK(h, cudaMemcpyAsync(h->pa.fixed + n0, fx.data(), n, cudaMemcpyHostToDevice, h->stream));
+  CUDA_OK(h, cudaMemsetAsync(h->pa.ovl + n0, 0, n, h->stream));
   h->np = nt;
   h->d_max = dmax;
   h->cell = std::max(dmax + h->P.rep_s, MIN_CELL);
@@ -409,7 +418,9 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   h->ncy = (int)std::ceil(h->ny / h->cell) + 1;
   if ((long long)h->ncx * h->ncy > h->max_cells)
     return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
-  launch_cover(h, c, h->stream);   // flag and owner maps of step 0 (primed == 0: fixed particles too)
+  // flag and owner maps and the repulsion grid of step 0 (primed == 0: every particle, full sweep)
+  CUDA_OK(h, cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->max_cells, h->stream));
+  launch_cover(h, c, h->stream);
   h->links_ready = 0;
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
@@ -438,7 +449,7 @@ int lbm_step(lbm_t* h, int nsteps) {
         cudaEventRecord(h->ev_fork, S0);
         cudaStreamWaitEvent(S1, h->ev_fork, 0);
       }
-      { Timed tm(h, K_INTEGRATE, S1); launch_cells_and_integrate(h); }
+      { Timed tm(h, K_INTEGRATE, S1); launch_integrate(h); }
       { Timed tm(h, K_UNCOVER, S1); launch_uncover(h); }
       { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1, S1); }
       { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h, h->cur ^ 1, S1); }
@@ -556,8 +567,8 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
     for (int s = 0; s < count[p]; ++s, ++o) {
       const size_t k = (size_t)p * h->la.cap + s;
       if (pid) pid[o] = p;
-      if (i) i[o] = node[k] % h->px;
-      if (j) j[o] = node[k] / h->px;
+      if (i) i[o] = node[k] & 0xffff;
+      if (j) j[o] = (int)((unsigned)node[k] >> 16);
       if (alpha) alpha[o] = dir[k] & LINK_DIR_MASK;
       if (q) q[o] = qq[k];
     }

@@ -65,10 +65,11 @@ struct ParticleArrays {      // SoA in the workspace, each max_particles long
   double *r, *rho_ratio, *Tw;
   double *Fx, *Fy, *Tz;      // hydrodynamic force / torque of the last step (Eqs. 13, 14)
   unsigned char* fixed;
+  unsigned char* ovl;        // sticky: the disc may share nodes with another particle's (k_cover)
 };
 
 struct LinkArrays {          // the paper's fixed index array: segment p = [p*cap, (p+1)*cap)
-  int* node;                 // j*px + i of the fluid node x_f
+  int* node;                 // fluid node x_f, packed i | j << 16 (nx, ny <= 46000 < 2^16)
   unsigned char* dir;        // alpha in 1..8
   double* q;
   int* count;                // links of particle p
@@ -125,7 +126,8 @@ void launch_set_equilibrium(lbm* h);
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
 // particles.cu (compiled with -fmad=false)
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st);
-void launch_cells_and_integrate(lbm* h);   // on h->chain
+void launch_integrate(lbm* h);             // on h->chain
+int particles_configure(lbm* h);           // per-handle kernel attributes (0 = ok)
 void launch_uncover(lbm* h);               // on h->chain
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st);
 // bounce_back.cu

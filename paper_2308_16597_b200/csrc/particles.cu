@@ -41,100 +41,179 @@ __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: link builder.  grid = particles, block = PT.
-__global__ void __launch_bounds__(PT)
+// a2: link builder.  grid = particles, block = LB_WARPS warps.
+//
+// The effective zone is cut into items = (row, 32-column chunk), dealt to the warps in contiguous
+// runs; a lane keeps the 8-bit direction masks of up to LB_ITEMS items in registers, so the whole
+// zone of a d <= 28 particle is one round with one block prefix.  The work is ordered so that
+// nothing waits on memory item by item:
+//   1. arithmetic only: can the node carry a link (outside the own disc, within r + 1.5 of the
+//      centre) and which neighbours lie inside the disc -- the separately rounded predicate that
+//      rasterised the disc;
+//   2. the flag bytes of all candidate nodes of the round, requested together (a candidate may be
+//      inside ANOTHER particle);
+//   3. only for a particle whose disc may overlap another one (sticky flag pa.ovl, set by k_cover):
+//      the owner of each solid neighbour, lowest id owns the node.  Without
+//      overlap every node inside the disc is owned by the particle and the loads are skipped;
+//   4. packed warp prefix (four 16-bit item counts per 64-bit shuffle), block prefix, emission in
+//      row-major order (neighbouring links -> neighbouring nodes for the bounce-back kernel) into
+//      shared memory;
+//   5. q and the ladder rung per link, one link per thread, both flag bytes requested together.
+constexpr int LB_WARPS = 4;
+constexpr int LB_ITEMS = 8;
+__global__ void __launch_bounds__(LB_WARPS * 32)
 k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
-              const double* __restrict__ pr, const unsigned char* __restrict__ flag,
-              const int* __restrict__ owner, LinkArrays la, int* __restrict__ status,
-              const LbmConst c) {
+              const double* __restrict__ pr, const unsigned char* __restrict__ ovl,
+              const unsigned char* __restrict__ flag, const int* __restrict__ owner, LinkArrays la,
+              int* __restrict__ status, const LbmConst c) {
+  extern __shared__ int s_node[];                           // la.cap packed nodes, then la.cap dir bytes
+  unsigned char* s_dir = (unsigned char*)(s_node + la.cap);
+  __shared__ int s_warp[LB_WARPS];
   const int p = blockIdx.x;
   const double xc = px_[p], yc = py_[p], r = pr[p];
+  const bool check_owner = ovl[p] != 0;
   int i0, i1, j0, j1;
   zone_of(xc, yc, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, H = j1 - j0 + 1, total = W * H;
+  const int W = i1 - i0 + 1, H = j1 - j0 + 1;
+  const int chunks = (W + 31) >> 5, n_items = H * chunks;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  __shared__ int s_warp[PT / 32];
-  __shared__ int s_running;
-  if (threadIdx.x == 0) s_running = 0;
-  __syncthreads();
-  const long long base = (long long)p * la.cap;
+  const unsigned FULL = 0xffffffffu;
+  const double r2 = r * r;
   const double rfar = (r + 1.5) * (r + 1.5);   // beyond this no neighbour can be inside the disc
+  int running = 0;                             // links emitted by earlier rounds (same in all threads)
 
-  for (int start = 0; start < total; start += PT) {
-    const int t = start + threadIdx.x;
-    unsigned mask = 0;
-    int i = 0, j = 0;
-    if (t < total) {
-      i = i0 + t % W;
-      j = j0 + t / W;
-      if (i >= 0 && i < c.nx && j >= 0 && j < c.ny) {
-        const double dx = (double)i - xc, dy = (double)j - yc;
-        // flag 2 = newborn: a fluid node of the step these links belong to
-        if (dx * dx + dy * dy <= rfar && flag[(long long)j * c.px + i] != 1) {
+  for (int first = 0; first < n_items; first += LB_WARPS * LB_ITEMS) {
+    const int in_round = min(n_items - first, LB_WARPS * LB_ITEMS);
+    const int ipw = (in_round + LB_WARPS - 1) / LB_WARPS;   // items per warp, contiguous
+    unsigned mask[LB_ITEMS];
+    int node[LB_ITEMS];
+    // ---- 1. arithmetic
 #pragma unroll
-          for (int al = 1; al <= 8; ++al) {
-            const int bi = i + p_ex[al], bj = j + p_ey[al];
-            if (bi >= 0 && bi < c.nx && bj >= 0 && bj < c.ny &&
-                owner[(long long)bj * c.px + bi] == p)
-              mask |= 1u << al;
-          }
+    for (int k = 0; k < LB_ITEMS; ++k) {
+      mask[k] = 0;
+      node[k] = 0;
+      const int item = first + warp * ipw + k;
+      if (k >= ipw || item >= first + in_round) continue;
+      const int row = chunks == 1 ? item : item / chunks;
+      const int i = i0 + ((item - row * chunks) << 5) + lane, j = j0 + row;
+      if (i > i1 || i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
+      // coordinates of the 3 x 3 neighbourhood: integers are exact in fp64, so xi + 1.0 is
+      // (double)(i + 1) bit for bit and the disc test below is the rasteriser's
+      const double xi = (double)i, yj = (double)j;
+      const double dx0 = xi - xc, dy0 = yj - yc;
+      const double sx0 = dx0 * dx0, sy0 = dy0 * dy0;
+      const double d2 = sx0 + sy0;
+      if (!(d2 > r2) || !(d2 <= rfar)) continue;
+      const double dxm = (xi - 1.0) - xc, dxp = (xi + 1.0) - xc;
+      const double dym = (yj - 1.0) - yc, dyp = (yj + 1.0) - yc;
+      const double sxm = dxm * dxm, sxp = dxp * dxp, sym = dym * dym, syp = dyp * dyp;
+      const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.ny - 1;
+      unsigned m = 0;
+      if (ei && sxp + sy0 <= r2) m |= 1u << 1;
+      if (no && sx0 + syp <= r2) m |= 1u << 2;
+      if (wi && sxm + sy0 <= r2) m |= 1u << 3;
+      if (so && sx0 + sym <= r2) m |= 1u << 4;
+      if (ei && no && sxp + syp <= r2) m |= 1u << 5;
+      if (wi && no && sxm + syp <= r2) m |= 1u << 6;
+      if (wi && so && sxm + sym <= r2) m |= 1u << 7;
+      if (ei && so && sxp + sym <= r2) m |= 1u << 8;
+      mask[k] = m;
+      node[k] = (int)((unsigned)i | ((unsigned)j << 16));
+    }
+    // ---- 2. flags of the candidates (flag 2 = newborn: a fluid node of the step the links are for)
+    unsigned char fl[LB_ITEMS];
+#pragma unroll
+    for (int k = 0; k < LB_ITEMS; ++k)
+      fl[k] = mask[k] ? flag[(long long)(int)((unsigned)node[k] >> 16) * c.px + (node[k] & 0xffff)] : 1;
+#pragma unroll
+    for (int k = 0; k < LB_ITEMS; ++k)
+      if (fl[k] == 1) mask[k] = 0;
+    // ---- 3. ownership of the solid neighbours, only if discs may overlap
+    if (check_owner) {
+#pragma unroll
+      for (int k = 0; k < LB_ITEMS; ++k) {
+        const int i = node[k] & 0xffff, j = (int)((unsigned)node[k] >> 16);
+        unsigned keep = 0;
+        for (unsigned t = mask[k]; t; t &= t - 1) {
+          const int al = __ffs(t) - 1;
+          if (owner[(long long)(j + p_ey[al]) * c.px + (i + p_ex[al])] == p) keep |= 1u << al;
         }
+        mask[k] = keep;
       }
     }
-    // block exclusive scan of popc(mask)
-    const int cnt = __popc(mask);
-    int incl = cnt;
+    // ---- 4. prefix: item-major within the warp, warps in order
+    unsigned long long pk0 = 0, pk1 = 0;   // 16-bit counts of items 0..3 and 4..7
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      pk0 |= (unsigned long long)__popc(mask[k]) << (16 * k);
+      pk1 |= (unsigned long long)__popc(mask[k + 4]) << (16 * k);
+    }
+    unsigned long long in0 = pk0, in1 = pk1;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-      const int v = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lane >= d) incl += v;
+      const unsigned long long v0 = __shfl_up_sync(FULL, in0, d);
+      const unsigned long long v1 = __shfl_up_sync(FULL, in1, d);
+      if (lane >= d) { in0 += v0; in1 += v1; }
     }
-    if (lane == 31) s_warp[warp] = incl;
+    const unsigned long long t0 = __shfl_sync(FULL, in0, 31), t1 = __shfl_sync(FULL, in1, 31);
+    const unsigned long long ex0 = in0 - pk0, ex1 = in1 - pk1;   // exclusive over lanes, per item
+    int item_off[LB_ITEMS];
+    int wtotal = 0;
+#pragma unroll
+    for (int k = 0; k < LB_ITEMS; ++k) {
+      item_off[k] = wtotal;
+      wtotal += (int)(((k < 4 ? t0 : t1) >> (16 * (k & 3))) & 0xffffu);
+    }
+    if (lane == 0) s_warp[warp] = wtotal;
     __syncthreads();
     int woff = 0, btotal = 0;
 #pragma unroll
-    for (int w = 0; w < PT / 32; ++w) {
+    for (int w = 0; w < LB_WARPS; ++w) {
       const int v = s_warp[w];
       if (w < warp) woff += v;
       btotal += v;
     }
-    int off = s_running + woff + incl - cnt;
-    if (cnt) {
-      if (off + cnt <= la.cap) {
-        const int node = j * c.px + i;
-        while (mask) {                         // compaction only; q follows in a balanced pass
-          const int al = __ffs(mask) - 1;
-          mask &= mask - 1;
-          la.node[base + off] = node;
-          la.dir[base + off] = (unsigned char)al;
+    if (running + btotal <= la.cap) {
+#pragma unroll
+      for (int k = 0; k < LB_ITEMS; ++k) {
+        unsigned m = mask[k];
+        if (!m) continue;
+        int off = running + woff + item_off[k] +
+                  (int)(((k < 4 ? ex0 : ex1) >> (16 * (k & 3))) & 0xffffu);
+        while (m) {
+          const int al = __ffs(m) - 1;
+          m &= m - 1;
+          s_node[off] = node[k];
+          s_dir[off] = (unsigned char)al;
           ++off;
         }
-      } else {
-        atomicOr(status, ST_LINK_OVERFLOW);
       }
+    } else if (threadIdx.x == 0) {
+      atomicOr(status, ST_LINK_OVERFLOW);
     }
-    __syncthreads();
-    if (threadIdx.x == 0) s_running += btotal;
+    running += btotal;
     __syncthreads();
   }
-  // q and the ladder rung for the compacted links, one link per thread (no divergence over
-  // directions): how many of x_f - e, x_f - 2e are fluid nodes inside the cavity
-  const int nl = min(s_running, la.cap);
-  for (int s = threadIdx.x; s < nl; s += PT) {
-    const int node = la.node[base + s];
-    const int al = la.dir[base + s];
-    const int i = node % c.px, j = node / c.px;
-    la.q[base + s] = link_q((double)i, (double)j, al, xc, yc, r);
-    int behind = 0;
-    int a1 = i - p_ex[al], b1 = j - p_ey[al];
-    if (c.periodic_x) a1 = (a1 + c.nx) % c.nx;
-    if (a1 >= 0 && a1 < c.nx && b1 >= 0 && b1 < c.ny && flag[(long long)b1 * c.px + a1] != 1) {
-      behind = 1;
-      int a2 = i - 2 * p_ex[al], b2 = j - 2 * p_ey[al];
-      if (c.periodic_x) a2 = (a2 + c.nx) % c.nx;
-      if (a2 >= 0 && a2 < c.nx && b2 >= 0 && b2 < c.ny && flag[(long long)b2 * c.px + a2] != 1)
-        behind = 2;
+  // ---- 5. q and the ladder rung, one link per thread: how many of x_f - e, x_f - 2e are fluid
+  // nodes inside the cavity (both flag bytes requested before either is tested)
+  const int nl = running <= la.cap ? running : 0;
+  const long long base = (long long)p * la.cap;
+  for (int s = threadIdx.x; s < nl; s += LB_WARPS * 32) {
+    const int nd = s_node[s];
+    const int al = s_dir[s];
+    const int i = nd & 0xffff, j = (int)((unsigned)nd >> 16);
+    int a1 = i - p_ex[al], b1 = j - p_ey[al], a2 = i - 2 * p_ex[al], b2 = j - 2 * p_ey[al];
+    if (c.periodic_x) {
+      a1 = (a1 + c.nx) % c.nx;
+      a2 = (a2 + c.nx) % c.nx;
     }
+    const bool in1 = a1 >= 0 && a1 < c.nx && b1 >= 0 && b1 < c.ny;
+    const bool in2 = a2 >= 0 && a2 < c.nx && b2 >= 0 && b2 < c.ny;
+    const unsigned char f1 = in1 ? flag[(long long)b1 * c.px + a1] : 1;
+    const unsigned char f2 = in2 ? flag[(long long)b2 * c.px + a2] : 1;
+    const int behind = f1 == 1 ? 0 : (f2 == 1 ? 1 : 2);
+    la.q[base + s] = link_q((double)i, (double)j, al, xc, yc, r);
+    la.node[base + s] = nd;
     la.dir[base + s] = (unsigned char)(al | (behind << LINK_BEHIND_SHIFT));
   }
   if (threadIdx.x == 0) la.count[p] = nl;
@@ -142,22 +221,6 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
 
 // ------------------------------------------------------------------------------------------
 // a5: repulsion grid
-__global__ void k_cells_build(const double* __restrict__ px_, const double* __restrict__ py_, int np,
-                              double cell, int ncx, int ncy, int* __restrict__ cell_count,
-                              int* __restrict__ cell_items, int* __restrict__ status,
-                              int* __restrict__ nb_count) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= np) return;
-  if (p == 0) *nb_count = 0;   // the newborn list of the previous step has been consumed
-  int ci = (int)floor(px_[p] / cell), cj = (int)floor(py_[p] / cell);
-  ci = min(max(ci, 0), ncx - 1);
-  cj = min(max(cj, 0), ncy - 1);
-  const int cidx = cj * ncx + ci;
-  const int slot = atomicAdd(&cell_count[cidx], 1);
-  if (slot < CELL_CAP) cell_items[cidx * CELL_CAP + slot] = p;
-  else atomicOr(status, ST_CELL_OVERFLOW);
-}
-
 __device__ __forceinline__ double ipow(double x, int p) {
   double r = 1.0;
   for (int k = 0; k < p; ++k) r = r * x;
@@ -180,8 +243,11 @@ constexpr int IW = 4;   // warps (particles) per CTA
 __global__ void __launch_bounds__(IW * 32)
 k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
             const int* __restrict__ cell_count, const int* __restrict__ cell_items,
-            int* __restrict__ status, const LbmConst c) {
+            int* __restrict__ status, int* __restrict__ nb_count, const LbmConst c) {
   const int lane = threadIdx.x & 31;
+  // the newborn list of the previous step has been consumed (refill, then the bounce-back kernel
+  // of this step cleared its flags; both precede this kernel)
+  if (blockIdx.x == 0 && threadIdx.x == 0) *nb_count = 0;
   const int ia = blockIdx.x * IW + (threadIdx.x >> 5);
   if (ia >= np) return;
   const unsigned FULL = 0xffffffffu;
@@ -290,14 +356,27 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
 }
 
 // ------------------------------------------------------------------------------------------
-// a6, flags.  Phase A: nodes owned by p that the disc at its NEW position no longer covers become
-// newborn candidates (flag 2, owner NONE) and are appended to the newborn list.
+// a6, flags.  Zone sweep shared by both phases: rows dealt to the warps, lanes across x (no
+// integer division for zones up to 32 nodes wide).
+template <typename F>
+__device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const LbmConst& c, F f) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int j = j0 + warp; j <= j1; j += PT / 32) {
+    if (j < 0 || j >= c.ny) continue;
+    for (int i = i0 + lane; i <= i1; i += 32)
+      if (i >= 0 && i < c.nx) f(i, j);
+  }
+}
+
+// Phase A: nodes owned by p that the disc at its NEW position no longer covers become newborn
+// candidates (flag 2, owner NONE) and are appended to the newborn list.
 __global__ void __launch_bounds__(PT)
 k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __restrict__ owner,
           int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
           int* __restrict__ status, int* __restrict__ cell_count, int ncells, const LbmConst c) {
   const int p = blockIdx.x;
-  // the repulsion grid of this step has been consumed by k_integrate: zero it for the next step
+  // the repulsion grid of this step has been consumed by k_integrate: zero it; k_cover refills it
+  // with the new positions for the next step
   for (int k = p * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count[k] = 0;
   if (pa.fixed[p]) return;
   const int nxt = cur ^ 1;
@@ -305,14 +384,11 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
   const double xn = pa.x[nxt][p], yn = pa.y[nxt][p];
   int i0, i1, j0, j1;
   zone_of(xo, yo, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
-  for (int t = threadIdx.x; t < total; t += PT) {
-    const int i = i0 + t % W, j = j0 + t / W;
-    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    if (!inside_disc((double)i, (double)j, xo, yo, r)) continue;
-    if (inside_disc((double)i, (double)j, xn, yn, r)) continue;
+  for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
+    if (!inside_disc((double)i, (double)j, xo, yo, r)) return;
+    if (inside_disc((double)i, (double)j, xn, yn, r)) return;
     const long long x = (long long)j * c.px + i;
-    if (owner[x] != p) continue;
+    if (owner[x] != p) return;
     owner[x] = OWNER_NONE;
     flag[x] = 2;
     const int e = atomicAdd(nb_count, 1);
@@ -322,29 +398,51 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
     } else {
       atomicOr(status, ST_NEWBORN_OVERFLOW);
     }
-  }
+  });
 }
 
 // Phase B: every node inside the disc at the position in buffer `buf` is solid; the lowest
 // particle id wins the owner map (same rule as a from-scratch recomputation).
+//
+// Invariant: every node inside the disc of a particle with pa.ovl == 0 is owned by it.  Such a
+// particle therefore only has to claim the nodes its move has newly covered (inside the new
+// disc, outside the old one -- arithmetic), not re-read the owner of its whole disc.  The flag is
+// sticky and is raised whenever two discs share a node: by the particle that finds a node of its
+// disc owned by a lower id, and for the particle a lower id takes a node from.  A flagged particle
+// (and every particle at set-up, `all` = 1) sweeps its whole disc, which also re-claims nodes
+// another particle has just uncovered.
+// Thread 0 also enters the particle into the repulsion grid of the step that will use this
+// position (k_uncover has zeroed the counts).
 __global__ void __launch_bounds__(PT)
-k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ flag,
-        int* __restrict__ owner, const LbmConst c) {
+k_cover(ParticleArrays pa, int buf, int all, unsigned char* __restrict__ flag,
+        int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
+        int* __restrict__ cell_items, int* __restrict__ status, const LbmConst c) {
   const int p = blockIdx.x;
-  if (skip_fixed && pa.fixed[p]) return;
   const double xn = pa.x[buf][p], yn = pa.y[buf][p], r = pa.r[p];
+  if (threadIdx.x == 0) {
+    int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
+    ci = min(max(ci, 0), ncx - 1);
+    cj = min(max(cj, 0), ncy - 1);
+    const int cidx = cj * ncx + ci;
+    const int slot = atomicAdd(&cell_count[cidx], 1);
+    if (slot < CELL_CAP) cell_items[cidx * CELL_CAP + slot] = p;
+    else atomicOr(status, ST_CELL_OVERFLOW);
+  }
+  if (!all && pa.fixed[p]) return;
+  const bool sweep = all || pa.ovl[p] != 0;
+  const double xo = pa.x[buf ^ 1][p], yo = pa.y[buf ^ 1][p];
   int i0, i1, j0, j1;
   zone_of(xn, yn, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, total = W * (j1 - j0 + 1);
-  for (int t = threadIdx.x; t < total; t += PT) {
-    const int i = i0 + t % W, j = j0 + t / W;
-    if (i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
-    if (!inside_disc((double)i, (double)j, xn, yn, r)) continue;
+  for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
+    if (!inside_disc((double)i, (double)j, xn, yn, r)) return;
+    if (!sweep && inside_disc((double)i, (double)j, xo, yo, r)) return;   // already ours
     const long long x = (long long)j * c.px + i;
-    if (owner[x] == p) continue;
+    if (owner[x] == p) return;
     const int prev = atomicMin(&owner[x], p);
     if (prev != p) flag[x] = 1;
-  }
+    if (prev < p) pa.ovl[p] = 1;                              // a lower id keeps the node
+    else if (prev != OWNER_NONE) pa.ovl[prev] = 1;            // taken from a higher id
+  });
 }
 
 } // namespace
@@ -352,20 +450,26 @@ k_cover(ParticleArrays pa, int buf, int skip_fixed, unsigned char* __restrict__ 
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_build_links<<<h->np, PT, 0, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r,
-                                      h->flag, h->owner, h->la, h->status_dev, h->C);
+  const size_t smem = (size_t)h->la.cap * 5 + 16;
+  k_build_links<<<h->np, LB_WARPS * 32, smem, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer],
+                                                    h->pa.r, h->pa.ovl, h->flag, h->owner, h->la,
+                                                    h->status_dev, h->C);
 }
 
-void launch_cells_and_integrate(lbm* h) {
+int particles_configure(lbm* h) {
+  const size_t smem = (size_t)h->la.cap * 5 + 16;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(k_build_links, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return -1;
+  return 0;
+}
+
+void launch_integrate(lbm* h) {
   if (h->np == 0) return;
-  const int blocks = (h->np + 127) / 128;
-  h->launches++;
-  k_cells_build<<<blocks, 128, 0, h->chain>>>(h->pa.x[h->cur], h->pa.y[h->cur], h->np, h->cell,
-                                               h->ncx, h->ncy, h->cell_count, h->cell_items,
-                                               h->status_dev, h->newborn_count);
   h->launches++;
   k_integrate<<<(h->np + IW - 1) / IW, IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
-                                             h->cell_count, h->cell_items, h->status_dev, h->C);
+                                             h->cell_count, h->cell_items, h->status_dev,
+                                             h->newborn_count, h->C);
 }
 
 void launch_uncover(lbm* h) {
@@ -376,10 +480,11 @@ void launch_uncover(lbm* h) {
                                          h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
 }
 
-// after add_particles every particle (fixed ones too) is rasterised; during stepping the fixed
-// ones never move
+// after add_particles every particle (fixed ones too) is rasterised with a full sweep; during
+// stepping the fixed ones never move
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_cover<<<h->np, PT, 0, st>>>(h->pa, which_buffer, h->primed ? 1 : 0, h->flag, h->owner, h->C);
+  k_cover<<<h->np, PT, 0, st>>>(h->pa, which_buffer, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
+                                h->ncx, h->ncy, h->cell_count, h->cell_items, h->status_dev, h->C);
 }
