@@ -174,24 +174,17 @@ def main():
 
     import numpy as np
     import torch
-    import torch.distributed as dist
-    from paper_2308_16597_b200 import binding
+    from paper_2308_16597_b200 import binding, replicas
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.rank_info()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+    replicas.init("nccl", dev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dev)
 
     K, W = args.steps, max(args.warmup, 3)
     w = wl.config(args.config)
@@ -217,11 +210,8 @@ def main():
     launches = sim.kernel_launches() - l0
     ms = ev0.elapsed_time(ev1)
     clk = clocks.stop(t0, t1)
-    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max = float(tmax.item())
-    value = world * n * K / (ms_max * 1e-3) / 1e6
+    ms_max = replicas.max_over_ranks(ms, dev)
+    value = replicas.whole_job_mlups(n, K, ms_max, world)
 
     # ---------------- per-kernel CUDA-event durations -> roofline.  Two separate passes after the
     # timed region: (a) strictly sequential on one stream (each kernel alone on the GPU), (b) as
@@ -291,15 +281,13 @@ def main():
         barrier()
         te = time.perf_counter() - te0
         d2h = 4 * n * 8 + n + sum(int(v.nbytes) for v in pr.values())
-        tt = torch.tensor([te], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        te_max = replicas.max_over_ranks(te, dev)
         assert np.isfinite(res["rho"]).all()
-        e2e = {"value": world * n * K / float(tt.item()) / 1e6, "unit": "MLUPS",
+        e2e = {"value": replicas.whole_job_mlups(n, K, te_max * 1e3, world), "unit": "MLUPS",
                "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                "job": "create + set_temperature(host) + add_particles(host) + step(K) + "
                       "get_fields(rho,ux,uy,T,flag -> pinned host) + get_particles",
-               "job_seconds": float(tt.item())}
+               "job_seconds": te_max}
         s2.close()
 
     # ---------------- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
@@ -328,8 +316,7 @@ def main():
                 "context": {"paper_single_gpu_mlups": 1750, "paper_hardware": "1x A100, OpenACC "
                             "(PAPER.md:271-281; d=40, Pr=5 workload: context, not like-for-like)"}}
         print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    replicas.shutdown()
 
 
 def read_traffic():
