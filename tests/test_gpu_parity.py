@@ -197,6 +197,21 @@ def test_small_sedimentation_many_particles(gpu, ob, wl):
     assert_links_after_injection(gpu, ob, wl, w, o.particles())
 
 
+def test_paper_table4_arrangement_small(gpu, ob, wl):
+    """The paper's own benchmark set-up (Table 4: d = 40, rho-ratio 1.1, nu = 0.01,
+    Pr = 5, regular lines of particles at pitch 50, Eq. 15 as printed: quadratic, s = 3) at a size
+    the oracle does in seconds: 4 lines of 8 particles in 400 x 300.  With a 10-unit gap between
+    neighbours every particle's interpolation stencils reach into the gap next door."""
+    w = wl.paper_table4(cols=8, lines=4, ny=300, name="table4_small")
+    # break the lattice symmetry a little so that the particles actually interact
+    rng = np.random.default_rng(40)
+    n = w.n_particles
+    w.particles.update(ux=1e-3 * rng.uniform(-1, 1, n), uy=-5e-3 * rng.uniform(0, 1, n),
+                       omega=1e-4 * rng.uniform(-1, 1, n))
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 100], r_min=20.0)
+    assert_links_after_injection(gpu, ob, wl, w, o.particles())
+
+
 def test_overlap_and_sequential_modes_agree_bitwise(gpu, wl):
     """The schedule with the particle update chain on its own stream, concurrent with the lattice
     kernel, must give the same bits as the strictly sequential single-stream schedule."""

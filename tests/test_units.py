@@ -107,3 +107,22 @@ def test_variable_diameter_sampler(wl):
     d = w.particles["diam"]
     assert d.min() >= 12 and d.max() <= 24 and d.std() > 1
     assert w.params["max_links_per_particle"] == 12 * 28 - 12
+
+
+def test_paper_table4_workload_matches_the_printed_table(wl):
+    """PAPER.md:232 and Table 4: 4,800 particles of d = 40 in 4000 x 4000, volume fraction 37.7 %,
+    Ar = 22.4, Gr_p = 60, Pr = 5; 60 lines of 80 particles, none touching a wall or a neighbour."""
+    import math
+    import numpy as np
+    w = wl.config(5)
+    P, p = w.particles, w.params
+    assert (w.nx, w.ny, w.n_particles) == (4000, 4000, 4800)
+    assert len(np.unique(P["y"])) == 60 and len(np.unique(P["x"])) == 80
+    assert round(100 * w.n_particles * math.pi * 20.0 ** 2 / (w.nx * w.ny), 1) == 37.7
+    assert round(math.sqrt(p["g"] * 40.0 ** 3 * 0.1) / p["nu"], 1) == 22.4
+    assert round(p["gbeta"] * 1.0 * 40.0 ** 3 / p["nu"] ** 2) == 60
+    assert p["nu"] / p["kappa"] == 5.0
+    assert (p["rep_power"], p["rep_s"], p["rep_eps"]) == (2, 3.0, 1e-3)
+    assert P["x"].min() - 20.0 > -0.5 and P["x"].max() + 20.0 < w.nx - 0.5
+    assert P["y"].max() + 20.0 < w.ny - 0.5 and P["y"].min() > 0.25 * w.ny
+    assert np.diff(np.unique(P["x"])).min() == 50.0
