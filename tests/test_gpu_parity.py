@@ -197,6 +197,58 @@ def test_small_sedimentation_many_particles(gpu, ob, wl):
     assert_links_after_injection(gpu, ob, wl, w, o.particles())
 
 
+def test_discs_driven_into_overlap(gpu, ob, wl):
+    """Degenerate case of the flag/owner bookkeeping: with a repulsion too weak to matter, fast
+    particles run into each other and into a fixed one, so discs share lattice nodes for many
+    steps (lowest id owns a shared node; a node uncovered by one particle while
+    still inside another stays solid).  Flags, links, fields and particle states are compared
+    with the oracle at several stages of the overlap: pair (0, 1) lower id arriving from the left,
+    pair (2, 3) higher id running into a fixed lower id, pair (4, 5) lower id running into a fixed
+    higher id, and (6, 7) overlapping and separating again in y."""
+    nx, ny = 330, 150
+    x = np.array([40.0, 66.0, 130.0, 156.0, 230.0, 204.0, 290.0, 290.5])
+    y = np.array([40.0, 41.0, 40.5, 40.0, 40.0, 41.5, 95.0, 122.0])
+    d = np.array([20.0, 20.0, 22.0, 18.0, 20.0, 24.0, 20.0, 21.0])
+    ux = np.array([0.12, -0.05, 0.0, -0.15, 0.0, 0.14, 0.0, 0.0])
+    uy = np.array([0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.12, -0.1])
+    fixed = np.array([0, 0, 1, 0, 1, 0, 0, 0], dtype=np.uint8)
+    n = len(x)
+    p = wl.default_params()
+    p.update(g=0.0, gbeta=1e-5, rep_s=2.0, rep_eps=1e3, rep_power=1, wall_T_type=[1, 1, 1, 1],
+             max_particles=n, max_links_per_particle=wl.max_links_for_diameter(24.0))
+    parts = dict(x=x, y=y, diam=d, rho_ratio=np.full(n, 8.0), T_w=np.linspace(0.3, 1.0, n),
+                 ux=ux, uy=uy, omega=np.zeros(n), fixed=fixed)
+    w = wl.Workload("overlap", nx, ny, p, 120, 120, particles=parts)
+    g, o = both(gpu, ob, w)
+    done = 0
+    seen_overlap = False
+    for c in (1, 30, 60, 61, 90, 120):
+        g.step(c - done)
+        o.step(c - done)
+        done = c
+        assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+        assert_particles_close(g.particles(), o.particles(), r_min=9.0, steps=c)
+        po = o.particles()
+        gap01 = np.hypot(po["x"][0] - po["x"][1], po["y"][0] - po["y"][1]) - 20.0
+        seen_overlap |= gap01 < -1.0
+    assert seen_overlap, "the case no longer drives the discs into overlap"
+
+
+def test_large_particle_wide_zone(gpu, ob, wl):
+    """A d = 70.6 particle (zone 75 nodes wide: three 32-column chunks, several rounds of the link
+    builder, 12N-12 = 876 slots) next to a d = 12 one, both moving."""
+    nx, ny = 200, 170
+    p = wl.default_params()
+    p.update(g=1e-4, gbeta=1e-5, wall_T_type=[1, 0, 1, 1], max_particles=2,
+             max_links_per_particle=wl.max_links_for_diameter(70.6))
+    parts = dict(x=np.array([90.3, 150.0]), y=np.array([100.2, 40.0]), diam=np.array([70.6, 12.0]),
+                 rho_ratio=np.array([1.2, 1.5]), T_w=np.array([1.0, 0.4]),
+                 ux=np.array([0.02, -0.01]), uy=np.array([-0.03, 0.02]), omega=np.array([1e-3, -2e-3]))
+    w = wl.Workload("large", nx, ny, p, 60, 60, particles=parts)
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 60], r_min=6.0)
+    assert_links_after_injection(gpu, ob, wl, w, o.particles())
+
+
 def test_paper_table4_arrangement_small(gpu, ob, wl):
     """The paper's own benchmark set-up (Table 4: d = 40, rho-ratio 1.1, nu = 0.01,
     Pr = 5, regular lines of particles at pitch 50, Eq. 15 as printed: quadratic, s = 3) at a size
