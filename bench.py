@@ -298,7 +298,7 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         edge = 600 if args.config >= 2 else (512 if args.config == 1 else 0)
-        steps_cpu = 60 if args.config >= 1 else 400
+        steps_cpu = 200 if args.config >= 1 else 4000    # about 15 s of single-thread work
         wc, v, dt = time_oracle(wl, args.config, edge, steps_cpu, 1)
         cpu = {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle",
                "sample": f"{wc.nx}x{wc.ny} sample of config {args.config} ({wc.n_particles} "
