@@ -2,6 +2,7 @@
 // launch sequence (SURVEY.md 3 / 7 "legal fused ordering"), read-out copies and event profiling.
 // No torch types, no exceptions across the boundary, no cudaMalloc of lattice state: everything
 // lives in the caller's workspace (only the pinned status word and the events are ours).
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -206,6 +207,26 @@ int check_status(lbm* h) {
   return LBM_OK;
 }
 
+// CTAs of a particle-chain kernel while it runs under the lattice kernel (DESIGN.md "Step
+// schedule").  Measured on B200: the lattice kernel keeps its speed when other work holds up to
+// two of its nine CTA slots per SM and loses 7 % at three; a chain CTA under a saturated memory
+// system needs about 30 us per d = 20 particle for its three zone kernels (about 70 us at d = 40).
+// Pick the fewest CTAs per SM (at least 2) with which the chain still ends within 70 % of the
+// lattice kernel's expected duration (224 B per node at 6 TB/s); LBM_CHAIN_CTAS_PER_SM overrides
+// (0 = one CTA per particle).
+void size_chain(lbm* h) {
+  if (const char* e = getenv("LBM_CHAIN_CTAS_PER_SM")) {
+    h->chain_ctas = atoi(e) * h->sm_count;
+    return;
+  }
+  if (h->np == 0) { h->chain_ctas = 0; return; }
+  const double sc_us = (double)h->nx * h->ny * 224.0 / 6.0e6;
+  const double tau_us = 30.0 * std::max(1.0, std::pow(h->d_max / 20.0, 1.3));
+  double per_sm = std::ceil(h->np * tau_us / (h->sm_count * 0.7 * sc_us));
+  per_sm = std::min(std::max(per_sm, 2.0), 16.0);
+  h->chain_ctas = (int)per_sm * h->sm_count;
+}
+
 void prime(lbm* h) {
   if (h->primed) return;
   Timed t(h, K_INIT, h->stream);
@@ -287,6 +308,13 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
       cudaGetLastError();
       h->chain_own = nullptr;
     }
+  }
+  {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (h->sm_count <= 0) h->sm_count = 148;
+    h->chain_ctas = 0;   // set by add_particles (size_chain)
   }
   // initial state: fluid everywhere, f = f_eq(rho0, 0), g = g_eq(T0, 0)
   const size_t nn = (size_t)h->px * ny;
@@ -413,6 +441,7 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   CUDA_OK(h, cudaMemsetAsync(h->pa.ovl + n0, 0, n, h->stream));
   h->np = nt;
   h->d_max = dmax;
+  size_chain(h);
   h->cell = std::max(dmax + h->P.rep_s, MIN_CELL);
   h->ncx = (int)std::ceil(h->nx / h->cell) + 1;
   h->ncy = (int)std::ceil(h->ny / h->cell) + 1;

@@ -86,6 +86,8 @@ struct lbm {
   cudaStream_t chain_own;    // the stream we created (NULL if creation failed)
   cudaEvent_t ev_fork, ev_join;
   int overlap;               // 1: chain runs on `chain_own` concurrently with the lattice kernel
+  int chain_ctas;            // CTAs per chain kernel while it runs under the lattice kernel (0 = one per item)
+  int sm_count;
   int links_ready;           // the index array holds the links of the current particle positions
   double *A, *B;             // 14 planes each
   unsigned char* flag;

@@ -65,11 +65,11 @@ __global__ void __launch_bounds__(LB_WARPS * 32)
 k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
               const double* __restrict__ pr, const unsigned char* __restrict__ ovl,
               const unsigned char* __restrict__ flag, const int* __restrict__ owner, LinkArrays la,
-              int* __restrict__ status, const LbmConst c) {
+              int np, int* __restrict__ status, const LbmConst c) {
   extern __shared__ int s_node[];                           // la.cap packed nodes, then la.cap dir bytes
   unsigned char* s_dir = (unsigned char*)(s_node + la.cap);
   __shared__ int s_warp[LB_WARPS];
-  const int p = blockIdx.x;
+  for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const double xc = px_[p], yc = py_[p], r = pr[p];
   const bool check_owner = ovl[p] != 0;
   int i0, i1, j0, j1;
@@ -217,6 +217,8 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
     la.dir[base + s] = (unsigned char)(al | (behind << LINK_BEHIND_SHIFT));
   }
   if (threadIdx.x == 0) la.count[p] = nl;
+  __syncthreads();   // the shared list is reused by the next particle
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -248,11 +250,11 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   // the newborn list of the previous step has been consumed (refill, then the bounce-back kernel
   // of this step cleared its flags; both precede this kernel)
   if (blockIdx.x == 0 && threadIdx.x == 0) *nb_count = 0;
-  const int ia = blockIdx.x * IW + (threadIdx.x >> 5);
-  if (ia >= np) return;
   const unsigned FULL = 0xffffffffu;
   const int nxt = cur ^ 1;
   const double PI = 3.14159265358979323846;
+  // grid-size agnostic: warp w of the grid takes particles w, w + (warps in the grid), ...
+  for (int ia = blockIdx.x * IW + (threadIdx.x >> 5); ia < np; ia += gridDim.x * IW) {
   const double ax = pa.x[cur][ia], ay = pa.y[cur][ia], ar = pa.r[ia], ratio = pa.rho_ratio[ia];
   const double Ca = PI * ar * ar * (ratio * c.rho0 - c.rho0) * c.g;
   double Fx = pa.Fx[ia], Fy = pa.Fy[ia];
@@ -318,7 +320,7 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
       if (lane == src) has = false;
     }
   }
-  if (lane != 0) return;
+  if (lane != 0) continue;
   if (!c.periodic_x) {
     const double dW = (ax + 0.5) - ar;
     if (dW <= c.rep_s) Fx += repulsion_mag(Ca, c, dW);
@@ -353,6 +355,7 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   pa.omega[nxt][ia] = om;
   if (!(isfinite(x) && isfinite(y) && isfinite(th) && isfinite(ux) && isfinite(uy) && isfinite(om)))
     atomicOr(status, ST_NONFINITE);
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -371,15 +374,15 @@ __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const L
 // Phase A: nodes owned by p that the disc at its NEW position no longer covers become newborn
 // candidates (flag 2, owner NONE) and are appended to the newborn list.
 __global__ void __launch_bounds__(PT)
-k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __restrict__ owner,
+k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, int* __restrict__ owner,
           int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
           int* __restrict__ status, int* __restrict__ cell_count, int ncells, const LbmConst c) {
-  const int p = blockIdx.x;
   // the repulsion grid of this step has been consumed by k_integrate: zero it; k_cover refills it
   // with the new positions for the next step
-  for (int k = p * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count[k] = 0;
-  if (pa.fixed[p]) return;
+  for (int k = blockIdx.x * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count[k] = 0;
   const int nxt = cur ^ 1;
+  for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
+  if (pa.fixed[p]) continue;
   const double xo = pa.x[cur][p], yo = pa.y[cur][p], r = pa.r[p];
   const double xn = pa.x[nxt][p], yn = pa.y[nxt][p];
   int i0, i1, j0, j1;
@@ -399,6 +402,7 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
       atomicOr(status, ST_NEWBORN_OVERFLOW);
     }
   });
+  }
 }
 
 // Phase B: every node inside the disc at the position in buffer `buf` is solid; the lowest
@@ -414,10 +418,10 @@ k_uncover(ParticleArrays pa, int cur, unsigned char* __restrict__ flag, int* __r
 // Thread 0 also enters the particle into the repulsion grid of the step that will use this
 // position (k_uncover has zeroed the counts).
 __global__ void __launch_bounds__(PT)
-k_cover(ParticleArrays pa, int buf, int all, unsigned char* __restrict__ flag,
+k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
         int* __restrict__ cell_items, int* __restrict__ status, const LbmConst c) {
-  const int p = blockIdx.x;
+  for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const double xn = pa.x[buf][p], yn = pa.y[buf][p], r = pa.r[p];
   if (threadIdx.x == 0) {
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
@@ -428,7 +432,7 @@ k_cover(ParticleArrays pa, int buf, int all, unsigned char* __restrict__ flag,
     if (slot < CELL_CAP) cell_items[cidx * CELL_CAP + slot] = p;
     else atomicOr(status, ST_CELL_OVERFLOW);
   }
-  if (!all && pa.fixed[p]) return;
+  if (!all && pa.fixed[p]) continue;
   const bool sweep = all || pa.ovl[p] != 0;
   const double xo = pa.x[buf ^ 1][p], yo = pa.y[buf ^ 1][p];
   int i0, i1, j0, j1;
@@ -443,17 +447,28 @@ k_cover(ParticleArrays pa, int buf, int all, unsigned char* __restrict__ flag,
     if (prev < p) pa.ovl[p] = 1;                              // a lower id keeps the node
     else if (prev != OWNER_NONE) pa.ovl[prev] = 1;            // taken from a higher id
   });
+  }
 }
 
 } // namespace
+
+// CTAs of a particle-chain kernel.  On the library's own stream (concurrent with the lattice
+// kernel) the chain is throttled to h->chain_ctas CTAs: the lattice kernel keeps its full speed
+// when it loses up to two of its nine CTA slots per SM to other work and the chain has the whole
+// lattice kernel to hide under.  Alone on the caller's stream
+// (set-up, sequential mode) a kernel gets one CTA per work item.
+static int chain_grid(const lbm* h, int items, cudaStream_t st) {
+  if (st == h->chain_own && h->chain_ctas > 0) return items < h->chain_ctas ? items : h->chain_ctas;
+  return items;
+}
 
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
   const size_t smem = (size_t)h->la.cap * 5 + 16;
-  k_build_links<<<h->np, LB_WARPS * 32, smem, st>>>(h->pa.x[which_buffer], h->pa.y[which_buffer],
-                                                    h->pa.r, h->pa.ovl, h->flag, h->owner, h->la,
-                                                    h->status_dev, h->C);
+  k_build_links<<<chain_grid(h, h->np, st), LB_WARPS * 32, smem, st>>>(
+      h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r, h->pa.ovl, h->flag, h->owner, h->la,
+      h->np, h->status_dev, h->C);
 }
 
 int particles_configure(lbm* h) {
@@ -467,7 +482,7 @@ int particles_configure(lbm* h) {
 void launch_integrate(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_integrate<<<(h->np + IW - 1) / IW, IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
+  k_integrate<<<chain_grid(h, (h->np + IW - 1) / IW, h->chain), IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
                                              h->cell_count, h->cell_items, h->status_dev,
                                              h->newborn_count, h->C);
 }
@@ -475,7 +490,7 @@ void launch_integrate(lbm* h) {
 void launch_uncover(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_uncover<<<h->np, PT, 0, h->chain>>>(h->pa, h->cur, h->flag, h->owner, h->newborn_node,
+  k_uncover<<<chain_grid(h, h->np, h->chain), PT, 0, h->chain>>>(h->pa, h->cur, h->np, h->flag, h->owner, h->newborn_node,
                                          h->newborn_pid, h->newborn_count, h->newborn_cap,
                                          h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
 }
@@ -485,6 +500,6 @@ void launch_uncover(lbm* h) {
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_cover<<<h->np, PT, 0, st>>>(h->pa, which_buffer, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
+  k_cover<<<chain_grid(h, h->np, st), PT, 0, st>>>(h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
                                 h->ncx, h->ncy, h->cell_count, h->cell_items, h->status_dev, h->C);
 }
