@@ -71,18 +71,28 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     const bool lo = q <= 0.5;
     const long long x1 = nbehind >= 1 ? node_at(c, i, j, -ex, -ey) : (long long)xf;
     const long long x2 = nbehind == 2 ? node_at(c, i, j, -2 * ex, -2 * ey) : (long long)xf;
-    const double* Fi = A + (long long)al * c.ps;
-    const double* Fb = A + (long long)ab * c.ps;
-    const double fi0 = Fi[xf];
-    const double fa = lo ? Fi[x1] : Fb[xf];      // f_i(x_f - e_i)    | f_ibar(x_f)
-    const double fc = lo ? Fi[x2] : Fb[x1];      // f_i(x_f - 2 e_i)  | f_ibar(x_f - e_i)
-    double gi0 = 0.0, gb0 = 0.0, gi1 = 0.0;
+    // Axis directions (alpha <= 4) live in pair planes (f_k, g_k): one 16-byte access brings the
+    // flow and the temperature population of a node and direction together, and the bounced pair
+    // is parked with one 16-byte store.
+    double fi0, fa, fc, gi0 = 0.0, gb0 = 0.0, gi1 = 0.0;
     if (al <= 4) {
-      const double* Gi = A + (long long)(9 + al) * c.ps;
-      const double* Gb = A + (long long)(9 + ab) * c.ps;
-      gi0 = Gi[xf];
-      gb0 = Gb[xf];
-      gi1 = Gi[x1];
+      const double* Pi = A + 2 * (long long)al * c.ps;
+      const double* Pb = A + 2 * (long long)ab * c.ps;
+      const double2 a0 = *reinterpret_cast<const double2*>(Pi + 2 * (long long)xf);
+      const double2 b0 = *reinterpret_cast<const double2*>(Pb + 2 * (long long)xf);
+      const double2 a1 = *reinterpret_cast<const double2*>(Pi + 2 * x1);
+      fc = lo ? Pi[2 * x2] : Pb[2 * x1];        // f_i(x_f - 2 e_i)  | f_ibar(x_f - e_i)
+      fi0 = a0.x;
+      fa = lo ? a1.x : b0.x;                    // f_i(x_f - e_i)    | f_ibar(x_f)
+      gi0 = a0.y;
+      gb0 = b0.y;
+      gi1 = a1.y;
+    } else {
+      const double* Fi = A + (long long)(al + 5) * c.ps;
+      const double* Fb = A + (long long)(ab + 5) * c.ps;
+      fi0 = Fi[xf];
+      fa = lo ? Fi[x1] : Fb[xf];
+      fc = lo ? Fi[x2] : Fb[x1];
     }
     // wall point and wall velocity u_w = U_c + Omega x (x_w - x_c)
     const double rwx = ((double)i + q * ex) - xc;
@@ -107,7 +117,6 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
       }
     }
     const long long xb = (long long)(j + ey) * c.px + (i + ex);   // solid node of the link
-    A[(long long)ab * c.ps + xb] = fbb;                           // parked for the pull at x_f
     if (al <= 4) {
       double cd2 = 0.0, cd4 = 1.0;
       if (nbehind >= 1) {
@@ -117,7 +126,10 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
         gi1 = 0.0;
       }
       const double gbb = (-gi0 + cd2 * gi1 + cd2 * gb0) + cd4 * (2.0 * c.wT * Tw);
-      A[(long long)(9 + ab) * c.ps + xb] = gbb;
+      // parked for the pull at x_f: the pair (f_ibar, g_ibar) of the solid node
+      *reinterpret_cast<double2*>(A + 2 * (long long)ab * c.ps + 2 * xb) = make_double2(fbb, gbb);
+    } else {
+      A[(long long)(ab + 5) * c.ps + xb] = fbb;
     }
     // Eqs. (13), (14)
     const double dpx = fi0 * ((double)ex - uwx) - fbb * ((double)b_ex[ab] - uwx);
@@ -200,7 +212,7 @@ k_refill(const double* __restrict__ A, double* __restrict__ B,
     if (lane < 27 && st < nvalid) {
       const int ci = (int)(snode % c.px), cj = (int)(snode / c.px);
       const long long src = node_at(c, ci, cj, -b_ex[k], -b_ey[k]);
-      v = src >= 0 ? A[(long long)k * c.ps + src] : A[(long long)b_opp[k] * c.ps + snode];
+      v = src >= 0 ? A[f_at(k, src, c.ps)] : A[f_at(b_opp[k], snode, c.ps)];
     }
     double f[9], g[5];
 #pragma unroll
@@ -244,7 +256,8 @@ k_refill(const double* __restrict__ A, double* __restrict__ B,
     for (int kk = 0; kk < 9; ++kk) if (lane == kk) out = f[kk];
 #pragma unroll
     for (int kk = 0; kk < 5; ++kk) if (lane == 9 + kk) out = g[kk];
-    if (lane < 14) B[(long long)lane * c.ps + x] = out;
+    if (lane < 9) B[f_at(lane, x, c.ps)] = out;
+    else if (lane < 14) B[g_at(lane - 9, x, c.ps)] = out;
     // flag[x] stays 2 until the newborn flags are cleared (next step's bounce-back kernel or a
     // read-out): other warps of this kernel still test their stencil nodes against it
   }

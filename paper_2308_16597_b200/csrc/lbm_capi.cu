@@ -524,20 +524,14 @@ int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, dou
   }
   if (f || g) {
     // f, g are defined as the post-collision populations; before the first step the resident
-    // state is still pre-collision, so collide it into the scratch copy (stream order keeps the
-    // macroscopic copies above ahead of this overwrite of B)
-    const double* src = h->A;
-    if (!h->primed) {
-      launch_init_collide(h, h->B);
-      src = h->B;
-    }
-    const size_t row = (size_t)h->nx * sizeof(double), pitch = (size_t)h->px * sizeof(double);
-    for (int k = 0; k < 14; ++k) {
-      double* dst = k < 9 ? (f ? f + (size_t)k * n : nullptr) : (g ? g + (size_t)(k - 9) * n : nullptr);
-      if (!dst) continue;
-      CUDA_OK(h, cudaMemcpy2DAsync(dst, row, src + (size_t)k * h->ps, pitch, row, h->ny,
-                                   cudaMemcpyDeviceToHost, h->stream));
-    }
+    // state is still pre-collision and the export kernel collides on the fly.  The dense
+    // population-major planes are staged in B (dead between steps; stream order keeps the
+    // macroscopic copies above ahead of this overwrite)
+    double* fd = h->B;
+    double* gd = h->B + 9 * n;
+    launch_export(h, f ? fd : nullptr, g ? gd : nullptr);
+    if (f) CUDA_OK(h, cudaMemcpyAsync(f, fd, 9 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (g) CUDA_OK(h, cudaMemcpyAsync(g, gd, 5 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   }
   if (flag)
     CUDA_OK(h, cudaMemcpy2DAsync(flag, h->nx, h->flag, h->px, h->nx, h->ny, cudaMemcpyDeviceToHost, h->stream));

@@ -1,9 +1,13 @@
 // lbm_internal.cuh -- shared declarations of the CUDA path (product).  Not part of the C ABI.
 //
-// HBM layout: structure of arrays, fp64.
-//   populations: 14 planes (f0..f8, g0..g4), plane k at base + k*ps doubles, node (i,j) at j*px + i
-//   px = nx rounded up to 16 doubles (128 B rows -> every row start is sector- and TMA-aligned),
-//   ps = px*ny rounded up to 32 doubles.  Two copies A (read) and B (written), swapped per step.
+// HBM layout: structure of arrays, fp64, node (i,j) at x = j*px + i,
+//   px = nx rounded up to 16 doubles, ps = px*ny rounded up to 32 doubles.
+//   populations: the D2Q5 directions k = 0..4 carry a flow AND a temperature population that
+//   stream along the same e_k, so they are stored as pairs: pair plane k (k = 0..4) at
+//   base + 2*k*ps holds (f_k(x), g_k(x)) at doubles 2x, 2x+1 (one 16-byte access per node and
+//   direction for the lattice kernel, the bounce-back kernel and the parked slot); the diagonal
+//   flow populations f5..f8 are plain planes at base + (k+5)*ps + x.  14*ps doubles per copy;
+//   two copies A (read) and B (written), swapped per step.
 //   flag : 1 byte/node, 0 fluid, 1 solid, 2 newborn (solid at t, fluid at t+1; only between the
 //          flag update and the refill kernel of one step)
 //   owner: int32/node, id of the lowest-numbered particle covering the node, OWNER_NONE = fluid
@@ -42,6 +46,14 @@ __device__ __forceinline__ void zone_of(double xc, double yc, double r, int& i0,
   i1 = (int)floor(__dadd_rn(xc, r)) + 1;
   j0 = (int)floor(__dsub_rn(yc, r)) - 1;
   j1 = (int)floor(__dadd_rn(yc, r)) + 1;
+}
+
+// double index of f_k / g_k of node x inside one copy of the populations
+__host__ __device__ __forceinline__ long long f_at(int k, long long x, long long ps) {
+  return k <= 4 ? 2 * k * ps + 2 * x : (k + 5) * ps + x;
+}
+__host__ __device__ __forceinline__ long long g_at(int k, long long x, long long ps) {
+  return 2 * k * ps + 2 * x + 1;
 }
 
 // constants every kernel needs; passed by value (lands in the constant bank)
@@ -125,6 +137,7 @@ void launch_stream_collide(lbm* h);        // on h->stream
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
 void launch_set_equilibrium(lbm* h);
+void launch_export(lbm* h, double* f_dense, double* g_dense);    // dense f[9][n], g[5][n], device
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
 // particles.cu (compiled with -fmad=false)
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st);

@@ -35,9 +35,8 @@ __device__ __forceinline__ void pull_boundary(const double* __restrict__ A, cons
     if (si < 0 || si >= c.nx) {
       if (c.periodic_x) si = (si + c.nx) % c.nx; else in = false;
     }
-    f[k] = in ? A[k * c.ps + (long long)sj * c.px + si] : A[opp_of(k) * c.ps + x];
+    f[k] = in ? A[f_at(k, (long long)sj * c.px + si, c.ps)] : A[f_at(opp_of(k), x, c.ps)];
   }
-  const double* G = A + 9 * c.ps;
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
     int si = i - ex_of(k), sj = j - ey_of(k);
@@ -47,46 +46,55 @@ __device__ __forceinline__ void pull_boundary(const double* __restrict__ A, cons
       if (c.periodic_x) si = (si + c.nx) % c.nx;
       else { in = false; wall = si < 0 ? 0 : 1; }
     }
-    if (in) g[k] = G[k * c.ps + (long long)sj * c.px + si];
+    if (in) g[k] = A[g_at(k, (long long)sj * c.px + si, c.ps)];
     else {
-      const double gb = G[opp_of(k) * c.ps + x];
+      const double gb = A[g_at(opp_of(k), x, c.ps)];
       g[k] = c.wall_type[wall] == 1 ? (2.0 * c.wT * c.wall_T[wall] - gb) : gb;
     }
   }
 }
 
-// one lattice update of node (i, j): pull, collide, store
+__device__ __forceinline__ double2 ldg2(const double* p) {
+  return __ldg(reinterpret_cast<const double2*>(p));
+}
+
+// one lattice update of node (i, j): pull, collide, store.  Interior nodes: five 16-byte loads of
+// the (f_k, g_k) pairs of the axis directions and four 8-byte loads of the diagonal f_k, each
+// coalesced across the warp (the pair planes shifted by one node stay 16-byte aligned); the same
+// nine accesses as stores.
 __device__ __forceinline__ void update_node(const double* __restrict__ A, double* __restrict__ B,
                                             const LbmConst& c, int i, int j) {
   const long long x = (long long)j * c.px + i;
+  const long long ps = c.ps;
   double f[9], g[5];
   if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
-    const double* __restrict__ F = A + x;
-    const long long ps = c.ps;
     const int px = c.px;
-    f[0] = __ldg(F);
-    f[1] = __ldg(F + 1 * ps - 1);
-    f[2] = __ldg(F + 2 * ps - px);
-    f[3] = __ldg(F + 3 * ps + 1);
-    f[4] = __ldg(F + 4 * ps + px);
-    f[5] = __ldg(F + 5 * ps - px - 1);
-    f[6] = __ldg(F + 6 * ps - px + 1);
-    f[7] = __ldg(F + 7 * ps + px + 1);
-    f[8] = __ldg(F + 8 * ps + px - 1);
-    g[0] = __ldg(F + 9 * ps);
-    g[1] = __ldg(F + 10 * ps - 1);
-    g[2] = __ldg(F + 11 * ps - px);
-    g[3] = __ldg(F + 12 * ps + 1);
-    g[4] = __ldg(F + 13 * ps + px);
+    const double* __restrict__ P = A + 2 * x;           // pair planes: node x at doubles 2x, 2x+1
+    const double2 p0 = ldg2(P);
+    const double2 p1 = ldg2(P + 2 * ps - 2);
+    const double2 p2 = ldg2(P + 4 * ps - 2 * px);
+    const double2 p3 = ldg2(P + 6 * ps + 2);
+    const double2 p4 = ldg2(P + 8 * ps + 2 * px);
+    const double* __restrict__ D = A + 10 * ps + x;     // diagonal planes f5..f8
+    f[5] = __ldg(D - px - 1);
+    f[6] = __ldg(D + ps - px + 1);
+    f[7] = __ldg(D + 2 * ps + px + 1);
+    f[8] = __ldg(D + 3 * ps + px - 1);
+    f[0] = p0.x; g[0] = p0.y;
+    f[1] = p1.x; g[1] = p1.y;
+    f[2] = p2.x; g[2] = p2.y;
+    f[3] = p3.x; g[3] = p3.y;
+    f[4] = p4.x; g[4] = p4.y;
   } else {
     pull_boundary(A, c, i, j, f, g);
   }
   mrt_collide(f, g, c);
-  double* __restrict__ O = B + x;
+  double* __restrict__ O = B + 2 * x;
 #pragma unroll
-  for (int k = 0; k < 9; ++k) O[k * c.ps] = f[k];
+  for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * ps) = make_double2(f[k], g[k]);
+  double* __restrict__ Q = B + 10 * ps + x;
 #pragma unroll
-  for (int k = 0; k < 5; ++k) O[(9 + k) * c.ps] = g[k];
+  for (int k = 0; k < 4; ++k) Q[k * ps] = f[5 + k];
 }
 
 // One thread per node, 128-thread CTAs along x.  Solid (1) and newborn (2) nodes do no lattice
@@ -115,9 +123,13 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   const unsigned lane = threadIdx.x & 31u;
   const unsigned grp = (m >> (lane & ~(unsigned)(SC_FILL - 1))) & ((1u << SC_FILL) - 1u);
   if (grp == 0u || i >= c.px) return;
-  double* __restrict__ O = B + (long long)j * c.px + i;
+  const long long x = (long long)j * c.px + i;
+  double* __restrict__ O = B + 2 * x;
 #pragma unroll
-  for (int k = 0; k < 14; ++k) O[k * c.ps] = 0.0;
+  for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
+  double* __restrict__ Q = B + 10 * c.ps + x;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) Q[k * c.ps] = 0.0;
 }
 
 // first step only: A holds the PRE-collision initial state f(x,0); collide it (in place when
@@ -131,14 +143,14 @@ k_init_collide(const double* A, double* O, const unsigned char* __restrict__ fla
   if (flag[x] != 0) return;
   double f[9], g[5];
 #pragma unroll
-  for (int k = 0; k < 9; ++k) f[k] = A[k * c.ps + x];
+  for (int k = 0; k < 9; ++k) f[k] = A[f_at(k, x, c.ps)];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) g[k] = A[(9 + k) * c.ps + x];
+  for (int k = 0; k < 5; ++k) g[k] = A[g_at(k, x, c.ps)];
   mrt_collide(f, g, c);
 #pragma unroll
-  for (int k = 0; k < 9; ++k) O[k * c.ps + x] = f[k];
+  for (int k = 0; k < 9; ++k) O[f_at(k, x, c.ps)] = f[k];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) O[(9 + k) * c.ps + x] = g[k];
+  for (int k = 0; k < 5; ++k) O[g_at(k, x, c.ps)] = g[k];
 }
 
 // f = f_eq(rho0, 0) = w_k rho0, g = g_eq(T0, 0) = wT_k T0 on every node (SURVEY 8(c) "Initial state")
@@ -149,10 +161,10 @@ __global__ void k_set_equilibrium(double* __restrict__ A, const LbmConst c) {
   const long long x = (long long)j * c.px + i;
   const double w[9] = {4.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 36, 1.0 / 36, 1.0 / 36, 1.0 / 36};
 #pragma unroll
-  for (int k = 0; k < 9; ++k) A[k * c.ps + x] = w[k] * c.rho0;
-  A[9 * c.ps + x] = c.wT0 * c.T0;
+  for (int k = 0; k < 9; ++k) A[f_at(k, x, c.ps)] = w[k] * c.rho0;
+  A[g_at(0, x, c.ps)] = c.wT0 * c.T0;
 #pragma unroll
-  for (int k = 1; k < 5; ++k) A[(9 + k) * c.ps + x] = c.wT * c.T0;
+  for (int k = 1; k < 5; ++k) A[g_at(k, x, c.ps)] = c.wT * c.T0;
 }
 
 // g = g_eq(T, u = 0) from a dense nx*ny temperature field (lbm_set_temperature)
@@ -162,9 +174,9 @@ __global__ void k_set_temperature(double* __restrict__ A, const double* __restri
   if (i >= c.nx) return;
   const long long x = (long long)j * c.px + i;
   const double t = T[(long long)j * c.nx + i];
-  A[9 * c.ps + x] = c.wT0 * t;
+  A[g_at(0, x, c.ps)] = c.wT0 * t;
 #pragma unroll
-  for (int k = 1; k < 5; ++k) A[(9 + k) * c.ps + x] = c.wT * t;
+  for (int k = 1; k < 5; ++k) A[g_at(k, x, c.ps)] = c.wT * t;
 }
 
 // read-out: dense nx*ny outputs
@@ -190,15 +202,41 @@ __global__ void k_macroscopic(const double* __restrict__ A, const unsigned char*
   }
   double f[9], g[5];
 #pragma unroll
-  for (int k = 0; k < 9; ++k) f[k] = A[k * c.ps + x];
+  for (int k = 0; k < 9; ++k) f[k] = A[f_at(k, x, c.ps)];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) g[k] = A[(9 + k) * c.ps + x];
+  for (int k = 0; k < 5; ++k) g[k] = A[g_at(k, x, c.ps)];
   double r, vx, vy, t;
   macroscopic(f, g, c, post, r, vx, vy, t);
   rho[o] = r;
   ux[o] = vx;
   uy[o] = vy;
   T[o] = t;
+}
+
+// read-out of the populations: dense population-major planes f[9][ny*nx], g[5][ny*nx] (the
+// layout lbm_get_fields hands out) from the paired device layout; `collide` = 1 before the first
+// step, when the resident state is still pre-collision
+__global__ void k_export(const double* __restrict__ A, const unsigned char* __restrict__ flag,
+                         int collide, double* __restrict__ fo, double* __restrict__ go, const LbmConst c) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y;
+  if (i >= c.nx) return;
+  const long long x = (long long)j * c.px + i;
+  const long long o = (long long)j * c.nx + i, n = (long long)c.nx * c.ny;
+  double f[9], g[5];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) f[k] = A[f_at(k, x, c.ps)];
+#pragma unroll
+  for (int k = 0; k < 5; ++k) g[k] = A[g_at(k, x, c.ps)];
+  if (collide && flag[x] == 0) mrt_collide(f, g, c);
+  if (fo) {
+#pragma unroll
+    for (int k = 0; k < 9; ++k) fo[k * n + o] = f[k];
+  }
+  if (go) {
+#pragma unroll
+    for (int k = 0; k < 5; ++k) go[k * n + o] = g[k];
+  }
 }
 
 inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1) / threads, ny); }
@@ -224,6 +262,12 @@ void launch_set_equilibrium(lbm* h) {
 void launch_set_temperature(lbm* h, const double* T_dev_dense) {
   h->launches++;
   k_set_temperature<<<grid_rows(h->nx, h->ny, 128), 128, 0, h->stream>>>(h->A, T_dev_dense, h->C);
+}
+
+void launch_export(lbm* h, double* f_dense, double* g_dense) {
+  h->launches++;
+  k_export<<<grid_rows(h->nx, h->ny, 128), 128, 0, h->stream>>>(h->A, h->flag, h->primed ? 0 : 1,
+                                                                f_dense, g_dense, h->C);
 }
 
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T) {
