@@ -37,19 +37,8 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
 }
 
 __global__ void __launch_bounds__(BT, 6)
-k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
-              unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
-              const int* __restrict__ nb_count, int nb_cap, const LbmConst c) {
+k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, const LbmConst c) {
   const int p = blockIdx.x;
-  // the nodes refilled by the previous step are ordinary fluid nodes from now on (this kernel
-  // reads no flags; the lattice kernel and the flag update of this step run after it)
-  {
-    const int nn = min(*nb_count, nb_cap);
-    for (int e = p * BT + threadIdx.x; e < nn; e += gridDim.x * BT) {
-      const int x = nb_node[e];
-      if (flag[x] == 2) flag[x] = 0;
-    }
-  }
   const int n = la.count[p];
   const long long base = (long long)p * la.cap;
   const double xc = pa.x[cur][p], yc = pa.y[cur][p];
@@ -172,10 +161,13 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
 // that was fluid at t (upstream slot of A, which holds a parked value where the upstream node is
 // solid; the node's own opposite slot at a cavity wall), so the 27 gathers are in flight
 // together; the extrapolation, the momentum constraint, Eq. (17) and the collision are then
-// evaluated redundantly by every lane and lane k < 14 stores plane k.
+// evaluated redundantly by every lane and lane k < 14 stores population k -- into the stash
+// record of the list entry, not into B: the kernel reads only A, the flags and the particle state
+// of t+1, so it runs in the particle chain UNDER the lattice kernel, whose zero fill of non-fluid
+// lanes may still touch the node's slots in B; k_refill_commit copies the record into B after it.
 constexpr int RW = 8;   // warps (newborn nodes) per CTA
 __global__ void __launch_bounds__(RW * 32)
-k_refill(const double* __restrict__ A, double* __restrict__ B,
+k_refill(const double* __restrict__ A, double* __restrict__ stash,
          const unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
          const int* __restrict__ nb_pid, const int* __restrict__ nb_count, int nb_cap,
          ParticleArrays pa, int cur, const LbmConst c) {
@@ -256,21 +248,36 @@ k_refill(const double* __restrict__ A, double* __restrict__ B,
     for (int kk = 0; kk < 9; ++kk) if (lane == kk) out = f[kk];
 #pragma unroll
     for (int kk = 0; kk < 5; ++kk) if (lane == 9 + kk) out = g[kk];
-    if (lane < 9) B[f_at(lane, x, c.ps)] = out;
-    else if (lane < 14) B[g_at(lane - 9, x, c.ps)] = out;
-    // flag[x] stays 2 until the newborn flags are cleared (next step's bounce-back kernel or a
-    // read-out): other warps of this kernel still test their stencil nodes against it
+    if (lane < 14) stash[(long long)e * 14 + lane] = out;
+    // flag[x] stays 2 until k_refill_commit: other warps of this kernel (and the link builder,
+    // which counts 2 as fluid) still test it
   }
 }
 
-// newborn nodes are ordinary fluid nodes from the next step on: done by the next step's
-// bounce-back kernel, and by this kernel at the end of an lbm_step call (before any read-out)
-__global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
-                                const int* __restrict__ nb_count, int nb_cap) {
+// After the lattice kernel: the refilled populations go into B and the newborn nodes become
+// ordinary fluid nodes.  16 threads per list entry (one per population, two idle), all in one warp.
+__global__ void k_refill_commit(double* __restrict__ B, const double* __restrict__ stash,
+                                unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
+                                const int* __restrict__ nb_count, int nb_cap, const LbmConst c) {
   const int n = min(*nb_count, nb_cap);
-  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
-    const int x = nb_node[e];
-    if (flag[x] == 2) flag[x] = 0;
+  const long long total = (long long)n * 16;
+  const int lane = threadIdx.x & 31;
+  for (long long t0 = (long long)blockIdx.x * blockDim.x + (threadIdx.x - lane); t0 < total;
+       t0 += (long long)gridDim.x * blockDim.x) {        // warp-uniform trip count
+    const long long t = t0 + lane;
+    const int e = (int)(t >> 4), k = (int)(t & 15);
+    int x = 0;
+    bool live = false;
+    if (e < n) {
+      x = nb_node[e];
+      live = flag[x] == 2;   // else covered again by another particle in the same step
+    }
+    __syncwarp();            // every thread of the entry has read the flag before it is cleared
+    if (live) {
+      if (k < 9) B[f_at(k, x, c.ps)] = stash[(long long)e * 14 + k];
+      else if (k < 14) B[g_at(k - 9, x, c.ps)] = stash[(long long)e * 14 + k];
+      else if (k == 15) flag[x] = 0;
+    }
   }
 }
 
@@ -279,24 +286,24 @@ __global__ void k_newborn_clear(unsigned char* __restrict__ flag, const int* __r
 void launch_bounce_back(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->flag, h->newborn_node,
-                                              h->newborn_count, h->newborn_cap, h->C);
+  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->C);
 }
 
-void launch_refill(lbm* h) {
+void launch_refill(lbm* h, cudaStream_t st) {
   if (h->np == 0) return;
   int blocks = (h->np + RW - 1) / RW;   // a handful of newborn nodes per particle and step
   if (blocks > 1184) blocks = 1184;
+  if (st == h->chain_own && h->chain_ctas > 0 && blocks > h->chain_ctas / 2) blocks = h->chain_ctas / 2;
   h->launches++;
-  k_refill<<<blocks, RW * 32, 0, h->stream>>>(h->A, h->B, h->flag, h->newborn_node, h->newborn_pid,
-                                               h->newborn_count, h->newborn_cap, h->pa, h->cur, h->C);
+  k_refill<<<blocks, RW * 32, 0, st>>>(h->A, h->stash, h->flag, h->newborn_node, h->newborn_pid,
+                                        h->newborn_count, h->newborn_cap, h->pa, h->cur ^ 1, h->C);
 }
 
-void launch_newborn_clear(lbm* h) {
+void launch_refill_commit(lbm* h) {
   if (h->np == 0) return;
-  int blocks = (h->np * 4 + 127) / 128;
+  int blocks = (h->np * 16 + 255) / 256;
   if (blocks > 1184) blocks = 1184;
   h->launches++;
-  k_newborn_clear<<<blocks, 128, 0, h->stream>>>(h->flag, h->newborn_node, h->newborn_count,
-                                                 h->newborn_cap);
+  k_refill_commit<<<blocks, 256, 0, h->stream>>>(h->B, h->stash, h->flag, h->newborn_node,
+                                                  h->newborn_count, h->newborn_cap, h->C);
 }

@@ -21,7 +21,7 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "integrate",
-    "flags_uncover", "flags_cover", "refill", "init_collide"};
+    "flags_uncover", "flags_cover", "refill", "init_collide", "refill_commit"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -109,6 +109,7 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   int* nb_node = c.take<int>((size_t)L.newborn_cap);
   int* nb_pid = c.take<int>((size_t)L.newborn_cap);
   int* nb_count = c.take<int>(1);
+  double* stash = c.take<double>((size_t)L.newborn_cap * 14);
   int* status = c.take<int>(1);
   if (h) {
     h->px = L.px;
@@ -125,6 +126,7 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
     h->newborn_node = nb_node;
     h->newborn_pid = nb_pid;
     h->newborn_count = nb_count;
+    h->stash = stash;
     h->newborn_cap = L.newborn_cap;
     h->status_dev = status;
   }
@@ -459,9 +461,10 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
 // Step schedule: the resident state A is f+(x,t), g+(x,t), the index array holds
 // the links of x_p(t).
 //   S0: bounce-back + momentum exchange (parks f_ibar(x_f,t+1) in solid slots of A, sums F, T_z)
-//   S1:   after it: integrate -> uncover -> cover -> links of x_p(t+1)      } concurrent with
-//   S0: fused pull-stream-collide A -> B over every node fluid at t          } each other
-//   S0: after both: refill of the nodes uncovered this step (A -> B), newborn flags cleared
+//   S1:   after it: integrate -> uncover -> cover -> refill (A -> stash)    } concurrent with
+//                    -> links of x_p(t+1)                                    } each other
+//   S0: fused pull-stream-collide A -> B over every node fluid at t          }
+//   S0: after both: refill commit (stash -> B at the uncovered nodes, newborn flags cleared)
 // Only the lattice kernel, the bounce-back kernel and the refill are on the critical path.
 int lbm_step(lbm_t* h, int nsteps) {
   if (!h) return LBM_E_ARG;
@@ -481,6 +484,7 @@ int lbm_step(lbm_t* h, int nsteps) {
       { Timed tm(h, K_INTEGRATE, S1); launch_integrate(h); }
       { Timed tm(h, K_UNCOVER, S1); launch_uncover(h); }
       { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1, S1); }
+      { Timed tm(h, K_REFILL, S1); launch_refill(h, S1); }
       { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h, h->cur ^ 1, S1); }
       h->cur ^= 1;
       if (S1 != S0) cudaEventRecord(h->ev_join, S1);
@@ -488,12 +492,11 @@ int lbm_step(lbm_t* h, int nsteps) {
     { Timed tm(h, K_STREAM_COLLIDE, S0); launch_stream_collide(h); }
     if (h->np > 0) {
       if (S1 != S0) cudaStreamWaitEvent(S0, h->ev_join, 0);
-      { Timed tm(h, K_REFILL, S0); launch_refill(h); }
+      { Timed tm(h, K_REFILL_COMMIT, S0); launch_refill_commit(h); }
     }
     std::swap(h->A, h->B);
     h->steps_done++;
   }
-  if (nsteps > 0) launch_newborn_clear(h);   // read-outs see flags 0/1 only
   return check_status(h);
 }
 

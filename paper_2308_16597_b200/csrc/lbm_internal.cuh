@@ -20,7 +20,7 @@
 #define OWNER_NONE 0x7f7f7f7f   // = cudaMemset(0x7f): larger than any particle id
 #define CELL_CAP 32          // particle centres per repulsion-grid cell
 #define MIN_CELL 16.0        // smallest repulsion-grid cell edge (workspace is sized for it)
-#define NEWBORN_PER_PARTICLE 64
+#define NEWBORN_PER_PARTICLE 32
 
 // status bits written by kernels, read once per lbm_step call
 #define ST_NONFINITE 1
@@ -30,7 +30,7 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
-  K_INIT, K_COUNT
+  K_INIT, K_REFILL_COMMIT, K_COUNT
 };
 
 // link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along
@@ -117,6 +117,7 @@ struct lbm {
   int* newborn_node;
   int* newborn_pid;
   int* newborn_count;
+  double* stash;             // 14 refilled populations per newborn-list entry
   int newborn_cap;
   int* status_dev;
   int* status_host;          // pinned
@@ -147,5 +148,5 @@ void launch_uncover(lbm* h);               // on h->chain
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st);
 // bounce_back.cu
 void launch_bounce_back(lbm* h);            // on h->stream
-void launch_refill(lbm* h);                 // on h->stream
-void launch_newborn_clear(lbm* h);          // on h->stream
+void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped
+void launch_refill_commit(lbm* h);          // on h->stream: stash -> B, newborn flags cleared
