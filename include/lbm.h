@@ -91,19 +91,22 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
 
 /* Advances nsteps time steps (each = rows a1..a6 of SURVEY 8(a); order PAPER.md:347-353):
  * bounce-back (Eqs. 9-12) + momentum exchange (Eqs. 13-14) on the links of x_p(t) -> { particle
- * update (Eqs. 7, 8, 15) -> flag update -> link build for x_p(t+1) } concurrently with { fused
- * pull-stream-collide (Eqs. 5, 6) } -> refill (Eqs. 16-17).
+ * update (Eqs. 7, 8, 15) -> flag update -> refill (Eqs. 16-17, into a stash) -> link build for
+ * x_p(t+1) } concurrently with { fused pull-stream-collide (Eqs. 5, 6) } -> refill commit.
  * Asynchronous kernels on the handle's stream, then ONE stream synchronisation at the end of the
  * call to read the device status word.  Errors: LBM_E_NONFINITE (a particle state is NaN/Inf,
  * checked once per call), LBM_E_CAPACITY (a link segment, cell or the newborn list overflowed;
  * the state is then undefined), LBM_E_CUDA. */
 int lbm_step(lbm_t* h, int nsteps);
 
-/* on = 1 (default): the particle update chain of a step (integrator, flag update, link build for
- * the next step) runs on the library's own high-priority stream concurrently with the lattice
- * kernel on the handle's stream; forked and joined with events inside every step, so the handle's
- * stream still orders everything for the caller.  on = 0: one stream, strictly sequential (same
- * results bit for bit on every fluid node; used for per-kernel timing and by the tests). */
+/* on = 1 (default): the particle update chain of a step (integrator, flag update, refill, link
+ * build for the next step) runs on the library's own high-priority stream concurrently with the
+ * lattice kernel on the handle's stream, as a few persistent CTAs per SM (chosen from the lattice
+ * and particle sizes; the environment variable LBM_CHAIN_CTAS_PER_SM, read by lbm_add_particles,
+ * overrides it, 0 = one CTA per particle); forked and joined with events inside every step, so
+ * the handle's stream still orders everything for the caller.  on = 0: one stream, strictly
+ * sequential, one CTA per particle (same results bit for bit on every fluid node; used for
+ * per-kernel timing and by the tests). */
 int lbm_set_overlap(lbm_t* h, int on);
 
 /* Readout.  Any pointer may be NULL = not wanted.

@@ -299,9 +299,7 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);
-    int prio = hi;
-    if (const char* e = getenv("LBM_CHAIN_PRIO")) prio = (e[0] == 'l') ? lo : (e[0] == 's' ? 0 : hi);
-    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, prio) == cudaSuccess &&
+    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess) {
       h->overlap = 1;

@@ -284,6 +284,34 @@ def test_overlap_and_sequential_modes_agree_bitwise(gpu, wl):
             assert np.array_equal(pa[k], pb[k]), k
 
 
+def test_chain_grid_size_does_not_change_results(gpu, wl, monkeypatch):
+    """The particle chain runs as a few persistent CTAs per SM under the lattice kernel; each CTA
+    then loops over many particles.  With 700 small particles and one CTA per SM (5 particles per
+    CTA) the results must equal, bit for bit, those of one CTA per particle."""
+    w = wl.sedimentation(900, 700, 700, seed=21, y_frac_lo=0.0, d_lo=8.0, d_hi=12.0, name="grid")
+    monkeypatch.setenv("LBM_CHAIN_CTAS_PER_SM", "1")
+    a = gpu.Simulation.from_workload(w)
+    monkeypatch.setenv("LBM_CHAIN_CTAS_PER_SM", "0")
+    b = gpu.Simulation.from_workload(w)
+    monkeypatch.delenv("LBM_CHAIN_CTAS_PER_SM")
+    c = gpu.Simulation.from_workload(w)          # the library's own choice
+    for n in (1, 40):
+        for s in (a, b, c):
+            s.step(n)
+        fb, pb = b.fields(populations=True), b.particles()
+        fluid = fb["flag"] == 0
+        for s in (a, c):
+            fs, ps = s.fields(populations=True), s.particles()
+            assert np.array_equal(fs["flag"], fb["flag"])
+            for k in ("f", "g"):
+                assert np.array_equal(fs[k][:, fluid], fb[k][:, fluid]), k
+            for k in pb:
+                assert np.array_equal(ps[k], pb[k]), k
+        La, Lb = a.links(), b.links()
+        for k in Lb:
+            assert np.array_equal(np.asarray(La[k]), np.asarray(Lb[k])), k
+
+
 # ------------------------------------------------------------------ boundary behaviour
 
 def test_error_codes(gpu, wl):
