@@ -41,62 +41,123 @@ __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc
 }
 
 // ------------------------------------------------------------------------------------------
-// a2: link builder.  grid = particles, block = LB_WARPS warps.
+// a2: link builder.  grid = particles (or fewer persistent CTAs), block = LB_WARPS warps.
 //
-// The effective zone is cut into items = (row, 32-column chunk), dealt to the warps in contiguous
-// runs; a lane keeps the 8-bit direction masks of up to LB_ITEMS items in registers, so the whole
-// zone of a d <= 28 particle is one round with one block prefix.  The work is ordered so that
-// nothing waits on memory item by item:
-//   1. arithmetic only: can the node carry a link (outside the own disc, within r + 1.5 of the
-//      centre) and which neighbours lie inside the disc -- the separately rounded predicate that
-//      rasterised the disc;
-//   2. the flag bytes of all candidate nodes of the round, requested together (a candidate may be
+// A fluid node can carry a link of particle p only in the ring r^2 < d^2 <= (r + 1.5)^2 around
+// the centre, so the work is made proportional to the perimeter, not to the area of the zone:
+//   0. one thread per zone row turns the ring into at most two column segments of that row
+//      (square roots only bracket them: each end is padded by one node and every candidate is
+//      then decided by the exact, separately rounded predicate that rasterised the disc); a block
+//      prefix over the rows numbers the candidates in row-major order;
+//   1. candidates are dealt to the threads, LB_CPT per thread and round, each found by a binary
+//      search in the row prefix; arithmetic only: is the node in the ring, which neighbours lie
+//      inside the disc;
+//   2. the flag bytes of all candidates of the round, requested together (a candidate may be
 //      inside ANOTHER particle);
 //   3. only for a particle whose disc may overlap another one (sticky flag pa.ovl, set by k_cover):
 //      the owner of each solid neighbour, lowest id owns the node.  Without
 //      overlap every node inside the disc is owned by the particle and the loads are skipped;
-//   4. packed warp prefix (four 16-bit item counts per 64-bit shuffle), block prefix, emission in
-//      row-major order (neighbouring links -> neighbouring nodes for the bounce-back kernel) into
-//      shared memory;
+//   4. packed block prefix (the LB_CPT counts of a thread in the 16-bit fields of one 64-bit
+//      shuffle), emission in row-major order (neighbouring links -> neighbouring nodes for the
+//      bounce-back kernel) into shared memory;
 //   5. q and the ladder rung per link, one link per thread, both flag bytes requested together.
 constexpr int LB_WARPS = 4;
-constexpr int LB_ITEMS = 8;
-__global__ void __launch_bounds__(LB_WARPS * 32)
+constexpr int LB_T = LB_WARPS * 32;
+constexpr int LB_CPT = 4;
+__global__ void __launch_bounds__(LB_T)
 k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
               const double* __restrict__ pr, const unsigned char* __restrict__ ovl,
               const unsigned char* __restrict__ flag, const int* __restrict__ owner, LinkArrays la,
-              int np, int* __restrict__ status, const LbmConst c) {
-  extern __shared__ int s_node[];                           // la.cap packed nodes, then la.cap dir bytes
-  unsigned char* s_dir = (unsigned char*)(s_node + la.cap);
+              int np, int max_rows, int* __restrict__ status, const LbmConst c) {
+  extern __shared__ int s_node[];                           // la.cap packed nodes, la.cap dir bytes,
+  unsigned char* s_dir = (unsigned char*)(s_node + la.cap); // then the row tables
+  int* s_off = s_node + la.cap + (la.cap + 3) / 4;          // max_rows + 1: candidates before row t
+  int* s_a1 = s_off + max_rows + 1;                         // first column of segment 1
+  int* s_n1 = s_a1 + max_rows;                              // its length
+  int* s_a2 = s_n1 + max_rows;                              // first column of segment 2
   __shared__ int s_warp[LB_WARPS];
+  __shared__ unsigned long long s_wpk[LB_WARPS];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned FULL = 0xffffffffu;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const double xc = px_[p], yc = py_[p], r = pr[p];
   const bool check_owner = ovl[p] != 0;
   int i0, i1, j0, j1;
   zone_of(xc, yc, r, i0, i1, j0, j1);
-  const int W = i1 - i0 + 1, H = j1 - j0 + 1;
-  const int chunks = (W + 31) >> 5, n_items = H * chunks;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned FULL = 0xffffffffu;
+  const int H = min(j1 - j0 + 1, max_rows);
   const double r2 = r * r;
   const double rfar = (r + 1.5) * (r + 1.5);   // beyond this no neighbour can be inside the disc
+  const int ilo = max(i0, 0), ihi = min(i1, c.nx - 1);
+
+  // ---- 0. ring segments per row and their prefix
+  int carry = 0;
+  for (int t0 = 0; t0 < H; t0 += LB_T) {
+    const int t = t0 + threadIdx.x;
+    int cnt = 0;
+    if (t < H) {
+      const int j = j0 + t;
+      int a1 = 0, n1 = 0, a2 = 0, n2 = 0;
+      const double dy = (double)j - yc, dy2 = dy * dy;
+      if (j >= 0 && j < c.ny && dy2 <= rfar) {
+        const double wo = sqrt(rfar - dy2);
+        const int oa = max((int)floor(xc - wo) - 1, ilo), ob = min((int)floor(xc + wo) + 2, ihi);
+        int ha = ob + 1, hb = ob;                 // hole = columns certainly inside the disc
+        if (dy2 < r2) {
+          const double wi = sqrt(r2 - dy2);
+          ha = (int)floor(xc - wi) + 2;
+          hb = (int)floor(xc + wi) - 1;
+        }
+        if (ha <= hb && ha > oa && hb < ob) {     // two segments around the hole
+          a1 = oa; n1 = ha - oa;
+          a2 = hb + 1; n2 = ob - hb;
+        } else if (ob >= oa) {                    // one segment
+          a1 = oa; n1 = ob - oa + 1;
+        }
+      }
+      s_a1[t] = a1; s_n1[t] = n1; s_a2[t] = a2;
+      cnt = n1 + n2;
+    }
+    int incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int v = __shfl_up_sync(FULL, incl, d);
+      if (lane >= d) incl += v;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    int woff = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < LB_WARPS; ++w) {
+      const int v = s_warp[w];
+      if (w < warp) woff += v;
+      tot += v;
+    }
+    if (t < H) s_off[t] = carry + woff + incl - cnt;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) s_off[H] = carry;
+  __syncthreads();
+  const int ncand = carry;
   int running = 0;                             // links emitted by earlier rounds (same in all threads)
 
-  for (int first = 0; first < n_items; first += LB_WARPS * LB_ITEMS) {
-    const int in_round = min(n_items - first, LB_WARPS * LB_ITEMS);
-    const int ipw = (in_round + LB_WARPS - 1) / LB_WARPS;   // items per warp, contiguous
-    unsigned mask[LB_ITEMS];
-    int node[LB_ITEMS];
+  for (int first = 0; first < ncand; first += LB_T * LB_CPT) {
+    unsigned mask[LB_CPT];
+    int node[LB_CPT];
     // ---- 1. arithmetic
 #pragma unroll
-    for (int k = 0; k < LB_ITEMS; ++k) {
+    for (int k = 0; k < LB_CPT; ++k) {
       mask[k] = 0;
       node[k] = 0;
-      const int item = first + warp * ipw + k;
-      if (k >= ipw || item >= first + in_round) continue;
-      const int row = chunks == 1 ? item : item / chunks;
-      const int i = i0 + ((item - row * chunks) << 5) + lane, j = j0 + row;
-      if (i > i1 || i < 0 || i >= c.nx || j < 0 || j >= c.ny) continue;
+      const int cnd = first + k * LB_T + threadIdx.x;
+      if (cnd >= ncand) continue;
+      int lo = 0, hi = H - 1;                  // last row whose prefix is <= cnd
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (s_off[mid] <= cnd) lo = mid; else hi = mid - 1;
+      }
+      const int l = cnd - s_off[lo], n1 = s_n1[lo];
+      const int i = l < n1 ? s_a1[lo] + l : s_a2[lo] + (l - n1), j = j0 + lo;
       // coordinates of the 3 x 3 neighbourhood: integers are exact in fp64, so xi + 1.0 is
       // (double)(i + 1) bit for bit and the disc test below is the rasteriser's
       const double xi = (double)i, yj = (double)j;
@@ -121,17 +182,17 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
       node[k] = (int)((unsigned)i | ((unsigned)j << 16));
     }
     // ---- 2. flags of the candidates (flag 2 = newborn: a fluid node of the step the links are for)
-    unsigned char fl[LB_ITEMS];
+    unsigned char fl[LB_CPT];
 #pragma unroll
-    for (int k = 0; k < LB_ITEMS; ++k)
+    for (int k = 0; k < LB_CPT; ++k)
       fl[k] = mask[k] ? flag[(long long)(int)((unsigned)node[k] >> 16) * c.px + (node[k] & 0xffff)] : 1;
 #pragma unroll
-    for (int k = 0; k < LB_ITEMS; ++k)
+    for (int k = 0; k < LB_CPT; ++k)
       if (fl[k] == 1) mask[k] = 0;
     // ---- 3. ownership of the solid neighbours, only if discs may overlap
     if (check_owner) {
 #pragma unroll
-      for (int k = 0; k < LB_ITEMS; ++k) {
+      for (int k = 0; k < LB_CPT; ++k) {
         const int i = node[k] & 0xffff, j = (int)((unsigned)node[k] >> 16);
         unsigned keep = 0;
         for (unsigned t = mask[k]; t; t &= t - 1) {
@@ -141,45 +202,43 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
         mask[k] = keep;
       }
     }
-    // ---- 4. prefix: item-major within the warp, warps in order
-    unsigned long long pk0 = 0, pk1 = 0;   // 16-bit counts of items 0..3 and 4..7
+    // ---- 4. prefix in candidate order: (k, warp, lane)
+    unsigned long long pk = 0;                 // 16-bit link counts of this thread's candidates
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      pk0 |= (unsigned long long)__popc(mask[k]) << (16 * k);
-      pk1 |= (unsigned long long)__popc(mask[k + 4]) << (16 * k);
-    }
-    unsigned long long in0 = pk0, in1 = pk1;
+    for (int k = 0; k < LB_CPT; ++k) pk |= (unsigned long long)__popc(mask[k]) << (16 * k);
+    unsigned long long incl = pk;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-      const unsigned long long v0 = __shfl_up_sync(FULL, in0, d);
-      const unsigned long long v1 = __shfl_up_sync(FULL, in1, d);
-      if (lane >= d) { in0 += v0; in1 += v1; }
+      const unsigned long long v = __shfl_up_sync(FULL, incl, d);
+      if (lane >= d) incl += v;
     }
-    const unsigned long long t0 = __shfl_sync(FULL, in0, 31), t1 = __shfl_sync(FULL, in1, 31);
-    const unsigned long long ex0 = in0 - pk0, ex1 = in1 - pk1;   // exclusive over lanes, per item
-    int item_off[LB_ITEMS];
-    int wtotal = 0;
-#pragma unroll
-    for (int k = 0; k < LB_ITEMS; ++k) {
-      item_off[k] = wtotal;
-      wtotal += (int)(((k < 4 ? t0 : t1) >> (16 * (k & 3))) & 0xffffu);
-    }
-    if (lane == 0) s_warp[warp] = wtotal;
+    if (lane == 31) s_wpk[warp] = incl;        // per-warp totals, still packed (<= 256 per field)
     __syncthreads();
-    int woff = 0, btotal = 0;
+    int before[LB_CPT];                        // links of earlier warps, per k
+    int total[LB_CPT];
+#pragma unroll
+    for (int k = 0; k < LB_CPT; ++k) before[k] = total[k] = 0;
 #pragma unroll
     for (int w = 0; w < LB_WARPS; ++w) {
-      const int v = s_warp[w];
-      if (w < warp) woff += v;
-      btotal += v;
-    }
-    if (running + btotal <= la.cap) {
+      const unsigned long long v = s_wpk[w];
 #pragma unroll
-      for (int k = 0; k < LB_ITEMS; ++k) {
+      for (int k = 0; k < LB_CPT; ++k) {
+        const int n = (int)((v >> (16 * k)) & 0xffffu);
+        if (w < warp) before[k] += n;
+        total[k] += n;
+      }
+    }
+    const unsigned long long excl = incl - pk;
+    int btotal = 0;
+#pragma unroll
+    for (int k = 0; k < LB_CPT; ++k) btotal += total[k];
+    if (running + btotal <= la.cap) {
+      int kbase = running;
+#pragma unroll
+      for (int k = 0; k < LB_CPT; ++k) {
         unsigned m = mask[k];
-        if (!m) continue;
-        int off = running + woff + item_off[k] +
-                  (int)(((k < 4 ? ex0 : ex1) >> (16 * (k & 3))) & 0xffffu);
+        int off = kbase + before[k] + (int)((excl >> (16 * k)) & 0xffffu);
+        kbase += total[k];
         while (m) {
           const int al = __ffs(m) - 1;
           m &= m - 1;
@@ -198,7 +257,7 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
   // nodes inside the cavity (both flag bytes requested before either is tested)
   const int nl = running <= la.cap ? running : 0;
   const long long base = (long long)p * la.cap;
-  for (int s = threadIdx.x; s < nl; s += LB_WARPS * 32) {
+  for (int s = threadIdx.x; s < nl; s += LB_T) {
     const int nd = s_node[s];
     const int al = s_dir[s];
     const int i = nd & 0xffff, j = (int)((unsigned)nd >> 16);
@@ -462,17 +521,24 @@ static int chain_grid(const lbm* h, int items, cudaStream_t st) {
   return items;
 }
 
+// rows of the largest effective zone the capacity admits (12N - 12 <= cap) and the
+// dynamic shared memory of the link builder: the compacted list + four row tables
+static int link_rows(const lbm* h) { return (h->la.cap + 12) / 12 + 2; }
+static size_t link_smem(const lbm* h) {
+  return ((size_t)h->la.cap + ((size_t)h->la.cap + 3) / 4 + 4 * (size_t)link_rows(h) + 4) * sizeof(int);
+}
+
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  const size_t smem = (size_t)h->la.cap * 5 + 16;
-  k_build_links<<<chain_grid(h, h->np, st), LB_WARPS * 32, smem, st>>>(
+  const int max_rows = link_rows(h);
+  k_build_links<<<chain_grid(h, h->np, st), LB_T, link_smem(h), st>>>(
       h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r, h->pa.ovl, h->flag, h->owner, h->la,
-      h->np, h->status_dev, h->C);
+      h->np, max_rows, h->status_dev, h->C);
 }
 
 int particles_configure(lbm* h) {
-  const size_t smem = (size_t)h->la.cap * 5 + 16;
+  const size_t smem = link_smem(h);
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(k_build_links, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return -1;
