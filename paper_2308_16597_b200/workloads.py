@@ -196,6 +196,27 @@ def paper_table4(cols: int = 80, lines: int = 60, name: str = "paper_table4_4800
                     notes="paper's E4 benchmark; 1750 MLUPS on 1x A100 (Table 5, PAPER.md:273-281)")
 
 
+def paper_dkt(name: str = "paper_dkt_two_hot_particles_400x1200") -> Workload:
+    """Appendix B of the paper (Table 6): draft-kissing-tumbling of
+    two hot circular particles in cold fluid.  400 x 1200 l.u., d = 40, rho_p/rho_f = 1.01,
+    nu = alpha_T = 0.01 (Pr = 1), g = 1.23e-4, beta = 1.28e-3 per lattice temperature unit
+    (Gr_p = 100), all walls cold and no-slip; the lower particle at (0.5 W - 0.005 d, 0.8 H), the
+    upper one at (0.5 W, 0.8 H + 2 d) (walls half a spacing outside the outermost nodes); the
+    paper's repulsion (Eq. 15: quadratic, s = 3, eps_w = 0.001)."""
+    nx, ny, d = 400, 1200, 40.0
+    x = np.array([0.5 * nx - 0.5 - 0.005 * d, 0.5 * nx - 0.5])
+    y = np.array([0.8 * ny - 0.5, 0.8 * ny - 0.5 + 2.0 * d])
+    p = default_params()
+    p.update(nu=0.01, kappa=0.01, rho0=1.0, T0=0.0, g=1.23e-4, gbeta=1.23e-4 * 1.28e-3,
+             rep_s=3.0, rep_eps=1e-3, rep_power=2, max_particles=2,
+             max_links_per_particle=max_links_for_diameter(d))
+    p["wall_T_type"] = [1, 1, 1, 1]
+    p["wall_T"] = [0.0, 0.0, 0.0, 0.0]
+    parts = _particle_dict(x, y, np.full(2, d), rho_ratio=1.01, T_w=1.0)
+    return Workload(name=name, nx=nx, ny=ny, params=p, steps=160000, parity_steps=100,
+                    particles=parts, notes="index 0 = lower particle (P2 of Fig. 18), 1 = upper (P1)")
+
+
 def config(k: int) -> Workload:
     """BASELINE.json configs[k], resolved as in SURVEY.md 8(d); k = 5 is the paper's own Table 4
     benchmark, which BASELINE.json's config 3 replaces for the headline."""

@@ -142,3 +142,45 @@ def test_config4_full_size(gpu, ob, wl):
     del o
     g.step(50)
     assert sampled_one_step_check(g, ob, w, 800) == 800
+
+
+def test_paper_dkt_drafting_kissing_tumbling(gpu, ob, wl):
+    """Appendix B of the paper (Table 6, Figs. 17-18): two hot particles of
+    d = 40 released 2 d apart in a 400 x 1200 cavity.  (i) parity with the oracle over the first
+    100 steps at full size; (ii) the qualitative sequence the paper validates against Tao et al.
+    -- the paper gives it only as curves, so the checks are on its stages: the upper particle
+    drafts in the wake of the lower one and falls faster, the two kiss (surface gap held at the
+    repulsion range, no overlap) for a while, then tumble apart sideways and the formerly upper
+    particle overtakes.  Fig. 17 shows contact at t* = 140 and separation at t* = 280
+    (t* = t / sqrt(d/g), 570 steps)."""
+    w = wl.paper_dkt()
+    d = 40.0
+    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
+    assert_links_equal(g.links(), o.links())
+    g.step(100)
+    o.step(100)
+    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
+    assert_particles_close(g.particles(), o.particles(), r_min=20.0, steps=100)
+    del o
+    tstar = 570.0
+    hist = []
+    done = 100
+    for target in range(4000, 116001, 4000):
+        g.step(target - done)
+        done = target
+        p = g.particles()
+        assert all(np.isfinite(v).all() for v in p.values())
+        hist.append((target / tstar, p["x"][1] - p["x"][0], p["y"][1] - p["y"][0],
+                     p["uy"][0], p["uy"][1]))
+    hist = np.array(hist)
+    t, dx, dy, uy_lo, uy_up = hist.T
+    dist = np.hypot(dx, dy) / d
+    # drafting: around t* = 70 the upper particle falls faster and has closed in
+    k = np.argmin(np.abs(t - 70.0))
+    assert uy_up[k] < 1.15 * uy_lo[k] < 0.0 and dist[k] < 1.8
+    # kissing: contact held at the repulsion range (s = 3 l.u.), never overlapping
+    contact = (t > 100.0) & (t < 160.0)
+    assert dist[contact].max() < 1.0 + 3.5 / d and dist.min() > 1.0
+    # tumbling: they separate sideways and the upper particle ends up below the lower one
+    assert np.abs(dx[-1]) > 1.2 * d and dy[-1] < 0.0
+    assert np.abs(dx[t < 120.0]).max() < 0.05 * d
