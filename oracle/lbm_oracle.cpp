@@ -9,6 +9,13 @@
  *
  * Citations: PAPER.md:<line> = the paper; "reading" = a choice the paper leaves open, listed in
  * DESIGN.md "Readings of the paper" (taken over from SURVEY.md 8(c)).
+ *
+ * Pins (tests/test_oracle_*.py, tests/test_units.py): every formula piece against its algebraic
+ * identities; Poiseuille, conduction, thermal decay, mass conservation; brute-force link scans;
+ * and the coupled fluid-particle step against Faxen's drag on a cylinder moving between two walls
+ * (Eqs. 9, 10, 13, 16) and the conduction shape factor of a hot cylinder between two cold walls
+ * (Eqs. 11, 12).  Parity unpinned: the readings no closed form sees (integrator order, fallback
+ * ladders in narrow gaps, e_c tie rule, pair repulsion) -- see DESIGN.md section 2.
  */
 #include "lbm_oracle.h"
 

@@ -157,6 +157,38 @@ def test_moving_rotating_particles_mixed_sizes(gpu, ob, wl):
     assert_links_after_injection(gpu, ob, wl, w, o.particles())
 
 
+def test_drag_on_a_moving_cylinder_matches_faxen_on_the_gpu(gpu, wl):
+    """The closed form the oracle is pinned to (tests/test_oracle_particles.py), checked on the
+    CUDA path directly, at two blockage ratios: Stokes drag on a cylinder moving along the
+    mid-plane between two walls (Faxen)."""
+    from test_oracle_particles import faxen_drag_per_length, faxen_workload
+    for d, W, L in ((10.0, 40, 240), (10.0, 50, 300)):
+        U, nu = 0.005, 1.0 / 6.0
+        steps = int(6.0 * W * W / (np.pi ** 2 * nu))
+        g = gpu.Simulation.from_workload(faxen_workload(wl, d=d, W=W, L=L, U=U, nu=nu, steps=steps))
+        g.step(steps - 200)
+        F = []
+        for _ in range(200):
+            g.step(1)
+            F.append(g.particles()["Fx"][0])
+        drag = -np.mean(F)
+        expected = faxen_drag_per_length(nu, U, d / W)
+        assert abs(drag / expected - 1.0) < 0.025, (d, W, drag, expected)
+
+
+def test_heat_flow_from_a_hot_cylinder_matches_the_shape_factor_on_the_gpu(gpu, wl):
+    """The conduction closed form the oracle is pinned to, on the CUDA path, for two geometries."""
+    from test_oracle_particles import (conduction_workload, shape_factor_cylinder_between_planes,
+                                       wall_heat_flow)
+    for d, W, L in ((10.0, 40, 400), (8.0, 48, 400)):
+        kappa = 0.1
+        g = gpu.Simulation.from_workload(conduction_workload(wl, d=d, W=W, L=L, kappa=kappa, steps=12000))
+        g.step(12000)
+        q = wall_heat_flow(g.fields()["T"], kappa)
+        expected = shape_factor_cylinder_between_planes(d, 0.5 * W) * kappa
+        assert abs(q / expected - 1.0) < 0.01, (d, W, q, expected)
+
+
 def test_paper_repulsion_variant(gpu, ob, wl):
     """Eq. (15) as the paper prints it: quadratic, s = 3, eps_w = 1e-3; two
     particles approaching head-on and one falling onto the bottom wall."""

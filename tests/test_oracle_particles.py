@@ -141,6 +141,101 @@ def test_zero_lift_on_symmetric_fixed_cylinder(ob, wl):
     assert P["Fx"][0] < 2e-6 * (F["flag"] == 0).sum()
 
 
+def faxen_drag_per_length(mu, U, k):
+    """Stokes drag per unit length on a circular cylinder moving with speed U along the mid-plane
+    between two parallel walls, k = diameter / wall spacing (Faxen 1946, as quoted in Happel &
+    Brenner, Low Reynolds Number Hydrodynamics, Sec. 7-8): F = 4 pi mu U / Lambda(k)."""
+    lam = (math.log(1.0 / k) - 0.9157 + 1.7244 * k ** 2 - 1.7302 * k ** 4 + 2.4056 * k ** 6
+           - 4.5913 * k ** 8)
+    return 4.0 * math.pi * mu * U / lam
+
+
+def faxen_workload(wl, d=10.0, W=40, L=240, U=0.005, nu=1.0 / 6.0, steps=6000):
+    """A heavy cylinder (density ratio 1e9: its velocity stays U) moving along the mid-plane of a
+    long closed cavity filled with fluid at rest (closed ends: no net flow past the cylinder, as in
+    Faxen's problem).  Re = U d / nu = 0.3."""
+    p = wl.default_params()
+    p.update(nu=nu, kappa=0.05, g=0.0, gbeta=0.0, max_particles=1, rep_s=0.5,
+             max_links_per_particle=wl.max_links_for_diameter(d))
+    parts = dict(x=np.array([0.3 * L]), y=np.array([0.5 * W - 0.5]), diam=np.array([d]),
+                 rho_ratio=np.array([1e9]), T_w=np.array([0.0]), ux=np.array([U]),
+                 uy=np.array([0.0]), omega=np.array([0.0]))
+    return wl.Workload("faxen", L, W, p, steps, steps, particles=parts)
+
+
+def test_drag_on_a_moving_cylinder_between_walls_matches_faxen(ob, wl):
+    """Pins the whole coupled step quantitatively -- interpolated moving-wall bounce-back (Eqs. 9,
+    10), Galilean-invariant momentum exchange (Eq. 13), flag update and refill (Eq. 16) of a
+    particle that really moves across the lattice -- to a textbook closed form: after the
+    transient (6000 steps = 6 viscous times W^2/(pi^2 nu)) the drag, averaged over the last 200
+    steps (one lattice spacing of travel), is Faxen's.  A dropped wall-velocity term, a wrong
+    interpolation coefficient or a force sign or factor error moves it by far more than the 2.5 %
+    allowed (measured: -0.9 % at d = 10 l.u.)."""
+    d, W, U, nu = 10.0, 40, 0.005, 1.0 / 6.0
+    o = ob.OracleSim.from_workload(faxen_workload(wl, d=d, W=W, U=U, nu=nu, steps=6000))
+    o.step(5800)
+    F = []
+    for _ in range(200):
+        o.step(1)
+        p = o.particles()
+        F.append((p["Fx"][0], p["Fy"][0], p["Tz"][0]))
+    F = np.array(F)
+    expected = faxen_drag_per_length(nu * 1.0, U, d / W)
+    drag = -F[:, 0].mean()
+    assert abs(drag / expected - 1.0) < 0.025, (drag, expected)
+    assert abs(F[:, 0] + drag).max() < 0.02 * drag          # lattice-position ripple is small
+    assert abs(F[:, 1]).max() < 1e-9 * drag and abs(F[:, 2]).max() < 1e-8 * drag * d   # symmetry
+    assert abs(p["ux"][0] - U) < 1e-6 * U and abs(p["x"][0] - (0.3 * 240 + 6000 * U)) < 1e-4
+
+
+def conduction_workload(wl, d=10.0, W=40, L=240, kappa=0.1, steps=6000):
+    """A fixed hot cylinder (T_w = 1) midway between two cold walls (T = 0) of a long cavity with
+    adiabatic ends, no flow (g beta = 0): pure conduction."""
+    p = wl.default_params()
+    p.update(nu=0.1, kappa=kappa, g=0.0, gbeta=0.0, max_particles=1, rep_s=0.5,
+             max_links_per_particle=wl.max_links_for_diameter(d),
+             wall_T_type=[0, 0, 1, 1], wall_T=[0.0, 0.0, 0.0, 0.0])
+    parts = dict(x=np.array([0.5 * L - 0.5]), y=np.array([0.5 * W - 0.5]), diam=np.array([d]),
+                 rho_ratio=np.array([2.0]), T_w=np.array([1.0]), fixed=np.array([1], dtype=np.uint8))
+    return wl.Workload("conduction", L, W, p, steps, steps, particles=parts)
+
+
+def wall_heat_flow(T, kappa):
+    """Heat per unit time into the two cold walls: the first node row lies half a spacing from
+    the wall (T_wall = 0), rho c_p = 1."""
+    return kappa * (T[0, :].sum() + T[-1, :].sum()) / 0.5
+
+
+def shape_factor_cylinder_between_planes(d, z):
+    """Conduction shape factor per unit length of a circular cylinder of diameter d midway between
+    two parallel isothermal planes at distance z from its axis, z >> d/2 (the standard heat
+    transfer table entry, e.g. Incropera & DeWitt Table 4.1): S = 2 pi / ln(8 z / (pi d))."""
+    return 2.0 * math.pi / math.log(8.0 * z / (math.pi * d))
+
+
+def test_heat_flow_from_a_hot_cylinder_matches_the_conduction_shape_factor(ob, wl):
+    """Pins the thermal side of the fluid-particle coupling -- the curved-wall Dirichlet
+    bounce-back of Eqs. (11), (12) with the D2Q5 collision (kappa) and the cold cavity walls -- to
+    a closed form: in steady conduction the heat flowing into the walls is S kappa (T_w - T_c)
+    with the textbook shape factor of a cylinder between two planes.  A wrong c_d coefficient, a
+    missing factor in the 2 w T_w term or a wrong thermal weight changes it by tens of per cent;
+    allowed 2 % (measured -0.7 % at d = 10, z = 20: the formula itself assumes z >> d/2 and the
+    cavity is 24 d long)."""
+    d, W, kappa = 10.0, 40, 0.1
+    o = ob.OracleSim.from_workload(conduction_workload(wl, d=d, W=W, kappa=kappa, steps=6000))
+    o.step(5000)
+    q1 = wall_heat_flow(o.fields()["T"], kappa)
+    o.step(1000)
+    f = o.fields()
+    q2 = wall_heat_flow(f["T"], kappa)
+    assert abs(q2 - q1) < 1e-2 * q2                              # (nearly) steady
+    expected = shape_factor_cylinder_between_planes(d, 0.5 * W) * kappa * 1.0
+    assert abs(q2 / expected - 1.0) < 0.02, (q2, expected)
+    fluid = f["flag"] == 0
+    assert f["T"][fluid].max() < 1.0 and f["T"][fluid].min() > -1e-12   # maximum principle
+    assert float(np.abs(f["ux"][fluid]).max()) < 1e-12            # no flow was started
+
+
 def test_repulsion_and_gravity_enter_the_first_step_in_closed_form(ob, wl):
     """At t = 0 the fluid is at rest, so F_hydro = 0 and U(1) = (weight + Eq. 15)/M exactly:
     pair at gap 1.5 (s = 2, p = 1 -> a quarter of C/eps) and a particle at gap 1.5 from the bottom
