@@ -176,6 +176,17 @@ def test_drag_on_a_moving_cylinder_matches_faxen_on_the_gpu(gpu, wl):
         assert abs(drag / expected - 1.0) < 0.025, (d, W, drag, expected)
 
 
+def test_terminal_velocity_matches_the_faxen_balance_on_the_gpu(gpu, wl):
+    """Freely settling cylinder: net weight = Faxen drag at the terminal speed (CUDA path)."""
+    from test_oracle_particles import settling_workload
+    U = 0.005
+    g = gpu.Simulation.from_workload(settling_workload(wl, U_target=U))
+    g.step(6000)
+    p = g.particles()
+    assert abs(-p["uy"][0] / U - 1.0) < 0.025, p["uy"][0]
+    assert abs(p["ux"][0]) < 1e-10 and abs(p["x"][0] - 19.5) < 1e-7
+
+
 def test_heat_flow_from_a_hot_cylinder_matches_the_shape_factor_on_the_gpu(gpu, wl):
     """The conduction closed form the oracle is pinned to, on the CUDA path, for two geometries."""
     from test_oracle_particles import (conduction_workload, shape_factor_cylinder_between_planes,

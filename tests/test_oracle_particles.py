@@ -188,6 +188,35 @@ def test_drag_on_a_moving_cylinder_between_walls_matches_faxen(ob, wl):
     assert abs(p["ux"][0] - U) < 1e-6 * U and abs(p["x"][0] - (0.3 * 240 + 6000 * U)) < 1e-4
 
 
+def settling_workload(wl, d=10.0, W=40, L=240, nu=1.0 / 6.0, ratio=1.2, U_target=0.005):
+    """A cylinder released from rest on the axis of a tall closed channel, with gravity chosen so
+    that the balance weight - buoyancy = Faxen drag gives the terminal speed U_target."""
+    lam = 4.0 * math.pi * nu * U_target / faxen_drag_per_length(nu, U_target, d / W)
+    g = U_target * 4.0 * nu / ((ratio - 1.0) * (0.5 * d) ** 2 * lam)
+    p = wl.default_params()
+    p.update(nu=nu, kappa=0.05, g=g, gbeta=0.0, max_particles=1, rep_s=0.5,
+             max_links_per_particle=wl.max_links_for_diameter(d))
+    parts = dict(x=np.array([0.5 * W - 0.5]), y=np.array([0.75 * L]), diam=np.array([d]),
+                 rho_ratio=np.array([ratio]), T_w=np.array([0.0]))
+    return wl.Workload("settling", W, L, p, 6000, 6000, particles=parts)
+
+
+def test_terminal_velocity_of_a_settling_cylinder_matches_the_faxen_balance(ob, wl):
+    """The closed loop of the coupling: weight minus buoyancy (pi r^2 (rho_p - rho_f) g), the
+    hydrodynamic force of Eqs. (9), (10), (13) and the integrator of Eqs. (7), (8) bring a freely
+    moving cylinder to the speed at which Faxen's drag balances its net weight: within 2.5 %
+    (measured +0.9 %), falling straight down the axis, not rotating."""
+    U = 0.005
+    o = ob.OracleSim.from_workload(settling_workload(wl, U_target=U))
+    o.step(5000)
+    u1 = o.particles()["uy"][0]
+    o.step(1000)
+    p = o.particles()
+    assert abs(p["uy"][0] - u1) < 2e-3 * U                         # terminal
+    assert abs(-p["uy"][0] / U - 1.0) < 0.025, p["uy"][0]
+    assert abs(p["ux"][0]) < 1e-12 and abs(p["omega"][0]) < 1e-12 and abs(p["x"][0] - 19.5) < 1e-9
+
+
 def conduction_workload(wl, d=10.0, W=40, L=240, kappa=0.1, steps=6000):
     """A fixed hot cylinder (T_w = 1) midway between two cold walls (T = 0) of a long cavity with
     adiabatic ends, no flow (g beta = 0): pure conduction."""
