@@ -65,11 +65,13 @@ def sampled_one_step_check(g, ob, w, nsamples=1500, seed=0):
     return len(pick)
 
 
-def numpy_flags(w):
-    """Independent rasterisation: node solid iff dx*dx + dy*dy <= r*r for some particle."""
+def numpy_flags(w, state=None):
+    """Independent rasterisation: node solid iff dx*dx + dy*dy <= r*r for some particle (at the
+    workload's initial positions, or at the positions in `state`)."""
     flag = np.zeros((w.ny, w.nx), dtype=np.uint8)
     P = w.particles
-    for x, y, d in zip(P["x"], P["y"], P["diam"]):
+    X, Y = (P["x"], P["y"]) if state is None else (state["x"], state["y"])
+    for x, y, d in zip(X, Y, P["diam"]):
         r = 0.5 * d
         i0, i1 = max(int(np.floor(x - r)) - 1, 0), min(int(np.floor(x + r)) + 1, w.nx - 1)
         j0, j1 = max(int(np.floor(y - r)) - 1, 0), min(int(np.floor(y + r)) + 1, w.ny - 1)
@@ -126,6 +128,14 @@ def test_config3_full_size(gpu, ob, wl):
     p = g.particles()
     assert all(np.isfinite(v).all() for v in p.values())
     assert (p["uy"] < 0).mean() > 0.9          # they are settling
+    # 307 steps of incremental flag updates (uncover / claim-only-new-nodes cover) against a
+    # from-scratch rasterisation of the final positions, and the final links against the oracle's
+    # link builder on the same injected state
+    assert np.array_equal(g.fields()["flag"], numpy_flags(w, p))
+    parts = dict(w.particles)
+    parts.update(x=p["x"], y=p["y"], ux=p["ux"], uy=p["uy"], omega=p["omega"])
+    w2 = wl.Workload("config3_inj", w.nx, w.ny, w.params, 1, 1, particles=parts)
+    assert_links_equal(g.links(), ob.OracleSim.from_workload(w2).links())
 
 
 def test_config4_full_size(gpu, ob, wl):
