@@ -194,3 +194,28 @@ def test_paper_dkt_drafting_kissing_tumbling(gpu, ob, wl):
     # tumbling: they separate sideways and the upper particle ends up below the lower one
     assert np.abs(dx[-1]) > 1.2 * d and dy[-1] < 0.0
     assert np.abs(dx[t < 120.0]).max() < 0.05 * d
+
+
+def test_config2_whole_run_is_schedule_independent(gpu, wl):
+    """Config 2 over more than its whole run length (6,000 steps; BASELINE names 5,000): the
+    benched schedule -- particle chain as persistent CTAs on a second stream under the lattice
+    kernel, refill through the stash -- and the strictly sequential one-CTA-per-particle schedule
+    must agree bit for bit in every particle state and on every fluid node.  Any race between the
+    two streams would show here (480 particles settle, collide and pile up meanwhile)."""
+    w = wl.config(2)
+    a = gpu.Simulation.from_workload(w)
+    b = gpu.Simulation.from_workload(w)
+    b.set_overlap(False)
+    for n in (1000, 5000):
+        a.step(n)
+        b.step(n)
+        pa, pb = a.particles(), b.particles()
+        for k in pa:
+            assert np.array_equal(pa[k], pb[k]), k
+        fa, fb = a.fields(populations=True), b.fields(populations=True)
+        assert np.array_equal(fa["flag"], fb["flag"])
+        fluid = fa["flag"] == 0
+        for k in ("f", "g"):
+            assert np.array_equal(fa[k][:, fluid], fb[k][:, fluid]), k
+    assert all(np.isfinite(v).all() for v in pa.values())
+    assert pa["y"].mean() < w.particles["y"].mean() - 50.0      # the suspension has settled a good way
