@@ -129,16 +129,21 @@ def test_paper_table4_workload_matches_the_printed_table(wl):
 
 
 def test_paper_dkt_workload_matches_table6(wl):
-    """PAPER.md:407-430, Table 6: Ar = 28.0, Re_p = 35.09, Gr_p = 100, Pr = 1; 400 x 1200, d = 40;
-    the lower particle 0.005 d left of the centreline, the upper one 2 d above it."""
+    """PAPER.md:407-430, Table 6 (values in tests/golden/paper_tables.txt): Ar = 28.0,
+    Re_p = 35.09, Gr_p = 100, Pr = 1; 400 x 1200, d = 40; the lower particle 0.005 d left of the
+    centreline, the upper one 2 d above it."""
     import math
     w = wl.paper_dkt()
     p, P = w.params, w.particles
-    d = 40.0
-    assert (w.nx, w.ny) == (400, 1200) and w.n_particles == 2
-    assert round(math.sqrt(p["g"] * d ** 3 * 0.01) / p["nu"], 0) == 28.0
-    assert abs(math.sqrt(p["g"] * math.pi * d * 0.01 / 2.0) * d / p["nu"] - 35.09) < 0.1
-    assert round(p["gbeta"] * d ** 3 / p["nu"] ** 2) == 101          # "Gr_p = 100" to 2 digits
-    assert p["nu"] == p["kappa"]
+    d = G["t6_d_lu"]
+    assert (w.nx, w.ny) == (G["t6_domain_w_lu"], G["t6_domain_h_lu"]) and w.n_particles == 2
+    assert (p["nu"], p["kappa"], p["g"]) == (G["t6_nu_lu"], G["t6_alpha_lu"], G["t6_g_lu"])
+    assert abs(p["gbeta"] - G["t6_g_lu"] * G["t6_beta_lu"]) < 1e-18
+    assert P["rho_ratio"][0] == G["t6_rho_ratio"] and P["diam"][0] == d
+    excess = G["t6_rho_ratio"] - 1.0
+    assert round(math.sqrt(p["g"] * d ** 3 * excess) / p["nu"], 0) == G["t6_Ar"]
+    assert abs(math.sqrt(p["g"] * math.pi * d * excess / 2.0) * d / p["nu"] - G["t6_Re_p"]) < 0.1
+    assert abs(p["gbeta"] * d ** 3 / p["nu"] ** 2 - G["t6_Gr_p"]) < 1.0     # printed to 2-3 digits
+    assert p["nu"] / p["kappa"] == G["t6_Pr"]
     assert abs((P["x"][1] - P["x"][0]) - 0.005 * d) < 1e-12 and P["y"][1] - P["y"][0] == 2 * d
     assert abs(P["x"][1] - (0.5 * w.nx - 0.5)) < 1e-12 and abs(P["y"][0] - (0.8 * w.ny - 0.5)) < 1e-12
