@@ -246,13 +246,16 @@ def main():
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     else:
         peak, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
-    achieved = alg_bytes / far_s / 1e9 if far_s > 0 else 0.0
+    # `achieved` is taken in the schedule the timed region runs (the particle chain sharing the
+    # GPU with the lattice kernel); the kernel alone on the GPU is reported beside it
+    achieved = alg_bytes / far_ovl_s / 1e9 if far_ovl_s > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": "k_stream_collide", "achieved": achieved,
-                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": read_traffic(),
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": read_traffic() if args.config == 3 else None,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                "avg_launch_ms": far_s * 1e3, "launches_timed": P,
-                "avg_launch_ms_while_overlapped": far_ovl_s * 1e3,
-                "achieved_while_overlapped": alg_bytes / far_ovl_s / 1e9 if far_ovl_s > 0 else 0.0,
+                "avg_launch_ms": far_ovl_s * 1e3, "launches_timed": P,
+                "avg_launch_ms_alone": far_s * 1e3,
+                "achieved_alone": alg_bytes / far_s / 1e9 if far_s > 0 else 0.0,
                 "share_of_sequential_step": seq["stream_collide"] / step_ms_seq if step_ms_seq else None,
                 "kernel_ms_per_step_sequential": seq, "kernel_ms_per_step_overlapped": ovl,
                 "whole_step_frac_of_hbm_roofline": value / world / (peak * 1e9 / BYTES_PER_LU / 1e6),
