@@ -36,7 +36,7 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
   return (long long)b * c.px + a;
 }
 
-__global__ void __launch_bounds__(BT, 6)
+__global__ void __launch_bounds__(BT, 8)
 k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, const LbmConst c) {
   const int p = blockIdx.x;
   const int n = la.count[p];
