@@ -89,6 +89,9 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     const double uwx = Ux - Om * rwy;
     const double uwy = Uy + Om * rwx;
     const double wall = 6.0 * b_w[al] * c.rho0 * ((double)b_ex[ab] * uwx + (double)b_ey[ab] * uwy);
+    // two reciprocals serve every coefficient of Eqs. (10)-(12) (within an ulp of the quotients)
+    const double inv = 1.0 / (2.0 * q + 1.0);
+    const double tq = 2.0 * q - 1.0;
     double fbb;
     if (lo) {
       if (nbehind == 2)
@@ -98,19 +101,20 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
       else
         fbb = fi0 + wall;
     } else {
+      const double rq = 1.0 / q;
       if (nbehind >= 1) {
-        const double cq = 1.0 / (q * (2.0 * q + 1.0));
-        fbb = cq * fi0 + ((2.0 * q - 1.0) / q) * fa - ((2.0 * q - 1.0) / (2.0 * q + 1.0)) * fc + cq * wall;
+        const double cq = rq * inv;
+        fbb = cq * fi0 + (tq * rq) * fa - (tq * inv) * fc + cq * wall;
       } else {
-        fbb = (fi0 + (2.0 * q - 1.0) * fa) / (2.0 * q) + wall / (2.0 * q);
+        fbb = (fi0 + tq * fa + wall) * (0.5 * rq);
       }
     }
     const long long xb = (long long)(j + ey) * c.px + (i + ex);   // solid node of the link
     if (al <= 4) {
       double cd2 = 0.0, cd4 = 1.0;
       if (nbehind >= 1) {
-        cd2 = (2.0 * q - 1.0) / (2.0 * q + 1.0);
-        cd4 = 2.0 / (2.0 * q + 1.0);
+        cd2 = tq * inv;
+        cd4 = 2.0 * inv;
       } else {
         gi1 = 0.0;
       }
