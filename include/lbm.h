@@ -89,6 +89,19 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
                       const double* ux, const double* uy, const double* omega,
                       const unsigned char* fixed);
 
+/* Adds n ELLIPTICAL particles (PAPER.md:206-224 and Appendix A): full axes major x minor, the
+ * major-labelled axis at angle theta (radians) to the x axis; everything else as in
+ * lbm_add_particles, with which it may be mixed.  Equal axes give a circle through the circle
+ * formulas.  Readings: the orientation is carried as a unit
+ * vector advanced by a Cayley rotation (no cos / sin after set-up); the repulsion gap of a pair is
+ * taken along the line of centres through the support functions, and the overlap test on insert
+ * uses the same (conservative) gap; mass rho_p pi a b, inertia M (a^2 + b^2) / 4.
+ * max_links_per_particle must admit 12N-12 with N = floor(largest full axis) + 4. */
+int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const double* major,
+                     const double* minor, const double* theta, const double* rho_ratio,
+                     const double* T_w, const double* ux, const double* uy, const double* omega,
+                     const unsigned char* fixed);
+
 /* Advances nsteps time steps (each = rows a1..a6 of SURVEY 8(a); order PAPER.md:347-353):
  * bounce-back (Eqs. 9-12) + momentum exchange (Eqs. 13-14) on the links of x_p(t) -> { particle
  * update (Eqs. 7, 8, 15) -> flag update -> refill (Eqs. 16-17, into a stash) -> link build for

@@ -60,6 +60,12 @@ const int E_ARG = -1, E_STATE = -2, E_CAPACITY = -3, E_NONFINITE = -5;
 struct Particle {
   double x, y, theta, ux, uy, omega;
   double r, rho_ratio, Tw;
+  /* ellipse (App. A; reading in DESIGN.md "Elliptical particles"): semi-axes
+   * a (along the body x axis), b, and the orientation as a unit vector (c, s) = (cos, sin) of
+   * theta, carried on its own so that no cos/sin is evaluated after set-up.  ell = 0: a circle
+   * of radius r = a = b, which takes the circle formulas bit for bit. */
+  double a, b, c, s;
+  int ell;
   double Fx, Fy, Tz; /* hydrodynamic force / torque of the last step, Eqs. (13), (14) */
   int fixed;
 };
@@ -121,17 +127,70 @@ inline bool inside(double xi, double yj, double xc, double yc, double r) {
   return d2 <= r2;
 }
 
+/* ellipse: body coordinates u = dx c + dy s, v = dy c - dx s; inside iff (u/a)^2 + (v/b)^2 <= 1,
+ * each operation separately rounded, in exactly this order */
+inline bool inside_ellipse(double xi, double yj, double xc, double yc, double a, double b,
+                           double c, double s) {
+  double dx = xi - xc;
+  double dy = yj - yc;
+  double u = dx * c + dy * s;
+  double v = dy * c - dx * s;
+  double ua = u / a;
+  double vb = v / b;
+  return ua * ua + vb * vb <= 1.0;
+}
+
+inline bool inside_p(const Particle& p, double xi, double yj) {
+  return p.ell ? inside_ellipse(xi, yj, p.x, p.y, p.a, p.b, p.c, p.s) : inside(xi, yj, p.x, p.y, p.r);
+}
+
+/* half extents of the bounding box of the particle: r, or sqrt((a c)^2 + (b s)^2) etc. */
+inline void half_extents(const Particle& p, double* hx, double* hy) {
+  if (!p.ell) {
+    *hx = p.r;
+    *hy = p.r;
+    return;
+  }
+  double ac = p.a * p.c, bs = p.b * p.s, as = p.a * p.s, bc = p.b * p.c;
+  *hx = std::sqrt(ac * ac + bs * bs);
+  *hy = std::sqrt(as * as + bc * bc);
+}
+
+/* effective zone (narrower reading): [INT(xc-hx)-1, INT(xc+hx)+1] x [.. hy ..] */
+inline void zone_p(const Particle& p, int* i0, int* i1, int* j0, int* j1) {
+  double hx, hy;
+  half_extents(p, &hx, &hy);
+  *i0 = (int)std::floor(p.x - hx) - 1;
+  *i1 = (int)std::floor(p.x + hx) + 1;
+  *j0 = (int)std::floor(p.y - hy) - 1;
+  *j1 = (int)std::floor(p.y + hy) + 1;
+}
+
+inline double q_p(const Particle& p, double xf, double yf, int al) {
+  return p.ell ? oracle_link_q_ellipse(xf, yf, al, p.x, p.y, p.a, p.b, p.c, p.s)
+               : oracle_link_q(xf, yf, al, p.x, p.y, p.r);
+}
+
+/* support function of the particle along the unit vector (nx, ny): half width in that direction */
+inline double support_p(const Particle& p, double nx, double ny) {
+  if (!p.ell) return p.r;
+  double m = nx * p.c + ny * p.s;
+  double w = ny * p.c - nx * p.s;
+  double am = p.a * m, bw = p.b * w;
+  return std::sqrt(am * am + bw * bw);
+}
+
 void compute_owner(const oracle_lbm* h, std::vector<int>& own) {
   own.assign((size_t)h->n, -1);
   for (int p = (int)h->parts.size() - 1; p >= 0; --p) { /* descending so the lowest pid wins */
     const Particle& a = h->parts[p];
-    int i0 = (int)std::floor(a.x - a.r) - 1, i1 = (int)std::floor(a.x + a.r) + 1;
-    int j0 = (int)std::floor(a.y - a.r) - 1, j1 = (int)std::floor(a.y + a.r) + 1;
+    int i0, i1, j0, j1;
+    zone_p(a, &i0, &i1, &j0, &j1);
     for (int j = j0; j <= j1; ++j) {
       if (j < 0 || j >= h->ny) continue;
       for (int i = i0; i <= i1; ++i) {
         if (i < 0 || i >= h->nx) continue;
-        if (inside((double)i, (double)j, a.x, a.y, a.r)) own[IDX(h, i, j)] = p;
+        if (inside_p(a, (double)i, (double)j)) own[IDX(h, i, j)] = p;
       }
     }
   }
@@ -142,8 +201,8 @@ void build_links(const oracle_lbm* h, std::vector<Link>& links) {
   links.clear();
   for (int p = 0; p < (int)h->parts.size(); ++p) {
     const Particle& a = h->parts[p];
-    int i0 = (int)std::floor(a.x - a.r) - 1, i1 = (int)std::floor(a.x + a.r) + 1;
-    int j0 = (int)std::floor(a.y - a.r) - 1, j1 = (int)std::floor(a.y + a.r) + 1;
+    int i0, i1, j0, j1;
+    zone_p(a, &i0, &i1, &j0, &j1);
     for (int al = 1; al <= 8; ++al)
       for (int j = j0; j <= j1; ++j) {
         if (j < 0 || j >= h->ny) continue;
@@ -159,7 +218,7 @@ void build_links(const oracle_lbm* h, std::vector<Link>& links) {
           L.i = i;
           L.j = j;
           L.alpha = al;
-          L.q = oracle_link_q((double)i, (double)j, al, a.x, a.y, a.r);
+          L.q = q_p(a, (double)i, (double)j, al);
           links.push_back(L);
         }
       }
@@ -334,9 +393,12 @@ int step_once(oracle_lbm* h) {
   std::vector<double> Ftx(np, 0.0), Fty(np, 0.0);
   for (int ia = 0; ia < np; ++ia) {
     const Particle& a = h->parts[ia];
-    double Ca = PI * a.r * a.r * (a.rho_ratio * P.rho0 - P.rho0) * P.g; /* Eq. 15's C */
+    /* area pi a b of an ellipse; a circle keeps pi r r (same operations, same bits) */
+    double Ca = PI * a.a * a.b * (a.rho_ratio * P.rho0 - P.rho0) * P.g; /* Eq. 15's C */
     double Fx = a.Fx, Fy = a.Fy;
-    Fy += -(a.rho_ratio * P.rho0 - P.rho0) * PI * a.r * a.r * P.g; /* weight minus buoyancy */
+    Fy += -(a.rho_ratio * P.rho0 - P.rho0) * PI * a.a * a.b * P.g; /* weight minus buoyancy */
+    double ahx, ahy;
+    half_extents(a, &ahx, &ahy);
     for (int ib = 0; ib < np; ++ib) {
       if (ib == ia) continue;
       const Particle& b = h->parts[ib];
@@ -344,23 +406,32 @@ int step_once(oracle_lbm* h) {
       double reach = a.r + b.r + P.rep_s;
       if (std::fabs(dx) > reach || std::fabs(dy) > reach) continue; /* cannot interact */
       double dist = std::sqrt(dx * dx + dy * dy);
-      double delta = dist - a.r - b.r;
+      /* gap along the line of centres through the support functions (reading: the paper does
+       * not state the pair form; for two circles this is |xa - xb| - ra - rb) */
+      double delta;
+      if (!a.ell && !b.ell) {
+        delta = dist - a.r - b.r;
+      } else {
+        if (!(dist > 0.0)) continue;
+        double nxh = dx / dist, nyh = dy / dist;
+        delta = dist - support_p(a, nxh, nyh) - support_p(b, nxh, nyh);
+      }
       if (!(delta <= P.rep_s) || !(dist > 0.0)) continue;
-      double Cb = PI * b.r * b.r * (b.rho_ratio * P.rho0 - P.rho0) * P.g;
+      double Cb = PI * b.a * b.b * (b.rho_ratio * P.rho0 - P.rho0) * P.g;
       double mag = oracle_repulsion_mag(0.5 * (Ca + Cb), P.rep_eps, P.rep_s, delta, P.rep_power);
       Fx += mag * (dx / dist);
       Fy += mag * (dy / dist);
     }
     /* walls W,E,S,N at -1/2, nx-1/2, -1/2, ny-1/2 */
     if (!P.periodic_x) {
-      double dW = (a.x + 0.5) - a.r;
+      double dW = (a.x + 0.5) - ahx;
       if (dW <= P.rep_s) Fx += oracle_repulsion_mag(Ca, P.rep_eps, P.rep_s, dW, P.rep_power);
-      double dE = ((double)nx - 0.5 - a.x) - a.r;
+      double dE = ((double)nx - 0.5 - a.x) - ahx;
       if (dE <= P.rep_s) Fx -= oracle_repulsion_mag(Ca, P.rep_eps, P.rep_s, dE, P.rep_power);
     }
-    double dS = (a.y + 0.5) - a.r;
+    double dS = (a.y + 0.5) - ahy;
     if (dS <= P.rep_s) Fy += oracle_repulsion_mag(Ca, P.rep_eps, P.rep_s, dS, P.rep_power);
-    double dN = ((double)ny - 0.5 - a.y) - a.r;
+    double dN = ((double)ny - 0.5 - a.y) - ahy;
     if (dN <= P.rep_s) Fy -= oracle_repulsion_mag(Ca, P.rep_eps, P.rep_s, dN, P.rep_power);
     Ftx[ia] = Fx;
     Fty[ia] = Fy;
@@ -368,10 +439,11 @@ int step_once(oracle_lbm* h) {
   for (int ia = 0; ia < np; ++ia) {
     Particle& a = h->parts[ia];
     if (a.fixed) continue;
-    double mass = a.rho_ratio * P.rho0 * PI * a.r * a.r;
-    double inertia = 0.5 * mass * a.r * a.r;
+    double mass = a.rho_ratio * P.rho0 * PI * a.a * a.b;
+    double inertia = a.ell ? 0.25 * mass * (a.a * a.a + a.b * a.b) : 0.5 * mass * a.r * a.r;
     double st[6] = {a.x, a.y, a.theta, a.ux, a.uy, a.omega};
     oracle_integrate(st, Ftx[ia], Fty[ia], a.Tz, mass, inertia);
+    if (a.ell) oracle_rotate_unit(&a.c, &a.s, 0.5 * (a.omega + st[5]));
     a.x = st[0];
     a.y = st[1];
     a.theta = st[2];
@@ -395,7 +467,16 @@ int step_once(oracle_lbm* h) {
       if (!(p >= 0 && own_new[x] < 0)) continue;
       const Particle& a = h->parts[p]; /* state at t+1 */
       double dxn = (double)i - a.x, dyn = (double)j - a.y;
-      int c = oracle_refill_direction(dxn, dyn);
+      /* outward normal of the wall at the newborn node: radial for a circle; for an
+       * ellipse the gradient of (u/a)^2 + (v/b)^2 turned back into the lattice frame */
+      double nrx = dxn, nry = dyn;
+      if (a.ell) {
+        double u = dxn * a.c + dyn * a.s, v = dyn * a.c - dxn * a.s;
+        double gu = (u / a.a) / a.a, gv = (v / a.b) / a.b;
+        nrx = gu * a.c - gv * a.s;
+        nry = gu * a.s + gv * a.c;
+      }
+      int c = oracle_refill_direction(nrx, nry);
       int nvalid = 0;
       long long xs[3] = {-1, -1, -1};
       for (int k = 1; k <= 3; ++k) {
@@ -593,6 +674,41 @@ extern "C" double oracle_link_q(double xf, double yf, int alpha, double xc, doub
   return t;
 }
 
+/* q for an ellipse: smaller root of the ray-ellipse quadratic in the body frame,
+ * |((u + t eu)/a, (v + t ev)/b)|^2 = 1 (definition of q) */
+extern "C" double oracle_link_q_ellipse(double xf, double yf, int alpha, double xc, double yc,
+                                        double a, double b, double c, double s) {
+  double ex = (double)EX[alpha], ey = (double)EY[alpha];
+  double dx = xf - xc, dy = yf - yc;
+  double u = dx * c + dy * s, v = dy * c - dx * s;
+  double eu = ex * c + ey * s, ev = ey * c - ex * s;
+  double ua = u / a, vb = v / b, ea = eu / a, eb = ev / b;
+  double A = ea * ea + eb * eb;
+  double B = 2.0 * (ua * ea + vb * eb);
+  double C = (ua * ua + vb * vb) - 1.0;
+  double disc = B * B - 4.0 * A * C;
+  if (disc < 0.0) disc = 0.0;
+  double t = (-B - std::sqrt(disc)) / (2.0 * A);
+  if (t < 0.0) t = 0.0;
+  if (t > 1.0) t = 1.0;
+  return t;
+}
+
+/* orientation unit vector advanced by the angle increment d through the Cayley rotation
+ * (cr, sr) = ((1 - t^2)/(1 + t^2), 2t/(1 + t^2)), t = d/2 (a rotation by 2 atan(d/2) = d + O(d^3)),
+ * then renormalised: only +, -, *, /, sqrt, so both implementations produce the same bits */
+extern "C" void oracle_rotate_unit(double* c, double* s, double d) {
+  double t = 0.5 * d;
+  double den = 1.0 + t * t;
+  double cr = (1.0 - t * t) / den;
+  double sr = (2.0 * t) / den;
+  double c1 = (*c) * cr - (*s) * sr;
+  double s1 = (*s) * cr + (*c) * sr;
+  double nrm = std::sqrt(c1 * c1 + s1 * s1);
+  *c = c1 / nrm;
+  *s = s1 / nrm;
+}
+
 /* Eq. (9) for q <= 1/2, Eq. (10) for q > 1/2, moving-wall term
  * 2 w_i rho0 (e_ibar . u_w)/c_s^2.  Fallback ladder (reading):
  *  q <= 1/2: nbehind=2 Eq.(9); nbehind=1 linear 2q f_i(x_f) + (1-2q) f_i(x_f-e_i); nbehind=0 halfway
@@ -756,11 +872,13 @@ extern "C" int oracle_set_temperature(oracle_lbm_t* h, const double* T) {
   return 0;
 }
 
-extern "C" int oracle_add_particles(oracle_lbm_t* h, int n, const double* x, const double* y,
-                                    const double* diam, const double* rho_ratio, const double* T_w,
-                                    const double* ux, const double* uy, const double* omega,
-                                    const unsigned char* fixed) {
-  if (!h || n < 0 || (n > 0 && (!x || !y || !diam || !rho_ratio || !T_w))) return E_ARG;
+/* circles: minor == NULL and theta == NULL; ellipses: full axes 2a = major[k], 2b = minor[k],
+ * theta[k] = angle of the a axis to the x axis (cos / sin taken once, here, by the host libm) */
+static int add_shapes(oracle_lbm_t* h, int n, const double* x, const double* y, const double* major,
+                      const double* minor, const double* theta, const double* rho_ratio,
+                      const double* T_w, const double* ux, const double* uy, const double* omega,
+                      const unsigned char* fixed) {
+  if (!h || n < 0 || (n > 0 && (!x || !y || !major || !rho_ratio || !T_w))) return E_ARG;
   if (h->steps_done > 0) return fail(h, E_STATE, "add_particles after the first step");
   if ((long long)h->parts.size() + n > h->P.max_particles)
     return fail(h, E_CAPACITY, "max_particles exceeded");
@@ -769,22 +887,32 @@ extern "C" int oracle_add_particles(oracle_lbm_t* h, int n, const double* x, con
     Particle a{};
     a.x = x[k];
     a.y = y[k];
-    a.r = 0.5 * diam[k];
+    a.a = 0.5 * major[k];
+    a.b = minor ? 0.5 * minor[k] : a.a;
+    a.theta = theta ? theta[k] : 0.0;
+    a.ell = (a.a != a.b);
+    a.c = a.ell ? std::cos(a.theta) : 1.0;
+    a.s = a.ell ? std::sin(a.theta) : 0.0;
+    a.r = a.a > a.b ? a.a : a.b; /* radius of a circle; largest semi-axis of an ellipse */
     a.rho_ratio = rho_ratio[k];
     a.Tw = T_w[k];
     a.ux = ux ? ux[k] : 0.0;
     a.uy = uy ? uy[k] : 0.0;
     a.omega = omega ? omega[k] : 0.0;
     a.fixed = fixed ? (fixed[k] != 0) : 0;
-    if (!(a.r > 0.0) || !(a.rho_ratio > 0.0)) return fail(h, E_ARG, "bad diameter or density");
+    if (!(a.a > 0.0) || !(a.b > 0.0) || !(a.rho_ratio > 0.0))
+      return fail(h, E_ARG, "bad diameter or density");
     if (!std::isfinite(a.x) || !std::isfinite(a.y) || !std::isfinite(a.ux) ||
-        !std::isfinite(a.uy) || !std::isfinite(a.omega) || !std::isfinite(a.Tw))
+        !std::isfinite(a.uy) || !std::isfinite(a.omega) || !std::isfinite(a.Tw) ||
+        !std::isfinite(a.theta) || !std::isfinite(a.r))
       return fail(h, E_ARG, "non-finite particle input");
+    double hx, hy;
+    half_extents(a, &hx, &hy);
     /* strictly inside the cavity walls at -1/2 and n-1/2 */
-    if (!(a.y - a.r > -0.5) || !(a.y + a.r < h->ny - 0.5))
+    if (!(a.y - hy > -0.5) || !(a.y + hy < h->ny - 0.5))
       return fail(h, E_ARG, "particle touches a y wall");
     if (!h->P.periodic_x) {
-      if (!(a.x - a.r > -0.5) || !(a.x + a.r < h->nx - 0.5))
+      if (!(a.x - hx > -0.5) || !(a.x + hx < h->nx - 0.5))
         return fail(h, E_ARG, "particle touches an x wall");
     } else {
       if ((int)std::floor(a.x - a.r) - 2 < 0 || (int)std::floor(a.x + a.r) + 2 > h->nx - 1)
@@ -793,19 +921,39 @@ extern "C" int oracle_add_particles(oracle_lbm_t* h, int n, const double* x, con
     int Nmax = (int)std::floor(2.0 * a.r) + 4; /* worst-case N of PAPER.md:258 for this diameter */
     if (12 * Nmax - 12 > h->P.max_links_per_particle)
       return fail(h, E_CAPACITY, "12N-12 exceeds max_links_per_particle");
-    for (const Particle& b : h->parts) {
+    auto overlaps = [&](const Particle& b) {
       double dx = a.x - b.x, dy = a.y - b.y;
-      if (std::sqrt(dx * dx + dy * dy) < a.r + b.r) return fail(h, E_ARG, "particles overlap");
-    }
-    for (const Particle& b : add) {
-      double dx = a.x - b.x, dy = a.y - b.y;
-      if (std::sqrt(dx * dx + dy * dy) < a.r + b.r) return fail(h, E_ARG, "particles overlap");
-    }
+      double dist = std::sqrt(dx * dx + dy * dy);
+      if (!a.ell && !b.ell) return dist < a.r + b.r;
+      if (!(dist > 0.0)) return true;
+      /* support-function gap along the line of centres (conservative for ellipses) */
+      return dist < support_p(a, dx / dist, dy / dist) + support_p(b, dx / dist, dy / dist);
+    };
+    for (const Particle& b : h->parts)
+      if (overlaps(b)) return fail(h, E_ARG, "particles overlap");
+    for (const Particle& b : add)
+      if (overlaps(b)) return fail(h, E_ARG, "particles overlap");
     add.push_back(a);
   }
   for (const Particle& a : add) h->parts.push_back(a);
   compute_owner(h, h->owner);
   return 0;
+}
+
+extern "C" int oracle_add_particles(oracle_lbm_t* h, int n, const double* x, const double* y,
+                                    const double* diam, const double* rho_ratio, const double* T_w,
+                                    const double* ux, const double* uy, const double* omega,
+                                    const unsigned char* fixed) {
+  return add_shapes(h, n, x, y, diam, nullptr, nullptr, rho_ratio, T_w, ux, uy, omega, fixed);
+}
+
+extern "C" int oracle_add_ellipses(oracle_lbm_t* h, int n, const double* x, const double* y,
+                                   const double* major, const double* minor, const double* theta,
+                                   const double* rho_ratio, const double* T_w, const double* ux,
+                                   const double* uy, const double* omega,
+                                   const unsigned char* fixed) {
+  if (n > 0 && (!minor || !theta)) return E_ARG;
+  return add_shapes(h, n, x, y, major, minor, theta, rho_ratio, T_w, ux, uy, omega, fixed);
 }
 
 extern "C" int oracle_step(oracle_lbm_t* h, int nsteps) {
@@ -904,7 +1052,7 @@ extern "C" int oracle_get_links_bruteforce(oracle_lbm_t* h, long long* n, int* p
   const int np = (int)h->parts.size();
   auto covering = [&](int a, int b) -> int { /* lowest pid whose disc covers node (a,b) */
     for (int p = 0; p < np; ++p)
-      if (inside((double)a, (double)b, h->parts[p].x, h->parts[p].y, h->parts[p].r)) return p;
+      if (inside_p(h->parts[p], (double)a, (double)b)) return p;
     return -1;
   };
   std::vector<Link> links;
@@ -921,8 +1069,7 @@ extern "C" int oracle_get_links_bruteforce(oracle_lbm_t* h, long long* n, int* p
           L.i = a;
           L.j = b;
           L.alpha = al;
-          L.q = oracle_link_q((double)a, (double)b, al, h->parts[p].x, h->parts[p].y,
-                              h->parts[p].r);
+          L.q = q_p(h->parts[p], (double)a, (double)b, al);
           links.push_back(L);
         }
   return copy_links(links, n, pid, i, j, alpha, q);

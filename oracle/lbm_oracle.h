@@ -40,6 +40,12 @@ int  oracle_add_particles(oracle_lbm_t* h, int n, const double* x, const double*
                           const double* diam, const double* rho_ratio, const double* T_w,
                           const double* ux, const double* uy, const double* omega,
                           const unsigned char* fixed);
+/* elliptical particles: full axes major (along the body axis that makes the
+ * angle theta with x) and minor; equal axes = a circle through the circle formulas */
+int  oracle_add_ellipses(oracle_lbm_t* h, int n, const double* x, const double* y,
+                         const double* major, const double* minor, const double* theta,
+                         const double* rho_ratio, const double* T_w, const double* ux,
+                         const double* uy, const double* omega, const unsigned char* fixed);
 int  oracle_step(oracle_lbm_t* h, int nsteps);
 int  oracle_get_fields(oracle_lbm_t* h, double* rho, double* ux, double* uy, double* T,
                        double* f, double* g, unsigned char* flag);
@@ -70,6 +76,9 @@ void   oracle_macroscopic(const oracle_params* p, const double* f9, const double
 void   oracle_collide_node(const oracle_params* p, const double* f9, const double* g5,
                            double* fpost9, double* gpost5);                 /* Eqs. (5), (6)  */
 double oracle_link_q(double xf, double yf, int alpha, double xc, double yc, double r);
+double oracle_link_q_ellipse(double xf, double yf, int alpha, double xc, double yc, double a,
+                             double b, double c, double s);
+void oracle_rotate_unit(double* c, double* s, double d);
 /* Eqs. (9)/(10) with the fallback ladder; nbehind = how many of x_f-e_i, x_f-2e_i are fluid
  * (counted contiguously from x_f): 2, 1 or 0.  fi_k = f_i^+(x_f - k e_i), fib_k = f_ibar^+(...) */
 double oracle_bounce_back_f(int alpha, double q, double fi_0, double fi_1, double fi_2,

@@ -52,6 +52,10 @@ def lib():
         _lib = C.CDLL(_build.build())
         L = _lib
         L.oracle_last_error.restype = C.c_char_p
+        L.oracle_link_q_ellipse.restype = C.c_double
+        L.oracle_link_q_ellipse.argtypes = [C.c_double, C.c_double, C.c_int] + [C.c_double] * 6
+        L.oracle_rotate_unit.restype = None
+        L.oracle_rotate_unit.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double]
         L.oracle_link_q.restype = C.c_double
         L.oracle_link_q.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double, C.c_double, C.c_double]
         L.oracle_bounce_back_f.restype = C.c_double
@@ -152,6 +156,16 @@ def link_q(xf, yf, alpha, xc, yc, r):
     return lib().oracle_link_q(xf, yf, alpha, xc, yc, r)
 
 
+def link_q_ellipse(xf, yf, alpha, xc, yc, a, b, c, s):
+    return lib().oracle_link_q_ellipse(xf, yf, alpha, xc, yc, a, b, c, s)
+
+
+def rotate_unit(c, s, d):
+    cc, ss = C.c_double(c), C.c_double(s)
+    lib().oracle_rotate_unit(C.byref(cc), C.byref(ss), d)
+    return cc.value, ss.value
+
+
 def bounce_back_f(alpha, q, fi_0, fi_1, fi_2, fib_0, fib_1, nbehind, rho0, uwx, uwy):
     return lib().oracle_bounce_back_f(alpha, q, fi_0, fi_1, fi_2, fib_0, fib_1, nbehind, rho0, uwx, uwy)
 
@@ -235,10 +249,20 @@ class OracleSim:
         assert T.size == self.n
         self._chk(lib().oracle_set_temperature(self._h, _d(T)))
 
-    def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None):
+    def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None,
+                      minor=None, theta=None):
+        """Circles of diameter `diam`; with `minor` and `theta`: ellipses of full axes diam x minor,
+        the `diam` axis at angle theta to x."""
         c = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64)  # noqa: E731
         x, y, diam, rho_ratio, T_w, ux, uy, omega = map(c, (x, y, diam, rho_ratio, T_w, ux, uy, omega))
         fx = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.uint8)
+        if minor is not None:
+            minor = c(minor)
+            theta = c(np.zeros_like(x) if theta is None else theta)
+            self._chk(lib().oracle_add_ellipses(
+                self._h, int(x.size), _d(x), _d(y), _d(diam), _d(minor), _d(theta), _d(rho_ratio),
+                _d(T_w), _d(ux), _d(uy), _d(omega), None if fx is None else fx.ctypes.data_as(_bp)))
+            return
         self._chk(lib().oracle_add_particles(
             self._h, int(x.size), _d(x), _d(y), _d(diam), _d(rho_ratio), _d(T_w), _d(ux), _d(uy),
             _d(omega), None if fx is None else fx.ctypes.data_as(_bp)))

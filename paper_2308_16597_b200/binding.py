@@ -72,6 +72,7 @@ def load_library():
     L.lbm_create.argtypes = [C.c_int, C.c_int, P, vp, sz, vp, C.POINTER(vp)]
     L.lbm_set_temperature.argtypes = [vp, _dp]
     L.lbm_add_particles.argtypes = [vp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
+    L.lbm_add_ellipses.argtypes = [vp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_step.argtypes = [vp, C.c_int]
     L.lbm_set_overlap.argtypes = [vp, C.c_int]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
@@ -87,7 +88,7 @@ def load_library():
     L.lbm_destroy.argtypes = [vp]
     L.lbm_last_error.argtypes = [vp]
     L.lbm_last_error.restype = C.c_char_p
-    for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_step",
+    for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_add_ellipses", "lbm_step",
                  "lbm_get_fields", "lbm_get_particles", "lbm_get_links", "lbm_profile_enable",
                  "lbm_profile_kernels", "lbm_profile_get", "lbm_destroy", "lbm_set_overlap"):
         getattr(L, name).restype = C.c_int
@@ -167,9 +168,19 @@ class Simulation:
         assert T.size == self.n
         self._chk(self._L.lbm_set_temperature(self._h, _d(T)))
 
-    def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None):
+    def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None,
+                      minor=None, theta=None):
+        """lbm_add_particles; with `minor` (and `theta`): lbm_add_ellipses, full axes diam x minor,
+        the `diam` axis at angle theta to x."""
         x, y, diam, rho_ratio, T_w, ux, uy, omega = map(_host, (x, y, diam, rho_ratio, T_w, ux, uy, omega))
         fx = None if fixed is None else np.ascontiguousarray(fixed, dtype=np.uint8)
+        if minor is not None:
+            minor = _host(minor)
+            theta = _host(np.zeros_like(x) if theta is None else theta)
+            self._chk(self._L.lbm_add_ellipses(
+                self._h, int(x.size), _d(x), _d(y), _d(diam), _d(minor), _d(theta), _d(rho_ratio),
+                _d(T_w), _d(ux), _d(uy), _d(omega), None if fx is None else fx.ctypes.data_as(_bp)))
+            return
         self._chk(self._L.lbm_add_particles(
             self._h, int(x.size), _d(x), _d(y), _d(diam), _d(rho_ratio), _d(T_w), _d(ux), _d(uy),
             _d(omega), None if fx is None else fx.ctypes.data_as(_bp)))

@@ -186,11 +186,25 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
     // state at t+1 (cur already points at the new buffer)
     const double dxn = (double)i - pa.x[cur][p], dyn = (double)j - pa.y[cur][p];
     // e_c maximises n . e_alpha/|e_alpha|, ties -> lowest alpha; separately rounded operations
+    // outward normal of the wall at the node: radial for a circle; for an ellipse the gradient of
+    // (u/a)^2 + (v/b)^2 turned back into the lattice frame (explicitly rounded, as the oracle)
+    double nrx = dxn, nry = dyn;
+    {
+      const double ea = pa.a[p], eb = pa.b[p];
+      if (ea != eb) {
+        const double oc = pa.cs[cur][p], os = pa.sn[cur][p];
+        const double u = __dadd_rn(__dmul_rn(dxn, oc), __dmul_rn(dyn, os));
+        const double v = __dsub_rn(__dmul_rn(dyn, oc), __dmul_rn(dxn, os));
+        const double gu = __ddiv_rn(__ddiv_rn(u, ea), ea), gv = __ddiv_rn(__ddiv_rn(v, eb), eb);
+        nrx = __dsub_rn(__dmul_rn(gu, oc), __dmul_rn(gv, os));
+        nry = __dadd_rn(__dmul_rn(gu, os), __dmul_rn(gv, oc));
+      }
+    }
     int ec = 1;
     double best = -1.0e300;
 #pragma unroll
     for (int a = 1; a <= 8; ++a) {
-      double s = __dadd_rn(__dmul_rn(dxn, (double)b_ex[a]), __dmul_rn(dyn, (double)b_ey[a]));
+      double s = __dadd_rn(__dmul_rn(nrx, (double)b_ex[a]), __dmul_rn(nry, (double)b_ey[a]));
       if (a >= 5) s = __dmul_rn(s, 0.70710678118654752440);
       if (s > best) { best = s; ec = a; }
     }

@@ -89,6 +89,12 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
     pa.uy[b] = c.take<double>(np);
     pa.omega[b] = c.take<double>(np);
   }
+  for (int b = 0; b < 2; ++b) {
+    pa.cs[b] = c.take<double>(np);
+    pa.sn[b] = c.take<double>(np);
+  }
+  pa.a = c.take<double>(np);
+  pa.b = c.take<double>(np);
   pa.r = c.take<double>(np);
   pa.rho_ratio = c.take<double>(np);
   pa.Tw = c.take<double>(np);
@@ -349,9 +355,12 @@ int lbm_set_temperature(lbm_t* h, const double* T_host) {
   return LBM_OK;
 }
 
-int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const double* diam,
-                      const double* rho_ratio, const double* T_w, const double* ux,
-                      const double* uy, const double* omega, const unsigned char* fixed) {
+// circles: minor == theta == NULL; ellipses: full axes diam (the axis at angle theta to x) x minor.
+// cos / sin of theta are taken once, here, by the host libm (as the oracle does).
+static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const double* diam,
+                      const double* minor, const double* theta, const double* rho_ratio,
+                      const double* T_w, const double* ux, const double* uy, const double* omega,
+                      const unsigned char* fixed) {
   if (!h) return LBM_E_ARG;
   if (n < 0 || (n > 0 && (!x || !y || !diam || !rho_ratio || !T_w)))
     return fail(h, LBM_E_ARG, "add_particles: NULL array or negative count");
@@ -362,8 +371,12 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
 
   // existing particles (host mirror via a device read; add_particles is a set-up call)
   const int n0 = h->np, nt = n0 + n;
-  std::vector<double> X(nt), Y(nt), R(nt);
+  std::vector<double> X(nt), Y(nt), R(nt), SA(nt), SB(nt), SC(nt), SS(nt);
   if (n0) {
+    CUDA_OK(h, cudaMemcpyAsync(SA.data(), h->pa.a, n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpyAsync(SB.data(), h->pa.b, n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpyAsync(SC.data(), h->pa.cs[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpyAsync(SS.data(), h->pa.sn[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaMemcpyAsync(X.data(), h->pa.x[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaMemcpyAsync(Y.data(), h->pa.y[h->cur], n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaMemcpyAsync(R.data(), h->pa.r, n0 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -371,15 +384,25 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   }
   double dmax = h->d_max;
   for (int k = 0; k < n; ++k) {
-    const double r = 0.5 * diam[k];
-    if (!(r > 0.0) || !(rho_ratio[k] > 0.0) || !std::isfinite(x[k]) || !std::isfinite(y[k]) ||
-        !std::isfinite(r) || !std::isfinite(T_w[k]) || (ux && !std::isfinite(ux[k])) ||
+    const double sa = 0.5 * diam[k], sb = minor ? 0.5 * minor[k] : sa;
+    const double th = theta ? theta[k] : 0.0;
+    const bool ell = sa != sb;
+    const double r = sa > sb ? sa : sb;   // radius of a circle; largest semi-axis of an ellipse
+    if (!(sa > 0.0) || !(sb > 0.0) || !(rho_ratio[k] > 0.0) || !std::isfinite(x[k]) || !std::isfinite(y[k]) ||
+        !std::isfinite(r) || !std::isfinite(th) || !std::isfinite(T_w[k]) || (ux && !std::isfinite(ux[k])) ||
         (uy && !std::isfinite(uy[k])) || (omega && !std::isfinite(omega[k])))
       return fail(h, LBM_E_ARG, "add_particles: particle %d has a bad or non-finite value", k);
-    if (!(y[k] - r > -0.5) || !(y[k] + r < h->ny - 0.5))
+    const double oc = ell ? std::cos(th) : 1.0, os = ell ? std::sin(th) : 0.0;
+    double hx = r, hy = r;                // half extents of the bounding box
+    if (ell) {
+      const double ac = sa * oc, bs = sb * os, as = sa * os, bc = sb * oc;
+      hx = std::sqrt(ac * ac + bs * bs);
+      hy = std::sqrt(as * as + bc * bc);
+    }
+    if (!(y[k] - hy > -0.5) || !(y[k] + hy < h->ny - 0.5))
       return fail(h, LBM_E_ARG, "add_particles: particle %d touches a y wall", k);
     if (!h->P.periodic_x) {
-      if (!(x[k] - r > -0.5) || !(x[k] + r < h->nx - 0.5))
+      if (!(x[k] - hx > -0.5) || !(x[k] + hx < h->nx - 0.5))
         return fail(h, LBM_E_ARG, "add_particles: particle %d touches an x wall", k);
     } else if ((int)std::floor(x[k] - r) - 2 < 0 || (int)std::floor(x[k] + r) + 2 > h->nx - 1) {
       return fail(h, LBM_E_ARG, "add_particles: zone of particle %d crosses the periodic seam", k);
@@ -391,6 +414,10 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
     X[n0 + k] = x[k];
     Y[n0 + k] = y[k];
     R[n0 + k] = r;
+    SA[n0 + k] = sa;
+    SB[n0 + k] = sb;
+    SC[n0 + k] = oc;
+    SS[n0 + k] = os;
     dmax = std::max(dmax, 2.0 * r);
   }
   // overlap test through a host cell grid (cell >= largest diameter)
@@ -406,7 +433,19 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
             if (it == grid.end()) continue;
             for (int m : it->second) {
               const double dx = X[k] - X[m], dy = Y[k] - Y[m];
-              if (std::sqrt(dx * dx + dy * dy) < R[k] + R[m])
+              const double dist = std::sqrt(dx * dx + dy * dy);
+              // circles: centre distance against r_a + r_b; with an ellipse: the support
+              // functions along the line of centres (conservative)
+              auto support = [&](int q, double nx, double ny) {
+                if (SA[q] == SB[q]) return R[q];
+                const double mm = nx * SC[q] + ny * SS[q], ww = ny * SC[q] - nx * SS[q];
+                const double am = SA[q] * mm, bw = SB[q] * ww;
+                return std::sqrt(am * am + bw * bw);
+              };
+              bool bad;
+              if (SA[k] == SB[k] && SA[m] == SB[m]) bad = dist < R[k] + R[m];
+              else bad = !(dist > 0.0) || dist < support(k, dx / dist, dy / dist) + support(m, dx / dist, dy / dist);
+              if (bad)
                 return fail(h, LBM_E_ARG, "add_particles: particles %d and %d overlap", m, k);
             }
           }
@@ -416,7 +455,7 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   // upload
   const int c = h->cur;
   std::vector<double> zero(n, 0.0), rr(n);
-  for (int k = 0; k < n; ++k) rr[k] = 0.5 * diam[k];
+  for (int k = 0; k < n; ++k) rr[k] = R[n0 + k];
   std::vector<unsigned char> fx(n, 0);
   if (fixed)
     for (int k = 0; k < n; ++k) fx[k] = fixed[k] ? 1 : 0;
@@ -426,12 +465,16 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   for (int b = 0; b < 2; ++b) {
     CUDA_OK(h, up(h->pa.x[b], x));
     CUDA_OK(h, up(h->pa.y[b], y));
-    CUDA_OK(h, up(h->pa.theta[b], nullptr));
+    CUDA_OK(h, up(h->pa.theta[b], theta));
+    CUDA_OK(h, up(h->pa.cs[b], SC.data() + n0));
+    CUDA_OK(h, up(h->pa.sn[b], SS.data() + n0));
     CUDA_OK(h, up(h->pa.ux[b], ux));
     CUDA_OK(h, up(h->pa.uy[b], uy));
     CUDA_OK(h, up(h->pa.omega[b], omega));
   }
   CUDA_OK(h, up(h->pa.r, rr.data()));
+  CUDA_OK(h, up(h->pa.a, SA.data() + n0));
+  CUDA_OK(h, up(h->pa.b, SB.data() + n0));
   CUDA_OK(h, up(h->pa.rho_ratio, rho_ratio));
   CUDA_OK(h, up(h->pa.Tw, T_w));
   CUDA_OK(h, up(h->pa.Fx, nullptr));
@@ -440,6 +483,7 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   CUDA_OK(h, cudaMemcpyAsync(h->pa.fixed + n0, fx.data(), n, cudaMemcpyHostToDevice, h->stream));
   CUDA_OK(h, cudaMemsetAsync(h->pa.ovl + n0, 0, n, h->stream));
   h->np = nt;
+  for (int k = n0; k < nt; ++k) h->n_ell += (SA[k] != SB[k]) ? 1 : 0;
   h->d_max = dmax;
   size_chain(h);
   h->cell = std::max(dmax + h->P.rep_s, MIN_CELL);
@@ -454,6 +498,20 @@ int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const d
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
   return LBM_OK;
+}
+
+int lbm_add_particles(lbm_t* h, int n, const double* x, const double* y, const double* diam,
+                      const double* rho_ratio, const double* T_w, const double* ux,
+                      const double* uy, const double* omega, const unsigned char* fixed) {
+  return add_shapes(h, n, x, y, diam, nullptr, nullptr, rho_ratio, T_w, ux, uy, omega, fixed);
+}
+
+int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const double* major,
+                     const double* minor, const double* theta, const double* rho_ratio,
+                     const double* T_w, const double* ux, const double* uy, const double* omega,
+                     const unsigned char* fixed) {
+  if (h && n > 0 && (!minor || !theta)) return fail(h, LBM_E_ARG, "add_ellipses: NULL array");
+  return add_shapes(h, n, x, y, major, minor, theta, rho_ratio, T_w, ux, uy, omega, fixed);
 }
 
 // Step schedule: the resident state A is f+(x,t), g+(x,t), the index array holds

@@ -74,7 +74,11 @@ struct LbmConst {
 
 struct ParticleArrays {      // SoA in the workspace, each max_particles long
   double *x[2], *y[2], *theta[2], *ux[2], *uy[2], *omega[2];   // double-buffered state
-  double *r, *rho_ratio, *Tw;
+  double *r, *rho_ratio, *Tw;   // r: radius of a circle, largest semi-axis of an ellipse
+  // elliptical particles: semi-axes a, b
+  // (a == b: a circle, which takes the circle formulas bit for bit) and the orientation as a unit
+  // vector (cs, sn), double-buffered with the state and advanced without any cos / sin
+  double *a, *b, *cs[2], *sn[2];
   double *Fx, *Fy, *Tz;      // hydrodynamic force / torque of the last step (Eqs. 13, 14)
   unsigned char* fixed;
   unsigned char* ovl;        // sticky: the disc may share nodes with another particle's (k_cover)
@@ -108,6 +112,7 @@ struct lbm {
   LinkArrays la;
   int cur;                   // which particle state buffer is current
   int np;                    // particles added
+  int n_ell;                 // of which ellipses (a != b): selects the kernel instantiations
   double d_max;              // largest diameter (sizes the repulsion grid)
   int* cell_count;
   int* cell_items;

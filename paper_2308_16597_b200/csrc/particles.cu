@@ -40,6 +40,99 @@ __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc
   return t;
 }
 
+// ---- shapes.  A particle is a circle (a == b: the formulas above, bit for bit) or an ellipse with
+// semi-axes a, b and orientation unit vector (c, s) (DESIGN.md "Elliptical
+// particles").  Every expression below is the oracle's, operation for operation (-fmad=false).
+struct Shape {
+  double x, y, r, a, b, c, s;
+  bool ell;
+};
+
+// ELL = false: the simulation holds circles only; the shape is then a compile-time circle and
+// every ellipse branch of the kernels folds away (same code and registers as before ellipses).
+template <bool ELL>
+__device__ __forceinline__ Shape load_shape(const ParticleArrays& pa, int buf, int p) {
+  Shape S;
+  S.x = pa.x[buf][p];
+  S.y = pa.y[buf][p];
+  S.r = pa.r[p];
+  if (ELL) {
+    S.a = pa.a[p];
+    S.b = pa.b[p];
+    S.ell = S.a != S.b;
+    S.c = S.ell ? pa.cs[buf][p] : 1.0;
+    S.s = S.ell ? pa.sn[buf][p] : 0.0;
+  } else {
+    S.a = S.r;
+    S.b = S.r;
+    S.ell = false;
+    S.c = 1.0;
+    S.s = 0.0;
+  }
+  return S;
+}
+
+__device__ __forceinline__ bool inside_ellipse(double xi, double yj, const Shape& S) {
+  const double dx = xi - S.x, dy = yj - S.y;
+  const double u = dx * S.c + dy * S.s;
+  const double v = dy * S.c - dx * S.s;
+  const double ua = u / S.a, vb = v / S.b;
+  return ua * ua + vb * vb <= 1.0;
+}
+
+__device__ __forceinline__ bool inside_shape(double xi, double yj, const Shape& S) {
+  return S.ell ? inside_ellipse(xi, yj, S) : inside_disc(xi, yj, S.x, S.y, S.r);
+}
+
+// half extents of the bounding box: r, or sqrt((a c)^2 + (b s)^2), sqrt((a s)^2 + (b c)^2)
+__device__ __forceinline__ void half_extents(const Shape& S, double& hx, double& hy) {
+  if (!S.ell) {
+    hx = S.r;
+    hy = S.r;
+    return;
+  }
+  const double ac = S.a * S.c, bs = S.b * S.s, as = S.a * S.s, bc = S.b * S.c;
+  hx = sqrt(ac * ac + bs * bs);
+  hy = sqrt(as * as + bc * bc);
+}
+
+// effective zone [INT(xc-hx)-1, INT(xc+hx)+1] x [INT(yc-hy)-1, INT(yc+hy)+1]
+__device__ __forceinline__ void zone_shape(const Shape& S, int& i0, int& i1, int& j0, int& j1) {
+  double hx, hy;
+  half_extents(S, hx, hy);
+  i0 = (int)floor(S.x - hx) - 1;
+  i1 = (int)floor(S.x + hx) + 1;
+  j0 = (int)floor(S.y - hy) - 1;
+  j1 = (int)floor(S.y + hy) + 1;
+}
+
+// q of a link towards an ellipse: smaller root of the ray-ellipse quadratic in the body frame
+__device__ __forceinline__ double link_q_ellipse(double xf, double yf, int al, const Shape& S) {
+  const double ex = (double)p_ex[al], ey = (double)p_ey[al];
+  const double dx = xf - S.x, dy = yf - S.y;
+  const double u = dx * S.c + dy * S.s, v = dy * S.c - dx * S.s;
+  const double eu = ex * S.c + ey * S.s, ev = ey * S.c - ex * S.s;
+  const double ua = u / S.a, vb = v / S.b, ea = eu / S.a, eb = ev / S.b;
+  const double A = ea * ea + eb * eb;
+  const double B = 2.0 * (ua * ea + vb * eb);
+  const double C = (ua * ua + vb * vb) - 1.0;
+  double disc = B * B - 4.0 * A * C;
+  if (disc < 0.0) disc = 0.0;
+  double t = (-B - sqrt(disc)) / (2.0 * A);
+  if (t < 0.0) t = 0.0;
+  if (t > 1.0) t = 1.0;
+  return t;
+}
+
+// support function along the unit vector (nx, ny)
+__device__ __forceinline__ double support_shape(const Shape& S, double nx, double ny) {
+  if (!S.ell) return S.r;
+  const double m = nx * S.c + ny * S.s;
+  const double w = ny * S.c - nx * S.s;
+  const double am = S.a * m, bw = S.b * w;
+  return sqrt(am * am + bw * bw);
+}
+
 // ------------------------------------------------------------------------------------------
 // a2: link builder.  grid = particles (or fewer persistent CTAs), block = LB_WARPS warps.
 //
@@ -64,11 +157,11 @@ __device__ __forceinline__ double link_q(double xf, double yf, int al, double xc
 constexpr int LB_WARPS = 4;
 constexpr int LB_T = LB_WARPS * 32;
 constexpr int LB_CPT = 4;
+template <bool ELL>
 __global__ void __launch_bounds__(LB_T)
-k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
-              const double* __restrict__ pr, const unsigned char* __restrict__ ovl,
-              const unsigned char* __restrict__ flag, const int* __restrict__ owner, LinkArrays la,
-              int np, int max_rows, int* __restrict__ status, const LbmConst c) {
+k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag,
+              const int* __restrict__ owner, LinkArrays la, int np, int max_rows,
+              int* __restrict__ status, const LbmConst c) {
   extern __shared__ int s_node[];                           // la.cap packed nodes, la.cap dir bytes,
   unsigned char* s_dir = (unsigned char*)(s_node + la.cap); // then the row tables
   int* s_off = s_node + la.cap + (la.cap + 3) / 4;          // max_rows + 1: candidates before row t
@@ -80,10 +173,11 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned FULL = 0xffffffffu;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
-  const double xc = px_[p], yc = py_[p], r = pr[p];
-  const bool check_owner = ovl[p] != 0;
+  const Shape S = load_shape<ELL>(pa, buf, p);
+  const double xc = S.x, yc = S.y, r = S.r;
+  const bool check_owner = pa.ovl[p] != 0;
   int i0, i1, j0, j1;
-  zone_of(xc, yc, r, i0, i1, j0, j1);
+  zone_shape(S, i0, i1, j0, j1);
   const int H = min(j1 - j0 + 1, max_rows);
   const double r2 = r * r;
   const double rfar = (r + 1.5) * (r + 1.5);   // beyond this no neighbour can be inside the disc
@@ -98,7 +192,9 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
       const int j = j0 + t;
       int a1 = 0, n1 = 0, a2 = 0, n2 = 0;
       const double dy = (double)j - yc, dy2 = dy * dy;
-      if (j >= 0 && j < c.ny && dy2 <= rfar) {
+      if (S.ell) {                                // first version: every column of the zone row
+        if (j >= 0 && j < c.ny && ihi >= ilo) { a1 = ilo; n1 = ihi - ilo + 1; }
+      } else if (j >= 0 && j < c.ny && dy2 <= rfar) {
         const double wo = sqrt(rfar - dy2);
         const int oa = max((int)floor(xc - wo) - 1, ilo), ob = min((int)floor(xc + wo) + 2, ihi);
         int ha = ob + 1, hb = ob;                 // hole = columns certainly inside the disc
@@ -161,6 +257,22 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
       // coordinates of the 3 x 3 neighbourhood: integers are exact in fp64, so xi + 1.0 is
       // (double)(i + 1) bit for bit and the disc test below is the rasteriser's
       const double xi = (double)i, yj = (double)j;
+      if (S.ell) {
+        if (inside_ellipse(xi, yj, S)) continue;
+        const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.ny - 1;
+        unsigned m = 0;
+        if (ei && inside_ellipse(xi + 1.0, yj, S)) m |= 1u << 1;
+        if (no && inside_ellipse(xi, yj + 1.0, S)) m |= 1u << 2;
+        if (wi && inside_ellipse(xi - 1.0, yj, S)) m |= 1u << 3;
+        if (so && inside_ellipse(xi, yj - 1.0, S)) m |= 1u << 4;
+        if (ei && no && inside_ellipse(xi + 1.0, yj + 1.0, S)) m |= 1u << 5;
+        if (wi && no && inside_ellipse(xi - 1.0, yj + 1.0, S)) m |= 1u << 6;
+        if (wi && so && inside_ellipse(xi - 1.0, yj - 1.0, S)) m |= 1u << 7;
+        if (ei && so && inside_ellipse(xi + 1.0, yj - 1.0, S)) m |= 1u << 8;
+        mask[k] = m;
+        node[k] = (int)((unsigned)i | ((unsigned)j << 16));
+        continue;
+      }
       const double dx0 = xi - xc, dy0 = yj - yc;
       const double sx0 = dx0 * dx0, sy0 = dy0 * dy0;
       const double d2 = sx0 + sy0;
@@ -271,7 +383,8 @@ k_build_links(const double* __restrict__ px_, const double* __restrict__ py_,
     const unsigned char f1 = in1 ? flag[(long long)b1 * c.px + a1] : 1;
     const unsigned char f2 = in2 ? flag[(long long)b2 * c.px + a2] : 1;
     const int behind = f1 == 1 ? 0 : (f2 == 1 ? 1 : 2);
-    la.q[base + s] = link_q((double)i, (double)j, al, xc, yc, r);
+    la.q[base + s] = S.ell ? link_q_ellipse((double)i, (double)j, al, S)
+                           : link_q((double)i, (double)j, al, xc, yc, r);
     la.node[base + s] = nd;
     la.dir[base + s] = (unsigned char)(al | (behind << LINK_BEHIND_SHIFT));
   }
@@ -301,6 +414,7 @@ __device__ __forceinline__ double repulsion_mag(double C, const LbmConst& c, dou
 // and the non-zero contributions are added in ascending particle id (warp min-reduction picks the
 // next one), so the sum order is fixed whatever order the cell slots were filled in.
 constexpr int IW = 4;   // warps (particles) per CTA
+template <bool ELL>
 __global__ void __launch_bounds__(IW * 32)
 k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
             const int* __restrict__ cell_count, const int* __restrict__ cell_items,
@@ -314,10 +428,11 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   const double PI = 3.14159265358979323846;
   // grid-size agnostic: warp w of the grid takes particles w, w + (warps in the grid), ...
   for (int ia = blockIdx.x * IW + (threadIdx.x >> 5); ia < np; ia += gridDim.x * IW) {
-  const double ax = pa.x[cur][ia], ay = pa.y[cur][ia], ar = pa.r[ia], ratio = pa.rho_ratio[ia];
-  const double Ca = PI * ar * ar * (ratio * c.rho0 - c.rho0) * c.g;
+  const Shape SA = load_shape<ELL>(pa, cur, ia);
+  const double ax = SA.x, ay = SA.y, ar = SA.r, ratio = pa.rho_ratio[ia];
+  const double Ca = PI * SA.a * SA.b * (ratio * c.rho0 - c.rho0) * c.g;   // area pi a b
   double Fx = pa.Fx[ia], Fy = pa.Fy[ia];
-  Fy += -(ratio * c.rho0 - c.rho0) * PI * ar * ar * c.g;
+  Fy += -(ratio * c.rho0 - c.rho0) * PI * SA.a * SA.b * c.g;
   int ci = (int)floor(ax / cell), cj = (int)floor(ay / cell);
   ci = min(max(ci, 0), ncx - 1);
   cj = min(max(cj, 0), ncy - 1);
@@ -352,14 +467,20 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
     if (k < total && my_cell >= 0) {
       const int best = cell_items[my_cell * CELL_CAP + my_slot];
       if (best != ia) {
-        const double bx = pa.x[cur][best], by = pa.y[cur][best], br = pa.r[best];
+        const Shape SB = load_shape<ELL>(pa, cur, best);
+        const double bx = SB.x, by = SB.y, br = SB.r;
         const double dx = ax - bx, dy = ay - by;
         const double reach = ar + br + c.rep_s;
         if (!(fabs(dx) > reach || fabs(dy) > reach)) {
           const double dist = sqrt(dx * dx + dy * dy);
-          const double delta = dist - ar - br;
+          // gap along the line of centres through the support functions (two circles: ra + rb)
+          double delta = dist - ar - br;
+          if ((SA.ell || SB.ell) && dist > 0.0) {
+            const double nxh = dx / dist, nyh = dy / dist;
+            delta = dist - support_shape(SA, nxh, nyh) - support_shape(SB, nxh, nyh);
+          }
           if (delta <= c.rep_s && dist > 0.0) {
-            const double Cb = PI * br * br * (pa.rho_ratio[best] * c.rho0 - c.rho0) * c.g;
+            const double Cb = PI * SB.a * SB.b * (pa.rho_ratio[best] * c.rho0 - c.rho0) * c.g;
             const double mag = repulsion_mag(0.5 * (Ca + Cb), c, delta);
             fx = mag * (dx / dist);
             fy = mag * (dy / dist);
@@ -380,25 +501,39 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
     }
   }
   if (lane != 0) continue;
+  double ahx, ahy;
+  half_extents(SA, ahx, ahy);
   if (!c.periodic_x) {
-    const double dW = (ax + 0.5) - ar;
+    const double dW = (ax + 0.5) - ahx;
     if (dW <= c.rep_s) Fx += repulsion_mag(Ca, c, dW);
-    const double dE = ((double)c.nx - 0.5 - ax) - ar;
+    const double dE = ((double)c.nx - 0.5 - ax) - ahx;
     if (dE <= c.rep_s) Fx -= repulsion_mag(Ca, c, dE);
   }
-  const double dS = (ay + 0.5) - ar;
+  const double dS = (ay + 0.5) - ahy;
   if (dS <= c.rep_s) Fy += repulsion_mag(Ca, c, dS);
-  const double dN = ((double)c.ny - 0.5 - ay) - ar;
+  const double dN = ((double)c.ny - 0.5 - ay) - ahy;
   if (dN <= c.rep_s) Fy -= repulsion_mag(Ca, c, dN);
 
   double x = ax, y = ay, th = pa.theta[cur][ia];
   double ux = pa.ux[cur][ia], uy = pa.uy[cur][ia], om = pa.omega[cur][ia];
+  double oc = SA.c, os = SA.s;
   if (!pa.fixed[ia]) {
-    const double mass = ratio * c.rho0 * PI * ar * ar;
-    const double inertia = 0.5 * mass * ar * ar;
+    const double mass = ratio * c.rho0 * PI * SA.a * SA.b;
+    const double inertia = SA.ell ? 0.25 * mass * (SA.a * SA.a + SA.b * SA.b) : 0.5 * mass * ar * ar;
     const double ux1 = ux + Fx / mass;
     const double uy1 = uy + Fy / mass;
     const double om1 = om + pa.Tz[ia] / inertia;
+    if (SA.ell) {
+      // orientation unit vector advanced by the Cayley rotation of the angle increment
+      // (only +, -, *, /, sqrt: the oracle's operations)
+      const double t = 0.5 * (0.5 * (om + om1));
+      const double den = 1.0 + t * t;
+      const double cr = (1.0 - t * t) / den, sr = (2.0 * t) / den;
+      const double c1 = oc * cr - os * sr, s1 = os * cr + oc * sr;
+      const double nrm = sqrt(c1 * c1 + s1 * s1);
+      oc = c1 / nrm;
+      os = s1 / nrm;
+    }
     x = x + 0.5 * (ux + ux1);
     y = y + 0.5 * (uy + uy1);
     th = th + 0.5 * (om + om1);
@@ -409,6 +544,8 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   pa.x[nxt][ia] = x;
   pa.y[nxt][ia] = y;
   pa.theta[nxt][ia] = th;
+  pa.cs[nxt][ia] = oc;
+  pa.sn[nxt][ia] = os;
   pa.ux[nxt][ia] = ux;
   pa.uy[nxt][ia] = uy;
   pa.omega[nxt][ia] = om;
@@ -432,6 +569,7 @@ __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const L
 
 // Phase A: nodes owned by p that the disc at its NEW position no longer covers become newborn
 // candidates (flag 2, owner NONE) and are appended to the newborn list.
+template <bool ELL>
 __global__ void __launch_bounds__(PT)
 k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, int* __restrict__ owner,
           int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
@@ -442,13 +580,12 @@ k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, 
   const int nxt = cur ^ 1;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   if (pa.fixed[p]) continue;
-  const double xo = pa.x[cur][p], yo = pa.y[cur][p], r = pa.r[p];
-  const double xn = pa.x[nxt][p], yn = pa.y[nxt][p];
+  const Shape So = load_shape<ELL>(pa, cur, p), Sn = load_shape<ELL>(pa, nxt, p);
   int i0, i1, j0, j1;
-  zone_of(xo, yo, r, i0, i1, j0, j1);
+  zone_shape(So, i0, i1, j0, j1);
   for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
-    if (!inside_disc((double)i, (double)j, xo, yo, r)) return;
-    if (inside_disc((double)i, (double)j, xn, yn, r)) return;
+    if (!inside_shape((double)i, (double)j, So)) return;
+    if (inside_shape((double)i, (double)j, Sn)) return;
     const long long x = (long long)j * c.px + i;
     if (owner[x] != p) return;
     owner[x] = OWNER_NONE;
@@ -476,12 +613,14 @@ k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, 
 // another particle has just uncovered.
 // Thread 0 also enters the particle into the repulsion grid of the step that will use this
 // position (k_uncover has zeroed the counts).
+template <bool ELL>
 __global__ void __launch_bounds__(PT)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
         int* __restrict__ cell_items, int* __restrict__ status, const LbmConst c) {
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
-  const double xn = pa.x[buf][p], yn = pa.y[buf][p], r = pa.r[p];
+  const Shape Sn = load_shape<ELL>(pa, buf, p);
+  const double xn = Sn.x, yn = Sn.y;
   if (threadIdx.x == 0) {
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
     ci = min(max(ci, 0), ncx - 1);
@@ -493,12 +632,12 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
   }
   if (!all && pa.fixed[p]) continue;
   const bool sweep = all || pa.ovl[p] != 0;
-  const double xo = pa.x[buf ^ 1][p], yo = pa.y[buf ^ 1][p];
+  const Shape So = load_shape<ELL>(pa, buf ^ 1, p);
   int i0, i1, j0, j1;
-  zone_of(xn, yn, r, i0, i1, j0, j1);
+  zone_shape(Sn, i0, i1, j0, j1);
   for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
-    if (!inside_disc((double)i, (double)j, xn, yn, r)) return;
-    if (!sweep && inside_disc((double)i, (double)j, xo, yo, r)) return;   // already ours
+    if (!inside_shape((double)i, (double)j, Sn)) return;
+    if (!sweep && inside_shape((double)i, (double)j, So)) return;   // already ours
     const long long x = (long long)j * c.px + i;
     if (owner[x] == p) return;
     const int prev = atomicMin(&owner[x], p);
@@ -532,15 +671,15 @@ void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
   const int max_rows = link_rows(h);
-  k_build_links<<<chain_grid(h, h->np, st), LB_T, link_smem(h), st>>>(
-      h->pa.x[which_buffer], h->pa.y[which_buffer], h->pa.r, h->pa.ovl, h->flag, h->owner, h->la,
-      h->np, max_rows, h->status_dev, h->C);
+  (h->n_ell ? k_build_links<true> : k_build_links<false>)<<<chain_grid(h, h->np, st), LB_T, link_smem(h), st>>>(
+      h->pa, which_buffer, h->flag, h->owner, h->la, h->np, max_rows, h->status_dev, h->C);
 }
 
 int particles_configure(lbm* h) {
   const size_t smem = link_smem(h);
   if (smem > 48 * 1024 &&
-      cudaFuncSetAttribute(k_build_links, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      (cudaFuncSetAttribute(k_build_links<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+       cudaFuncSetAttribute(k_build_links<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess))
     return -1;
   return 0;
 }
@@ -548,7 +687,7 @@ int particles_configure(lbm* h) {
 void launch_integrate(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_integrate<<<chain_grid(h, (h->np + IW - 1) / IW, h->chain), IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
+  (h->n_ell ? k_integrate<true> : k_integrate<false>)<<<chain_grid(h, (h->np + IW - 1) / IW, h->chain), IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
                                              h->cell_count, h->cell_items, h->status_dev,
                                              h->newborn_count, h->C);
 }
@@ -556,7 +695,7 @@ void launch_integrate(lbm* h) {
 void launch_uncover(lbm* h) {
   if (h->np == 0) return;
   h->launches++;
-  k_uncover<<<chain_grid(h, h->np, h->chain), PT, 0, h->chain>>>(h->pa, h->cur, h->np, h->flag, h->owner, h->newborn_node,
+  (h->n_ell ? k_uncover<true> : k_uncover<false>)<<<chain_grid(h, h->np, h->chain), PT, 0, h->chain>>>(h->pa, h->cur, h->np, h->flag, h->owner, h->newborn_node,
                                          h->newborn_pid, h->newborn_count, h->newborn_cap,
                                          h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
 }
@@ -566,6 +705,6 @@ void launch_uncover(lbm* h) {
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st) {
   if (h->np == 0) return;
   h->launches++;
-  k_cover<<<chain_grid(h, h->np, st), PT, 0, st>>>(h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
+  (h->n_ell ? k_cover<true> : k_cover<false>)<<<chain_grid(h, h->np, st), PT, 0, st>>>(h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
                                 h->ncx, h->ncy, h->cell_count, h->cell_items, h->status_dev, h->C);
 }

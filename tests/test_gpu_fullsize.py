@@ -219,3 +219,29 @@ def test_config2_whole_run_is_schedule_independent(gpu, wl):
             assert np.array_equal(fa[k][:, fluid], fb[k][:, fluid]), k
     assert all(np.isfinite(v).all() for v in pa.values())
     assert pa["y"].mean() < w.particles["y"].mean() - 50.0      # the suspension has settled a good way
+
+
+def test_settling_ellipse_turns_broadside(gpu, wl):
+    """Qualitative physics of an elliptical particle (the paper's Appendix A shows it as curves
+    only): a 2:1 ellipse released at 60 degrees in a channel four major axes
+    wide, Re about 10, turns its major axis horizontal in a damped oscillation, drifts sideways
+    while it is inclined and returns to the centreline, and reaches a steady settling speed."""
+    p = wl.default_params()
+    p.update(nu=0.02, kappa=0.02, g=2e-5, gbeta=0.0, rep_s=3.0, rep_power=2,
+             wall_T_type=[1, 1, 1, 1], max_particles=1,
+             max_links_per_particle=wl.max_links_for_diameter(40.0))
+    parts = dict(x=np.array([79.5]), y=np.array([1040.0]), diam=np.array([40.0]),
+                 minor=np.array([20.0]), theta=np.array([np.radians(60.0)]),
+                 rho_ratio=np.array([1.1]), T_w=np.array([0.0]))
+    g = gpu.Simulation.from_workload(wl.Workload("ellipse_settling", 160, 1200, p, 1, 1, particles=parts))
+    hist = []
+    for _ in range(30):
+        g.step(4000)
+        q = g.particles()
+        hist.append((q["x"][0], q["y"][0], np.degrees(q["theta"][0]), q["uy"][0]))
+    x, y, th, uy = np.array(hist).T
+    assert np.isfinite(hist).all()
+    assert th[0] < 60.0 and th.min() < -3.0            # turns, and overshoots the horizontal
+    assert np.abs(th[-5:]).max() < 5.0                 # ends broadside
+    assert x.min() < 79.5 - 15.0 and abs(x[-1] - 79.5) < 6.0   # sideways drift, then back
+    assert np.abs(uy[-5:] - uy[-1]).max() < 0.02 * abs(uy[-1]) and uy[-1] < 0.0

@@ -124,6 +124,8 @@ def test_config0_single_hot_particle(gpu, ob, wl):
 def assert_links_after_injection(gpu, ob, wl, w, po):
     parts = dict(w.particles)
     parts.update(x=po["x"], y=po["y"], ux=po["ux"], uy=po["uy"], omega=po["omega"])
+    if "minor" in parts:
+        parts.update(theta=po["theta"])
     w2 = wl.Workload(w.name + "_inj", w.nx, w.ny, w.params, 1, 1, particles=parts)
     try:
         g2, o2 = both(gpu, ob, w2)
@@ -290,6 +292,34 @@ def test_large_particle_wide_zone(gpu, ob, wl):
     w = wl.Workload("large", nx, ny, p, 60, 60, particles=parts)
     g, o, _ = run_and_compare(gpu, ob, w, [1, 60], r_min=6.0)
     assert_links_after_injection(gpu, ob, wl, w, o.particles())
+
+
+def test_elliptical_particles(gpu, ob, wl):
+    """Elliptical particles (App. A) next to
+    circles: different axis ratios and orientations, spinning and translating, one hugging a wall,
+    two within repulsion range of each other, one nearly a circle.  Links (ray-ellipse q) bit-exact
+    at step 0 and on the injected final state; fields and particle states after 1, 2 and 120
+    steps."""
+    nx, ny = 330, 210
+    x = np.array([60.3, 118.0, 200.5, 262.0, 150.2, 24.0, 285.0])
+    y = np.array([70.7, 72.0, 150.0, 60.4, 140.9, 150.0, 170.0])
+    major = np.array([40.0, 24.0, 50.0, 20.0, 30.0, 36.0, 24.0])
+    minor = np.array([20.0, 12.0, 25.0, 20.0, 29.0, 14.0, 16.0])
+    theta = np.radians([60.0, -20.0, 90.0, 0.0, 33.0, 90.0, 10.0])
+    n = len(x)
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=n,
+             max_links_per_particle=wl.max_links_for_diameter(50.0))
+    parts = dict(x=x, y=y, diam=major, minor=minor, theta=theta,
+                 rho_ratio=np.linspace(1.2, 1.8, n), T_w=np.linspace(0.3, 1.0, n),
+                 ux=np.array([0.01, -0.012, 0.0, 0.005, -0.01, 0.0, -0.008]),
+                 uy=np.array([0.0, 0.004, -0.01, 0.01, 0.0, -0.01, 0.0]),
+                 omega=np.array([2e-3, -3e-3, 1e-3, 2e-3, -1e-3, 0.0, 4e-3]))
+    w = wl.Workload("ellipses", nx, ny, p, 120, 120, particles=parts)
+    g, o, _ = run_and_compare(gpu, ob, w, [1, 2, 120], r_min=6.0)
+    assert_links_after_injection(gpu, ob, wl, w, o.particles())
+    th = g.particles()["theta"]
+    assert np.abs(th - theta).max() > 0.05           # they did turn
 
 
 def test_paper_table4_arrangement_small(gpu, ob, wl):

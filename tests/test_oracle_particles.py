@@ -372,3 +372,119 @@ def test_config0_physical_sanity(ob, wl):
     assert F["T"][fl].max() > 0.5 and F["T"][fl].min() > -0.02
     jc, ic = int(round(P["y"][0])), 64
     assert F["T"][jc + 13, ic] > F["T"][jc - 13, ic]                # the warm wake trails above
+
+
+# ------------------------------------------------------------------ elliptical particles
+
+def ellipse_sim(ob, wl, nx, ny, x, y, major, minor, theta, **kw):
+    n = len(x)
+    p = params(wl, n, dmax=float(np.max(major)), **kw)
+    parts = dict(x=np.asarray(x, float), y=np.asarray(y, float), diam=np.asarray(major, float),
+                 minor=np.asarray(minor, float), theta=np.asarray(theta, float),
+                 rho_ratio=np.full(n, 1.5), T_w=np.full(n, 1.0))
+    w = wl.Workload("ell", nx, ny, p, 1, 1, particles=parts)
+    return ob.OracleSim.from_workload(w), w
+
+
+def numpy_ellipse_flags(nx, ny, x, y, major, minor, theta):
+    """Independent rasterisation with the documented operation order: u = dx c + dy s,
+    v = dy c - dx s, (u/a)^2 + (v/b)^2 <= 1 (numpy evaluates each operation separately rounded)."""
+    I, J = np.meshgrid(np.arange(nx, dtype=np.float64), np.arange(ny, dtype=np.float64))
+    flag = np.zeros((ny, nx), dtype=np.uint8)
+    for xc, yc, A, B, th in zip(x, y, major, minor, theta):
+        a, b, c, s = 0.5 * A, 0.5 * B, math.cos(th), math.sin(th)
+        dx, dy = I - xc, J - yc
+        u, v = dx * c + dy * s, dy * c - dx * s
+        ua, vb = u / a, v / b
+        flag |= (ua * ua + vb * vb <= 1.0).astype(np.uint8)
+    return flag
+
+
+def test_ellipse_rasterisation_matches_numpy_and_the_area(ob, wl):
+    x, y = [40.3, 110.7, 170.0], [45.6, 50.2, 48.0]
+    major, minor = [50.0, 30.0, 24.0], [20.0, 29.0, 8.0]
+    theta = np.radians([25.0, -70.0, 90.0])
+    o, _ = ellipse_sim(ob, wl, 210, 100, x, y, major, minor, theta)
+    flag = o.fields()["flag"]
+    assert np.array_equal(flag, numpy_ellipse_flags(210, 100, x, y, major, minor, theta))
+    # lattice points in an ellipse: area pi a b up to a perimeter-sized error
+    for k in range(3):
+        sub = numpy_ellipse_flags(210, 100, x[k:k + 1], y[k:k + 1], major[k:k + 1], minor[k:k + 1],
+                                  theta[k:k + 1])
+        area = math.pi * 0.25 * major[k] * minor[k]
+        assert abs(int(sub.sum()) - area) < 0.5 * (major[k] + minor[k])
+
+
+def test_ray_ellipse_q_closed_forms(ob):
+    """q on the axes of an axis-aligned ellipse is the distance to the vertex; turning the ellipse
+    by 90 degrees swaps the axes; a = b reduces to the circle's q."""
+    a, b = 12.0, 6.0
+    assert abs(ob.link_q_ellipse(-13.0, 0.0, 1, 0.0, 0.0, a, b, 1.0, 0.0) - 1.0) < 1e-12
+    assert abs(ob.link_q_ellipse(-12.5, 0.0, 1, 0.0, 0.0, a, b, 1.0, 0.0) - 0.5) < 1e-12
+    assert abs(ob.link_q_ellipse(0.0, 6.25, 4, 0.0, 0.0, a, b, 1.0, 0.0) - 0.25) < 1e-12
+    assert abs(ob.link_q_ellipse(0.0, 12.75, 4, 0.0, 0.0, a, b, 0.0, 1.0) - 0.75) < 1e-12    # turned
+    # diagonal ray towards a circle written as an ellipse: same as the circle routine
+    for xf, yf, al in ((-8.0, -7.0, 5), (7.5, 7.2, 7), (-7.1, 7.9, 8)):
+        qe = ob.link_q_ellipse(xf, yf, al, 0.3, -0.2, 10.0, 10.0, math.cos(0.7), math.sin(0.7))
+        assert abs(qe - ob.link_q(xf, yf, al, 0.3, -0.2, 10.0)) < 1e-12
+    # a general case against the parametric intersection solved with numpy
+    xc, yc, th = 1.3, -0.4, 0.6
+    c, s = math.cos(th), math.sin(th)
+    xf, yf, al = -9.0, -8.0, 5                        # e5 = (1, 1); its neighbour is inside
+    q = ob.link_q_ellipse(xf, yf, al, xc, yc, a, b, c, s)
+    px, py = xf + q * 1.0 - xc, yf + q * 1.0 - yc
+    u, v = px * c + py * s, py * c - px * s
+    assert 0.0 < q < 1.0 and abs((u / a) ** 2 + (v / b) ** 2 - 1.0) < 1e-12
+
+
+def test_ellipse_zone_scan_equals_bruteforce(ob, wl):
+    x, y = [40.3, 85.0, 130.0], [45.6, 50.2, 48.0]
+    major, minor = [40.0, 30.0, 24.0], [18.0, 29.5, 10.0]
+    theta = np.radians([35.0, -70.0, 80.0])
+    o, _ = ellipse_sim(ob, wl, 170, 100, x, y, major, minor, theta)
+    A, B = sorted_links(o.links()), sorted_links(o.links_bruteforce())
+    assert len(A["q"]) == len(B["q"]) > 300
+    for k in A:
+        assert np.array_equal(A[k], B[k]), k
+    assert (A["q"] >= 0).all() and (A["q"] <= 1).all()
+    # every link's solid end is inside the ellipse and its fluid end outside (numpy predicate)
+    flag = numpy_ellipse_flags(170, 100, x, y, major, minor, theta)
+    assert (flag[A["j"], A["i"]] == 0).all()
+    assert (flag[A["j"] + EY[A["alpha"]], A["i"] + EX[A["alpha"]]] == 1).all()
+
+
+def test_orientation_vector_is_advanced_by_an_exact_rotation(ob):
+    """The Cayley step is a rotation by 2 atan(d/2): the vector stays on the unit circle and n
+    steps compose to the angle n * 2 atan(d/2), which equals n d to O(d^3)."""
+    c, s, d, n = math.cos(0.3), math.sin(0.3), 2.0e-3, 5000
+    for _ in range(n):
+        c, s = ob.rotate_unit(c, s, d)
+    assert abs(c * c + s * s - 1.0) < 1e-15
+    ang = 0.3 + n * 2.0 * math.atan(0.5 * d)
+    assert abs(c - math.cos(ang)) < 1e-12 and abs(s - math.sin(ang)) < 1e-12
+    assert abs(ang - (0.3 + n * d)) < n * d ** 3 / 10.0
+
+
+def test_ellipse_mass_inertia_and_torque_free_spin(ob, wl):
+    """An ellipse in a fluid at rest without gravity: released with a spin, its angular velocity
+    decays (viscous torque opposes it) and its centre stays put by symmetry; a first step under
+    gravity alone moves it by the free-fall increment of a body of area pi a b."""
+    o, w = ellipse_sim(ob, wl, 120, 120, [59.5], [59.5], [40.0], [20.0], [0.4], g=0.0)
+    o.step(1)
+    # gravity: first-step velocity -(1 - 1/ratio) g, independent of the shape (hydro force is zero)
+    p2 = params(wl, 1, dmax=40.0, g=2e-4)
+    parts = dict(x=np.array([59.5]), y=np.array([59.5]), diam=np.array([40.0]), minor=np.array([20.0]),
+                 theta=np.array([0.4]), rho_ratio=np.array([1.5]), T_w=np.array([0.0]))
+    o2 = ob.OracleSim.from_workload(wl.Workload("e", 120, 120, p2, 1, 1, particles=parts))
+    o2.step(1)
+    q = o2.particles()
+    assert abs(q["uy"][0] + (1.0 - 1.0 / 1.5) * 2e-4) < 1e-15 and abs(q["ux"][0]) < 1e-18
+    # spin decay
+    parts.update(omega=np.array([2e-3]))
+    o3 = ob.OracleSim.from_workload(wl.Workload("e", 120, 120, params(wl, 1, dmax=40.0, g=0.0), 1, 1,
+                                                particles=parts))
+    o3.step(300)
+    q = o3.particles()
+    assert 0.0 < q["omega"][0] < 2e-3
+    assert abs(q["x"][0] - 59.5) < 1e-6 and abs(q["y"][0] - 59.5) < 1e-6
+    assert q["theta"][0] > 0.4 + 0.1
