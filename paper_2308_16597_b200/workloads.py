@@ -196,6 +196,38 @@ def paper_table4(cols: int = 80, lines: int = 60, name: str = "paper_table4_4800
                     notes="paper's E4 benchmark; 1750 MLUPS on 1x A100 (Table 5, PAPER.md:273-281)")
 
 
+def paper_table3(name: str = "paper_table3_129_ellipses_1000x2000") -> Workload:
+    """The paper's elliptical-particle case (Table 3): 129 hot
+    elliptical particles, full axes A x B = 50 x 25 l.u., rho_p/rho_f = 1.5, in a 1000 x 2000
+    cavity, nu = 0.01, alpha_T = 0.002 (Pr = 5), g = 9.8e-7, beta = 8.16e-3 per lattice
+    temperature unit (Gr_p = 10), all walls cold; one particle at (0.5 W, 0.75 H) and six rings
+    of 6, 12, 18, 24, 31, 37 particles around it; the paper's repulsion (quadratic, s = 3).
+
+    Readings (the paper shows the cluster only as a picture, Fig. 3a): ring k has radius 60 k l.u.
+    (one major axis plus a 10-unit gap), its particles equally spaced starting on the +x axis,
+    every major axis horizontal."""
+    nx, ny = 1000, 2000
+    cx, cy = 0.5 * nx - 0.5, 0.75 * ny - 0.5
+    xs, ys = [cx], [cy]
+    for k, count in enumerate((6, 12, 18, 24, 31, 37), start=1):
+        ang = 2.0 * math.pi * np.arange(count) / count
+        xs.extend(cx + 60.0 * k * np.cos(ang))
+        ys.extend(cy + 60.0 * k * np.sin(ang))
+    x, y = np.asarray(xs, dtype=np.float64), np.asarray(ys, dtype=np.float64)
+    n = x.shape[0]
+    p = default_params()
+    p.update(nu=0.01, kappa=0.002, rho0=1.0, T0=0.0, g=9.8e-7, gbeta=9.8e-7 * 8.16e-3,
+             rep_s=3.0, rep_eps=1e-3, rep_power=2, max_particles=n,
+             max_links_per_particle=max_links_for_diameter(50.0))
+    p["wall_T_type"] = [1, 1, 1, 1]
+    p["wall_T"] = [0.0, 0.0, 0.0, 0.0]
+    parts = _particle_dict(x, y, np.full(n, 50.0), rho_ratio=1.5, T_w=1.0)
+    parts["minor"] = np.full(n, 25.0)
+    parts["theta"] = np.zeros(n)
+    return Workload(name=name, nx=nx, ny=ny, params=p, steps=100000, parity_steps=20,
+                    particles=parts)
+
+
 def paper_dkt(name: str = "paper_dkt_two_hot_particles_400x1200") -> Workload:
     """Appendix B of the paper (Table 6): draft-kissing-tumbling of
     two hot circular particles in cold fluid.  400 x 1200 l.u., d = 40, rho_p/rho_f = 1.01,

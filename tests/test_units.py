@@ -147,3 +147,28 @@ def test_paper_dkt_workload_matches_table6(wl):
     assert p["nu"] / p["kappa"] == G["t6_Pr"]
     assert abs((P["x"][1] - P["x"][0]) - 0.005 * d) < 1e-12 and P["y"][1] - P["y"][0] == 2 * d
     assert abs(P["x"][1] - (0.5 * w.nx - 0.5)) < 1e-12 and abs(P["y"][0] - (0.8 * w.ny - 0.5)) < 1e-12
+
+
+def test_paper_table3_workload_matches_the_printed_table(wl):
+    """PAPER.md:206-224, Table 3: 129 ellipses of 50 x 25 l.u. in 1000 x 2000, volume fraction
+    6.3 %, Re_p = 31.0, Ar = 24.7, Gr_p = 10, Pr = 5; rings of 6, 12, 18, 24, 31, 37 around one."""
+    import math
+    import numpy as np
+    w = wl.paper_table3()
+    p, P = w.params, w.particles
+    A, B = G["t3_major_lu"], G["t3_minor_lu"]
+    assert (w.nx, w.ny, w.n_particles) == (G["t3_domain_w_lu"], G["t3_domain_h_lu"], G["t3_n_particles"])
+    assert (P["diam"] == A).all() and (P["minor"] == B).all() and (P["rho_ratio"] == G["t3_rho_ratio"]).all()
+    assert (p["nu"], p["kappa"], p["g"]) == (G["t3_nu_lu"], G["t3_alpha_lu"], G["t3_g_lu"])
+    frac = 100.0 * w.n_particles * math.pi * 0.25 * A * B / (w.nx * w.ny)
+    assert round(frac, 1) == G["t3_volume_fraction_percent"]
+    ex = G["t3_rho_ratio"] - 1.0
+    assert round(math.sqrt(p["g"] * A ** 3 * ex) / p["nu"], 1) == G["t3_Ar"]
+    assert round(math.sqrt(p["g"] * math.pi * A * ex / 2.0) * A / p["nu"], 1) == G["t3_Re_p"]
+    assert round(p["gbeta"] * A ** 3 / p["nu"] ** 2) == G["t3_Gr_p"] and p["nu"] / p["kappa"] == G["t3_Pr"]
+    # the cluster: one centre particle and rings of the printed sizes, nobody touching
+    r = np.hypot(P["x"] - P["x"][0], P["y"] - P["y"][0])
+    counts = [int((np.abs(r - 60.0 * k) < 1e-9).sum()) for k in range(1, 7)]
+    assert counts == [6, 12, 18, 24, 31, 37] and abs(P["y"][0] - (0.75 * w.ny - 0.5)) < 1e-12
+    d = np.hypot(P["x"][:, None] - P["x"][None, :], P["y"][:, None] - P["y"][None, :])
+    assert d[np.triu_indices(len(r), 1)].min() > A + 3.0
