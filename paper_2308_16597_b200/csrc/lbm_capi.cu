@@ -21,7 +21,7 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "integrate",
-    "flags_uncover", "flags_cover", "refill", "init_collide", "refill_commit"};
+    "flags_uncover", "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -289,6 +289,7 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   h->stream = (cudaStream_t)cuda_stream;
   carve(h, dev_workspace, nx, ny, p);
   fill_const(h);
+  h->two_step = stream_collide_configure() == 0 ? 1 : 0;
   if (particles_configure(h) != 0) {
     delete h;
     return fail(nullptr, LBM_E_CUDA, "lbm_create: max_links_per_particle needs more shared memory than the device has");
@@ -531,6 +532,14 @@ int lbm_step(lbm_t* h, int nsteps) {
   }
   cudaStream_t S0 = h->stream, S1 = h->chain;
   for (int s = 0; s < nsteps; ++s) {
+    if (h->np == 0 && h->two_step && nsteps - s >= 2) {
+      // particle-free lattice: two time steps per pass over the populations (A -> B)
+      { Timed tm(h, K_STREAM_COLLIDE_2STEP, S0); launch_stream_collide_2step(h); }
+      std::swap(h->A, h->B);
+      h->steps_done += 2;
+      ++s;
+      continue;
+    }
     if (h->np > 0) {
       { Timed tm(h, K_BOUNCE_BACK, S0); launch_bounce_back(h); }
       if (S1 != S0) {
@@ -554,6 +563,12 @@ int lbm_step(lbm_t* h, int nsteps) {
     h->steps_done++;
   }
   return check_status(h);
+}
+
+int lbm_set_two_step(lbm_t* h, int on) {
+  if (!h) return LBM_E_ARG;
+  h->two_step = on ? 1 : 0;
+  return LBM_OK;
 }
 
 int lbm_set_overlap(lbm_t* h, int on) {

@@ -30,7 +30,7 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
-  K_INIT, K_REFILL_COMMIT, K_COUNT
+  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_COUNT
 };
 
 // link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along
@@ -104,6 +104,7 @@ struct lbm {
   int overlap;               // 1: chain runs on `chain_own` concurrently with the lattice kernel
   int chain_ctas;            // CTAs per chain kernel while it runs under the lattice kernel (0 = one per item)
   int sm_count;
+  int two_step;              // particle-free lattice: advance two steps per pass (lbm_set_two_step)
   int links_ready;           // the index array holds the links of the current particle positions
   double *A, *B;             // 14 planes each
   unsigned char* flag;
@@ -140,6 +141,8 @@ struct lbm {
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
 void launch_stream_collide(lbm* h);        // on h->stream
+void launch_stream_collide_2step(lbm* h);  // on h->stream; particle-free lattices only
+int stream_collide_configure();            // kernel attributes (0 = ok)
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
 void launch_set_equilibrium(lbm* h);

@@ -70,6 +70,36 @@ def test_all_wall_types_and_body_force(gpu, ob, wl):
     run_and_compare(gpu, ob, w, [1, 60])
 
 
+def test_two_steps_per_pass_equals_one_step_per_pass_bitwise(gpu, wl):
+    """Particle-free lattices advance two time steps per pass (shared-memory tile).
+    Same arithmetic per step, so every population must equal the one-step kernel's bit for bit:
+    ragged sizes (tiles of 32 x 14 with partial tiles in both directions), every wall type, a
+    body force, and the periodic wrap; odd step counts leave one step to the one-step kernel."""
+    rng = np.random.default_rng(17)
+    cases = []
+    p = wl.default_params()
+    p.update(wall_T_type=[1, 0, 1, 1], wall_T=[0.3, 0.0, 1.0, -0.2], gbeta=2e-4, T0=0.25,
+             body_ax=1e-5, body_ay=-2e-5, nu=0.05, kappa=0.03)
+    cases.append((141, 37, p))
+    cases.append((64, 28, dict(p)))                      # whole tiles exactly
+    q = wl.default_params()
+    q.update(periodic_x=1, body_ax=1e-6, nu=0.1, gbeta=1e-4, wall_T_type=[0, 0, 1, 1], wall_T=[0, 0, 1.0, 0.0])
+    cases.append((77, 45, q))                            # periodic, nx not a multiple of 32
+    cases.append((33, 15, dict(q)))
+    for nx, ny, prm in cases:
+        T = 0.25 + 0.5 * rng.uniform(-1, 1, size=(ny, nx))
+        w = wl.Workload("two_step", nx, ny, prm, 1, 1, T_init=T)
+        a = gpu.Simulation.from_workload(w)
+        b = gpu.Simulation.from_workload(w)
+        b.set_two_step(False)
+        for n in (1, 2, 7, 40):
+            a.step(n)
+            b.step(n)
+            fa, fb = a.fields(populations=True), b.fields(populations=True)
+            for k in ("f", "g", "rho", "ux", "uy", "T"):
+                assert np.array_equal(fa[k], fb[k]), (nx, ny, n, k)
+
+
 def test_periodic_poiseuille(gpu, ob, wl):
     """x-periodic body-force channel (the closed-form check's set-up): wrap-around pulls."""
     p = wl.default_params()
