@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--profile-steps", type=int, default=200)
+    ap.add_argument("--edge", type=int, default=0,
+                    help="config 1 only: particle-free lattice of this edge instead of 1024 "
+                         "(same physics and initial-state recipe)")
     return ap.parse_args()
 
 
@@ -192,6 +195,9 @@ def main():
 
     K, W = args.steps, max(args.warmup, 3)
     w = wl.config(args.config)
+    if args.edge and args.config == 1:
+        w = oracle_sample_workload(wl, 1, args.edge)
+        w.name = f"config1_rayleigh_benard_{args.edge}"
     n = w.nx * w.ny
     stream = torch.cuda.current_stream(dev)
 
