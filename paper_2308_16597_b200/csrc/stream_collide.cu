@@ -152,11 +152,11 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
 // keep the result f+(x, t+1), g+(x, t+1) in shared memory, population-major.  Phase 2: the tile's
 // nodes pull from shared memory (walls as in pull_boundary, on tile-local indices, so the periodic
 // wrap needs no arithmetic), collide again and store f+(x, t+2) to B.  Per two updates a node costs
-// (TB_W+2)(TB_H+2)/(TB_X TB_Y) = 1.45 reads and one write of its 112 B: 137 B per update instead
-// of 224 B; the arithmetic is the one-step kernel's, so the result is the same bit for bit.
-constexpr int TB_X = 32, TB_Y = 14;
+// (TB_W+2)(TB_H+2)/(TB_X TB_Y) = 1.46 reads and one write of its 112 B: 138 B per update instead
+// of 224 B (the halo re-reads hit L2: 111 B of DRAM traffic measured); the arithmetic is the one-step kernel's, so the result is the same bit for bit.
+constexpr int TB_X = 30, TB_Y = 14;   // TB_W = 32: one warp per tile row
 constexpr int TB_W = TB_X + 2, TB_H = TB_Y + 2;
-constexpr int TB_THREADS = TB_W * TB_H;   // 544 = 17 warps
+constexpr int TB_THREADS = TB_W * TB_H;   // 512 = 16 warps
 constexpr int TB_SMEM = 14 * TB_THREADS * (int)sizeof(double);
 
 __global__ void __launch_bounds__(TB_THREADS)
