@@ -180,24 +180,33 @@ k_stream_collide_2step(const double* __restrict__ A, double* __restrict__ B, con
   __syncthreads();
   // phase 2: the tile's own nodes
   if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= c.ny) return;
+  if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
+    // interior: every upstream neighbour is a node of the tile's halo'd image
+    const double* __restrict__ S = s_pop + threadIdx.x;
 #pragma unroll
-  for (int k = 0; k < 9; ++k) {
-    const int si = i - ex_of(k), sj = j - ey_of(k);
-    bool in = (sj >= 0 && sj < c.ny);
-    if ((si < 0 || si >= c.nx) && !c.periodic_x) in = false;
-    f[k] = in ? s_pop[k * TB_THREADS + (ty - ey_of(k)) * TB_W + (tx - ex_of(k))]
-              : s_pop[opp_of(k) * TB_THREADS + threadIdx.x];
-  }
+    for (int k = 0; k < 9; ++k) f[k] = S[k * TB_THREADS - ey_of(k) * TB_W - ex_of(k)];
 #pragma unroll
-  for (int k = 0; k < 5; ++k) {
-    const int si = i - ex_of(k), sj = j - ey_of(k);
-    bool in = (sj >= 0 && sj < c.ny);
-    int wall = sj < 0 ? 2 : 3;
-    if ((si < 0 || si >= c.nx) && !c.periodic_x) { in = false; wall = si < 0 ? 0 : 1; }
-    if (in) g[k] = s_pop[(9 + k) * TB_THREADS + (ty - ey_of(k)) * TB_W + (tx - ex_of(k))];
-    else {
-      const double gb = s_pop[(9 + opp_of(k)) * TB_THREADS + threadIdx.x];
-      g[k] = c.wall_type[wall] == 1 ? (2.0 * c.wT * c.wall_T[wall] - gb) : gb;
+    for (int k = 0; k < 5; ++k) g[k] = S[(9 + k) * TB_THREADS - ey_of(k) * TB_W - ex_of(k)];
+  } else {
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+      const int si = i - ex_of(k), sj = j - ey_of(k);
+      bool in = (sj >= 0 && sj < c.ny);
+      if ((si < 0 || si >= c.nx) && !c.periodic_x) in = false;
+      f[k] = in ? s_pop[k * TB_THREADS + (ty - ey_of(k)) * TB_W + (tx - ex_of(k))]
+                : s_pop[opp_of(k) * TB_THREADS + threadIdx.x];
+    }
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const int si = i - ex_of(k), sj = j - ey_of(k);
+      bool in = (sj >= 0 && sj < c.ny);
+      int wall = sj < 0 ? 2 : 3;
+      if ((si < 0 || si >= c.nx) && !c.periodic_x) { in = false; wall = si < 0 ? 0 : 1; }
+      if (in) g[k] = s_pop[(9 + k) * TB_THREADS + (ty - ey_of(k)) * TB_W + (tx - ex_of(k))];
+      else {
+        const double gb = s_pop[(9 + opp_of(k)) * TB_THREADS + threadIdx.x];
+        g[k] = c.wall_type[wall] == 1 ? (2.0 * c.wT * c.wall_T[wall] - gb) : gb;
+      }
     }
   }
   mrt_collide(f, g, c);
