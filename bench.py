@@ -271,6 +271,8 @@ def main():
                 "share_of_sequential_step": seq[kname] / step_ms_seq if step_ms_seq else None,
                 "kernel_ms_per_step_sequential": seq, "kernel_ms_per_step_overlapped": ovl,
                 "whole_step_frac_of_hbm_roofline": value / world / (peak * 1e9 / BYTES_PER_LU / 1e6),
+                # north_star words the roofline as "about 8 TB/s" (nominal): 35,714 MLUPS
+                "whole_step_frac_of_nominal_8TBs_roofline": value / world / (8.0e12 / BYTES_PER_LU / 1e6),
                 "fluid_fraction": n_fluid / n}
     sim.close()
     del sim
