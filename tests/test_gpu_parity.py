@@ -441,6 +441,27 @@ def test_error_codes(gpu, wl):
         s.set_temperature(np.zeros((64, 64)))
     assert e.value.code == gpu.LBM_E_STATE
     assert len(s.particles()["x"]) == 1
+    # ellipses: a turned ellipse whose bounding box leaves the cavity, one whose support-function
+    # gap to a circle is negative, and a major axis too long for the link capacity
+    p3 = wl.default_params()
+    p3.update(max_particles=3, max_links_per_particle=wl.max_links_for_diameter(30.0))
+    s3 = gpu.Simulation(96, 64, p3)
+    ell = dict(rho_ratio=np.array([1.5]), T_w=np.array([1.0]))
+    with pytest.raises(gpu.LbmError) as e:      # vertical 30 x 10 ellipse at y = 14: hy = 15 > 14.5
+        s3.add_particles(x=np.array([40.0]), y=np.array([14.0]), diam=np.array([30.0]),
+                         minor=np.array([10.0]), theta=np.array([np.pi / 2]), **ell)
+    assert e.value.code == gpu.LBM_E_ARG
+    s3.add_particles(x=np.array([40.0]), y=np.array([14.0]), diam=np.array([30.0]),
+                     minor=np.array([10.0]), theta=np.array([0.0]), **ell)      # horizontal: fits
+    with pytest.raises(gpu.LbmError) as e:      # circle of d = 20 at distance 22 along x: 15 + 10 > 22
+        s3.add_particles(x=np.array([62.0]), y=np.array([14.0]), diam=np.array([20.0]), **ell)
+    assert e.value.code == gpu.LBM_E_ARG
+    s3.add_particles(x=np.array([40.0]), y=np.array([31.0]), diam=np.array([20.0]), **ell)   # above: 5 + 10 < 17
+    with pytest.raises(gpu.LbmError) as e:
+        s3.add_particles(x=np.array([70.0]), y=np.array([40.0]), diam=np.array([44.0]),
+                         minor=np.array([8.0]), theta=np.array([0.0]), **ell)
+    assert e.value.code == gpu.LBM_E_CAPACITY
+    assert len(s3.particles()["x"]) == 2 and len(s3.links()["q"]) > 0
     # no particles at all: empty link list, empty particle arrays
     s2 = gpu.Simulation(32, 32, wl.default_params())
     assert len(s2.links()["q"]) == 0 and len(s2.particles()["x"]) == 0
