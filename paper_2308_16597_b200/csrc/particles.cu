@@ -4,13 +4,18 @@
 // is taken with separately rounded fp64 operations, the same way the paper-order CPU oracle does,
 // so link lists are bit-exact ("Hard parts").
 //
-// a2  PAPER.md:250-258  per-step collection of (i, j, alpha) into a fixed index array: one CTA
-//     per particle scans the particle's effective zone [INT(xc-r)-1, INT(xc+r)+1]^2 and compacts
-//     the links into the particle's segment with popc + warp-shuffle scan + block prefix.
-// a5  PAPER.md:88-97, 142-147  Eqs. (7), (8), (15): one thread per particle; neighbours through
-//     a uniform cell grid (cell edge >= d_max + s), visited in ascending particle id so that the
+// a2  PAPER.md:250-258  per-step collection of (i, j, alpha) into a fixed index array: a CTA per
+//     particle enumerates the ring of candidate nodes of the particle's effective zone
+//     [INT(xc-r)-1, INT(xc+r)+1]^2 row by row and compacts the links into the particle's segment
+//     with popc + a packed warp-shuffle scan + block prefix.
+// a5  PAPER.md:88-97, 142-147  Eqs. (7), (8), (15): one warp per particle; neighbours through
+//     a uniform cell grid (cell edge >= d_max + s), added in ascending particle id so that the
 //     sum order is fixed.
 // a6  PAPER.md:151  "a solid node may be uncovered by the particle and become a fluid node".
+// Shapes: circles, and ellipses through the Shape helpers below; the kernels
+// are templated on whether the simulation holds an ellipse at all.  All four kernels loop over
+// the particles (grid-size agnostic): under the lattice kernel they run as a few persistent CTAs
+// per SM.
 #include "lbm_internal.cuh"
 
 namespace {
