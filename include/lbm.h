@@ -122,6 +122,17 @@ int lbm_step(lbm_t* h, int nsteps);
  * per-kernel timing and by the tests). */
 int lbm_set_overlap(lbm_t* h, int on);
 
+/* on = 1 (default; the environment variable LBM_GRAPH=0 turns the default off): lbm_step replays
+ * whole periods of the step schedule as CUDA graphs -- 8 time steps per graph launch while that
+ * many remain, then 2, an odd last step launched directly -- instead of issuing every kernel,
+ * event record and stream wait from the host (the single-GPU analogue of the paper's async(n)
+ * work queues).  The graph is captured on streams the library owns (the fork /
+ * join onto the particle-chain stream becomes graph edges) and launched into the handle's stream,
+ * so the caller's ordering is unchanged; the kernels, their arguments and their order are those of
+ * on = 0, hence the same results bit for bit.  Event profiling (lbm_profile_enable) always uses
+ * direct launches. */
+int lbm_set_graph(lbm_t* h, int on);
+
 /* on = 1 (default): while no particle has been added, lbm_step advances the lattice two time steps
  * per pass over the populations (shared-memory tile with a one-node halo; about 137 B instead of
  * 224 B of HBM traffic per lattice update), an odd last step through the one-step kernel.  The

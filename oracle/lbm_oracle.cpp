@@ -91,6 +91,8 @@ struct oracle_lbm {
   std::vector<double> fnew, gnew;   /* f(.,t+1), g(.,t+1) */
   std::vector<int> owner;           /* -1 fluid, else id of the (lowest-numbered) covering particle */
   std::vector<Particle> parts;
+  bool have_post = false;           /* fpost/gpost were injected (oracle_set_state): the next step
+                                       starts at "collect links", its collision is already done */
   long long steps_done = 0;
   std::string err;
 };
@@ -262,7 +264,9 @@ int step_once(oracle_lbm* h) {
   const double wT = (4.0 + aT) / 20.0; /* thermal weight of directions 1..4 (reading) */
 
   /* 1-3: macroscopic + collision of f and g on fluid nodes (Eqs. 5, 6) */
-  for (int j = 0; j < ny; ++j)
+  const bool injected = h->have_post;
+  h->have_post = false;
+  for (int j = 0; j < ny && !injected; ++j)
     for (int i = 0; i < nx; ++i) {
       long long x = IDX(h, i, j);
       if (h->owner[x] >= 0) continue;
@@ -470,12 +474,7 @@ int step_once(oracle_lbm* h) {
       /* outward normal of the wall at the newborn node: radial for a circle; for an
        * ellipse the gradient of (u/a)^2 + (v/b)^2 turned back into the lattice frame */
       double nrx = dxn, nry = dyn;
-      if (a.ell) {
-        double u = dxn * a.c + dyn * a.s, v = dyn * a.c - dxn * a.s;
-        double gu = (u / a.a) / a.a, gv = (v / a.b) / a.b;
-        nrx = gu * a.c - gv * a.s;
-        nry = gu * a.s + gv * a.c;
-      }
+      if (a.ell) oracle_ellipse_normal(dxn, dyn, a.a, a.b, a.c, a.s, &nrx, &nry);
       int c = oracle_refill_direction(nrx, nry);
       int nvalid = 0;
       long long xs[3] = {-1, -1, -1};
@@ -805,6 +804,18 @@ extern "C" int oracle_refill_direction(double nx_, double ny_) {
   return best;
 }
 
+/* Outward normal (not normalised) of an ellipse at the point (dx, dy) relative to its centre:
+ * the gradient of (u/a)^2 + (v/b)^2, u = dx c + dy s, v = dy c - dx s, turned back into the
+ * lattice frame.  The "n" of PAPER.md:151 for an elliptical particle (reading, DESIGN.md
+ * "Elliptical particles"); for a = b it is parallel to (dx, dy). */
+extern "C" void oracle_ellipse_normal(double dx, double dy, double a, double b, double c, double s,
+                                      double* nx_, double* ny_) {
+  double u = dx * c + dy * s, v = dy * c - dx * s;
+  double gu = (u / a) / a, gv = (v / b) / b;
+  *nx_ = gu * c - gv * s;
+  *ny_ = gu * s + gv * c;
+}
+
 /* Eq. (16) f_new = 3 f(1) - 3 f(2) + f(3); fallback (reading): 2 nodes -> 2 f(1) - f(2);
  * 1 node -> f(1); 0 nodes -> f_eq(rho0, u_w).  Then the MRT velocity constraint:
  * m = M f_new, j = rho_new u_w with rho_new = sum f_new, f_new = M^-1 m. */
@@ -1008,6 +1019,38 @@ extern "C" int oracle_get_fields(oracle_lbm_t* h, double* rho, double* ux, doubl
           for (int k = 0; k < 5; ++k) g[k * n + x] = go[k];
       }
     }
+  return 0;
+}
+
+/* Test infrastructure of the deep-run parity check: replaces the whole state by one taken from
+ * elsewhere (the CUDA path's read-out after many steps): POST-collision populations f+(x,t),
+ * g+(x,t) on the fluid nodes -- what lbm_get_fields hands out -- and the particle states; the
+ * solid map is rasterised from the positions.  The next oracle_step then starts after the
+ * collision ("collect links" onwards).  Circles only keep their exact geometry; an
+ * ellipse's orientation vector is re-derived from theta. */
+extern "C" int oracle_set_state(oracle_lbm_t* h, const double* fpost, const double* gpost, int n,
+                                const double* x, const double* y, const double* theta,
+                                const double* ux, const double* uy, const double* omega) {
+  if (!h || !fpost || !gpost) return E_ARG;
+  if (n != (int)h->parts.size()) return fail(h, E_ARG, "set_state: particle count differs");
+  std::memcpy(h->fpost.data(), fpost, sizeof(double) * 9 * (size_t)h->n);
+  std::memcpy(h->gpost.data(), gpost, sizeof(double) * 5 * (size_t)h->n);
+  for (int k = 0; k < n; ++k) {
+    Particle& a = h->parts[k];
+    a.x = x[k];
+    a.y = y[k];
+    a.theta = theta[k];
+    a.ux = ux[k];
+    a.uy = uy[k];
+    a.omega = omega[k];
+    if (a.ell) {
+      a.c = std::cos(a.theta);
+      a.s = std::sin(a.theta);
+    }
+  }
+  compute_owner(h, h->owner);
+  h->have_post = true;
+  if (h->steps_done == 0) h->steps_done = 1; /* no more set-up calls after this */
   return 0;
 }
 

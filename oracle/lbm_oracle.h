@@ -60,6 +60,12 @@ int  oracle_get_links_bruteforce(oracle_lbm_t* h, long long* n, int* pid, int* i
                                  int* alpha, double* q);
 /* pre-collision populations f(x,t), g(x,t) (the oracle's own state), 9n and 5n doubles */
 int  oracle_get_precollision(oracle_lbm_t* h, double* f, double* g);
+/* deep-run parity check: inject post-collision populations (9n, 5n doubles, population-major) and
+ * particle states taken from elsewhere; the next oracle_step starts after the collision.  Until
+ * that step has run, oracle_get_fields / oracle_get_precollision still show the old state. */
+int  oracle_set_state(oracle_lbm_t* h, const double* fpost, const double* gpost, int n,
+                      const double* x, const double* y, const double* theta,
+                      const double* ux, const double* uy, const double* omega);
 int  oracle_destroy(oracle_lbm_t* h);
 const char* oracle_last_error(const oracle_lbm_t* h);
 
@@ -95,6 +101,10 @@ double oracle_repulsion_mag(double C, double eps, double s, double delta, int po
 void   oracle_integrate(double* state6, double Fx, double Fy, double Tz, double mass,
                         double inertia);
 int    oracle_refill_direction(double nx_, double ny_);                     /* e_c */
+/* outward normal (not normalised) of an ellipse (semi-axes a, b, orientation (c, s)) at the point
+ * (dx, dy) relative to its centre: the n of PAPER.md:151 for an elliptical particle */
+void   oracle_ellipse_normal(double dx, double dy, double a, double b, double c, double s,
+                             double* nx_, double* ny_);
 /* Eq. (16) + fallback ladder + MRT momentum constraint */
 void   oracle_refill_f(int nvalid, const double* f1, const double* f2, const double* f3,
                        double rho0, double uwx, double uwy, double* out9);

@@ -76,6 +76,9 @@ def lib():
         L.oracle_momentum_exchange.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double,
                                                C.c_double, C.c_double, C.c_double, _dp]
         L.oracle_refill_f.argtypes = [C.c_int, _dp, _dp, _dp, C.c_double, C.c_double, C.c_double, _dp]
+        L.oracle_ellipse_normal.restype = None
+        L.oracle_ellipse_normal.argtypes = [C.c_double] * 6 + [_dp, _dp]
+        L.oracle_set_state.argtypes = [C.c_void_p, _dp, _dp, C.c_int] + [_dp] * 6
     return _lib
 
 
@@ -194,6 +197,12 @@ def refill_direction(nx_, ny_):
     return lib().oracle_refill_direction(nx_, ny_)
 
 
+def ellipse_normal(dx, dy, a, b, c, s):
+    nx_, ny_ = C.c_double(), C.c_double()
+    lib().oracle_ellipse_normal(dx, dy, a, b, c, s, C.byref(nx_), C.byref(ny_))
+    return nx_.value, ny_.value
+
+
 def refill_f(nvalid, f1, f2, f3, rho0, uwx, uwy):
     f1 = np.ascontiguousarray(f1, dtype=np.float64)
     f2 = np.ascontiguousarray(f2, dtype=np.float64)
@@ -284,6 +293,17 @@ class OracleSim:
             res["f"] = f.reshape(9, self.ny, self.nx)
             res["g"] = g.reshape(5, self.ny, self.nx)
         return res
+
+    def set_state(self, f_post, g_post, particles):
+        """Inject post-collision populations (9, ny, nx), (5, ny, nx) and a particle-state dict
+        (x, y, theta, ux, uy, omega); the next step() starts after the collision."""
+        f = np.ascontiguousarray(f_post, dtype=np.float64).reshape(-1)
+        g = np.ascontiguousarray(g_post, dtype=np.float64).reshape(-1)
+        assert f.size == 9 * self.n and g.size == 5 * self.n
+        P = {k: np.ascontiguousarray(particles[k], dtype=np.float64)
+             for k in ("x", "y", "theta", "ux", "uy", "omega")}
+        self._chk(lib().oracle_set_state(self._h, _d(f), _d(g), int(P["x"].size),
+                                         *[_d(P[k]) for k in ("x", "y", "theta", "ux", "uy", "omega")]))
 
     def precollision(self):
         f, g = _arr(9 * self.n), _arr(5 * self.n)

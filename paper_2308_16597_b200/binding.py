@@ -76,6 +76,7 @@ def load_library():
     L.lbm_step.argtypes = [vp, C.c_int]
     L.lbm_set_overlap.argtypes = [vp, C.c_int]
     L.lbm_set_two_step.argtypes = [vp, C.c_int]
+    L.lbm_set_graph.argtypes = [vp, C.c_int]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
     L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
@@ -92,7 +93,7 @@ def load_library():
     for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_add_ellipses", "lbm_step",
                  "lbm_get_fields", "lbm_get_particles", "lbm_get_links", "lbm_profile_enable",
                  "lbm_profile_kernels", "lbm_profile_get", "lbm_destroy", "lbm_set_overlap",
-                 "lbm_set_two_step"):
+                 "lbm_set_two_step", "lbm_set_graph"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -193,6 +194,9 @@ class Simulation:
 
     def set_overlap(self, on=True):
         self._chk(self._L.lbm_set_overlap(self._h, 1 if on else 0))
+
+    def set_graph(self, on=True):
+        self._chk(self._L.lbm_set_graph(self._h, 1 if on else 0))
 
     def set_two_step(self, on=True):
         self._chk(self._L.lbm_set_two_step(self._h, 1 if on else 0))

@@ -37,7 +37,10 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
 }
 
 __global__ void __launch_bounds__(BT, 8)
-k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, const LbmConst c) {
+k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, int early,
+              const LbmConst c) {
+  if (early) pdl_launch_dependents();
+  pdl_wait();   // the previous step's refill commit (and, through it, everything before)
   const int p = blockIdx.x;
   const int n = la.count[p];
   const long long base = (long long)p * la.cap;
@@ -172,7 +175,7 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
 constexpr int RW = 8;   // warps (newborn nodes) per CTA
 __global__ void __launch_bounds__(RW * 32)
 k_refill(const double* __restrict__ A, double* __restrict__ stash,
-         const unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
+         const unsigned char* __restrict__ flag, int* __restrict__ nb_node,
          const int* __restrict__ nb_pid, const int* __restrict__ nb_count, int nb_cap,
          ParticleArrays pa, int cur, const LbmConst c) {
   const unsigned FULL = 0xffffffffu;
@@ -180,7 +183,10 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
   const int n = min(*nb_count, nb_cap);
   for (int e = blockIdx.x * RW + (threadIdx.x >> 5); e < n; e += gridDim.x * RW) {
     const int x = nb_node[e];
-    if (flag[x] != 2) continue;   // covered again by another particle in the same step
+    if (flag[x] != 2) {           // covered again by another particle in the same step:
+      if (lane == 0) nb_node[e] = -1;   // the commit kernel skips the entry without a flag load
+      continue;
+    }
     const int p = nb_pid[e];
     const int i = x % c.px, j = x / c.px;
     // state at t+1 (cur already points at the new buffer)
@@ -274,54 +280,54 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
 
 // After the lattice kernel: the refilled populations go into B and the newborn nodes become
 // ordinary fluid nodes.  16 threads per list entry (one per population, two idle), all in one warp.
+// Entries whose node was covered again in the same step were marked -1 by k_refill.  Also zeroes
+// the OTHER newborn counter, the one the next step's k_move appends to.
 __global__ void k_refill_commit(double* __restrict__ B, const double* __restrict__ stash,
                                 unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
-                                const int* __restrict__ nb_count, int nb_cap, const LbmConst c) {
+                                const int* __restrict__ nb_count, int* __restrict__ nb_count_next,
+                                int nb_cap, int early, const LbmConst c) {
+  if (early) pdl_launch_dependents();
+  pdl_wait();
+  if (blockIdx.x == 0 && threadIdx.x == 0) *nb_count_next = 0;
   const int n = min(*nb_count, nb_cap);
   const long long total = (long long)n * 16;
-  const int lane = threadIdx.x & 31;
-  for (long long t0 = (long long)blockIdx.x * blockDim.x + (threadIdx.x - lane); t0 < total;
-       t0 += (long long)gridDim.x * blockDim.x) {        // warp-uniform trip count
-    const long long t = t0 + lane;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
     const int e = (int)(t >> 4), k = (int)(t & 15);
-    int x = 0;
-    bool live = false;
-    if (e < n) {
-      x = nb_node[e];
-      live = flag[x] == 2;   // else covered again by another particle in the same step
-    }
-    __syncwarp();            // every thread of the entry has read the flag before it is cleared
-    if (live) {
-      if (k < 9) B[f_at(k, x, c.ps)] = stash[(long long)e * 14 + k];
-      else if (k < 14) B[g_at(k - 9, x, c.ps)] = stash[(long long)e * 14 + k];
-      else if (k == 15) flag[x] = 0;
-    }
+    const int x = nb_node[e];
+    if (x < 0) continue;
+    if (k < 9) B[f_at(k, x, c.ps)] = stash[(long long)e * 14 + k];
+    else if (k < 14) B[g_at(k - 9, x, c.ps)] = stash[(long long)e * 14 + k];
+    else if (k == 15) flag[x] = 0;
   }
 }
 
 } // namespace
 
-void launch_bounce_back(lbm* h) {
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
-  k_bounce_back<<<h->np, BT, 0, h->stream>>>(h->A, h->la, h->pa, h->cur, h->C);
+  launch_k(k_bounce_back, dim3(h->np), dim3(BT), 0, st, pdl, h->A, h->la, h->pa, h->cur,
+           h->chain_ctas > 0 ? 0 : 1, h->C);
 }
 
+// newborn list of the step whose particle buffer index is h->cur (called before cur is flipped)
 void launch_refill(lbm* h, cudaStream_t st) {
   if (h->np == 0) return;
   int blocks = (h->np + RW - 1) / RW;   // a handful of newborn nodes per particle and step
   if (blocks > 1184) blocks = 1184;
-  if (st == h->chain_own && h->chain_ctas > 0 && blocks > h->chain_ctas / 2) blocks = h->chain_ctas / 2;
+  if (st != h->stream && h->chain_ctas > 0 && blocks > h->chain_ctas / 2) blocks = h->chain_ctas / 2;
   h->launches++;
   k_refill<<<blocks, RW * 32, 0, st>>>(h->A, h->stash, h->flag, h->newborn_node, h->newborn_pid,
-                                        h->newborn_count, h->newborn_cap, h->pa, h->cur ^ 1, h->C);
+                                        h->newborn_count + h->cur, h->newborn_cap, h->pa, h->cur ^ 1, h->C);
 }
 
-void launch_refill_commit(lbm* h) {
+void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   int blocks = (h->np * 16 + 255) / 256;
   if (blocks > 1184) blocks = 1184;
   h->launches++;
-  k_refill_commit<<<blocks, 256, 0, h->stream>>>(h->B, h->stash, h->flag, h->newborn_node,
-                                                  h->newborn_count, h->newborn_cap, h->C);
+  launch_k(k_refill_commit, dim3(blocks), dim3(256), 0, st, pdl, h->B, (const double*)h->stash, h->flag,
+           (const int*)h->newborn_node, (const int*)(h->newborn_count + step_parity),
+           h->newborn_count + (step_parity ^ 1), h->newborn_cap, h->chain_ctas > 0 ? 0 : 1, h->C);
 }

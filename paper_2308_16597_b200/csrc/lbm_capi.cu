@@ -20,8 +20,8 @@ namespace {
 char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
-    "stream_collide", "build_links", "bounce_back_force", "integrate",
-    "flags_uncover", "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step"};
+    "stream_collide", "build_links", "bounce_back_force", "integrate_uncover",
+    "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -39,6 +39,19 @@ int fail(lbm* h, int code, const char* fmt, ...) {
   } while (0)
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+constexpr int LBM_GRAPH_STEPS = 8;   // time steps per graph launch (an even number: one or more periods)
+
+// Every entry point runs on the device the handle was created on, whatever device is current in
+// the calling thread, and leaves the caller's choice as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(const lbm* h) {
+    if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->device) cudaSetDevice(h->device);
+    else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 // Lays the arrays out in the workspace.  With base == nullptr only the size is computed.
 struct Carver {
@@ -110,11 +123,15 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   la.q = c.take<double>(nl);
   la.count = c.take<int>(np);
   la.cap = p->max_links_per_particle;
-  int* cell_count = c.take<int>((size_t)L.max_cells);
-  int* cell_items = c.take<int>((size_t)L.max_cells * CELL_CAP);
+  int* cell_count[2];
+  int* cell_items[2];
+  for (int b = 0; b < 2; ++b) {
+    cell_count[b] = c.take<int>((size_t)L.max_cells);
+    cell_items[b] = c.take<int>((size_t)L.max_cells * CELL_CAP);
+  }
   int* nb_node = c.take<int>((size_t)L.newborn_cap);
   int* nb_pid = c.take<int>((size_t)L.newborn_cap);
-  int* nb_count = c.take<int>(1);
+  int* nb_count = c.take<int>(2);
   double* stash = c.take<double>((size_t)L.newborn_cap * 14);
   int* status = c.take<int>(1);
   if (h) {
@@ -126,8 +143,10 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
     h->owner = owner;
     h->pa = pa;
     h->la = la;
-    h->cell_count = cell_count;
-    h->cell_items = cell_items;
+    for (int b = 0; b < 2; ++b) {
+      h->cell_count[b] = cell_count[b];
+      h->cell_items[b] = cell_items[b];
+    }
     h->max_cells = L.max_cells;
     h->newborn_node = nb_node;
     h->newborn_pid = nb_pid;
@@ -203,7 +222,6 @@ struct Timed {
 };
 
 int check_status(lbm* h) {
-  if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
   CUDA_OK(h, cudaMemcpyAsync(h->status_host, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
@@ -245,7 +263,7 @@ void prime(lbm* h) {
 // links of the current positions (the first step's; afterwards every step builds the next one's)
 void ensure_links(lbm* h) {
   if (h->links_ready || h->np == 0) return;
-  launch_build_links(h, h->cur, h->stream);
+  launch_build_links(h, h->cur, h->stream, false);
   h->links_ready = 1;
 }
 
@@ -289,7 +307,9 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   h->stream = (cudaStream_t)cuda_stream;
   carve(h, dev_workspace, nx, ny, p);
   fill_const(h);
-  h->two_step = stream_collide_configure() == 0 ? 1 : 0;
+  cudaGetDevice(&h->device);
+  h->two_step_ok = stream_collide_configure() == 0 ? 1 : 0;
+  h->two_step = h->two_step_ok;
   if (particles_configure(h) != 0) {
     delete h;
     return fail(nullptr, LBM_E_CUDA, "lbm_create: max_links_per_particle needs more shared memory than the device has");
@@ -300,25 +320,40 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     delete h;
     return LBM_E_CUDA;
   }
-  // second stream for the particle update chain: highest priority, so
-  // that its short latency-bound kernels get SM slots as CTAs of the lattice kernel retire
+  // streams of the step schedule: the serial chain of small kernels
+  // (bounce-back, particle update, flags, links, refill commit) on a stream of the highest
+  // priority, so that its latency-bound kernels get SM slots as CTAs of the lattice kernel retire;
+  // the refill on a third stream beside the link builder; the lattice kernel on the caller's stream
   h->chain = h->stream;
+  h->side = h->stream;
   {
     int lo = 0, hi = 0;
     cudaDeviceGetStreamPriorityRange(&lo, &hi);
-    if (cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
-        cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
-        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) == cudaSuccess) {
+    h->chain_priority = hi;
+    bool ok = cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
+              cudaStreamCreateWithPriority(&h->side_own, cudaStreamNonBlocking, hi) == cudaSuccess;
+    cudaEvent_t* evs[6] = {&h->ev_in, &h->ev_out, &h->ev_bb, &h->ev_sc, &h->ev_cov, &h->ev_ref};
+    for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+    if (ok) {
       h->overlap = 1;
       h->chain = h->chain_own;
+      h->side = h->side_own;
     } else {
       cudaGetLastError();
       h->chain_own = nullptr;
     }
   }
+  if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) == cudaSuccess) {
+    const char* e = getenv("LBM_GRAPH");
+    h->use_graph = (e && atoi(e) == 0) ? 0 : 1;
+    const char* e2 = getenv("LBM_PDL");
+    h->use_pdl = (e2 && atoi(e2) == 0) ? 0 : 1;
+  } else {
+    cudaGetLastError();
+    h->cap_stream = nullptr;
+  }
   {
-    int dev = 0;
-    cudaGetDevice(&dev);
+    const int dev = h->device;
     cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (h->sm_count <= 0) h->sm_count = 148;
     h->chain_ctas = 0;   // set by add_particles (size_chain)
@@ -328,8 +363,9 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   cudaMemsetAsync(h->flag, 0, nn, h->stream);
   cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
   cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
-  cudaMemsetAsync(h->newborn_count, 0, sizeof(int), h->stream);
-  if (h->max_cells) cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->max_cells, h->stream);
+  cudaMemsetAsync(h->newborn_count, 0, 2 * sizeof(int), h->stream);
+  for (int b = 0; b < 2; ++b)
+    if (h->max_cells) cudaMemsetAsync(h->cell_count[b], 0, sizeof(int) * (size_t)h->max_cells, h->stream);
   cudaMemsetAsync(h->B, 0, sizeof(double) * 14 * (size_t)h->ps, h->stream);
   launch_set_equilibrium(h);
   e = cudaStreamSynchronize(h->stream);
@@ -347,6 +383,7 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
 int lbm_set_temperature(lbm_t* h, const double* T_host) {
   if (!h || !T_host) return h ? fail(h, LBM_E_ARG, "set_temperature: NULL") : LBM_E_ARG;
   if (h->primed) return fail(h, LBM_E_STATE, "set_temperature after the first step");
+  DeviceGuard dg(h);
   // B is scratch until the first step writes it
   const size_t n = (size_t)h->nx * h->ny;
   CUDA_OK(h, cudaMemcpyAsync(h->B, T_host, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -366,6 +403,7 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
   if (n < 0 || (n > 0 && (!x || !y || !diam || !rho_ratio || !T_w)))
     return fail(h, LBM_E_ARG, "add_particles: NULL array or negative count");
   if (h->primed) return fail(h, LBM_E_STATE, "add_particles after the first step");
+  DeviceGuard dg(h);
   if (n == 0) return LBM_OK;
   if ((long long)h->np + n > h->P.max_particles)
     return fail(h, LBM_E_CAPACITY, "add_particles: max_particles (%d) exceeded", h->P.max_particles);
@@ -493,8 +531,8 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
   if ((long long)h->ncx * h->ncy > h->max_cells)
     return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
   // flag and owner maps and the repulsion grid of step 0 (primed == 0: every particle, full sweep)
-  CUDA_OK(h, cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->max_cells, h->stream));
-  launch_cover(h, c, h->stream);
+  CUDA_OK(h, cudaMemsetAsync(h->cell_count[c], 0, sizeof(int) * (size_t)h->max_cells, h->stream));
+  launch_cover(h, c, h->stream, false);
   h->links_ready = 0;
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
@@ -515,74 +553,232 @@ int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const do
   return add_shapes(h, n, x, y, major, minor, theta, rho_ratio, T_w, ux, uy, omega, fixed);
 }
 
+// While a graph is being captured: remember the node the last launch on a chain stream became
+// (the stream's only capture dependency), so that it can be given the chain's priority afterwards.
+static void note_chain_node(lbm* h, cudaStream_t S1) {
+  if (!h->cap_nodes) return;
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  const cudaGraphNode_t* deps = nullptr;
+  size_t ndeps = 0;
+  if (cudaStreamGetCaptureInfo(S1, &st, nullptr, nullptr, &deps, &ndeps) == cudaSuccess &&
+      st == cudaStreamCaptureStatusActive && ndeps == 1)
+    static_cast<std::vector<cudaGraphNode_t>*>(h->cap_nodes)->push_back(deps[0]);
+}
+
 // Step schedule: the resident state A is f+(x,t), g+(x,t), the index array holds
-// the links of x_p(t).
-//   S0: bounce-back + momentum exchange (parks f_ibar(x_f,t+1) in solid slots of A, sums F, T_z)
-//   S1:   after it: integrate -> uncover -> cover -> refill (A -> stash)    } concurrent with
-//                    -> links of x_p(t+1)                                    } each other
-//   S0: fused pull-stream-collide A -> B over every node fluid at t          }
-//   S0: after both: refill commit (stash -> B at the uncovered nodes, newborn flags cleared)
-// Only the lattice kernel, the bounce-back kernel and the refill are on the critical path.
+// the links of x_p(t).  Three streams, S0 = the caller's (or the capturing) stream:
+//   S1: bounce-back + momentum exchange (parks f_ibar(x_f,t+1) in solid slots of A, sums F, T_z)
+//   S0:   after it: fused pull-stream-collide A -> B over every node fluid at t
+//   S1: integrate + uncover -> cover -> links of x_p(t+1)        } concurrent with the
+//   S2:                        after cover: refill (A -> stash)   } lattice kernel
+//   S1: after the lattice kernel and the refill: refill commit (stash -> B, newborn flags cleared)
+// S1 is one dependent chain from step to step (the next bounce-back follows the commit), each link
+// a programmatic dependent launch.  The caller's stream is joined to it at both ends of a call.
+// Enqueues ONE time step (the streams may be capturing) and flips the host-side phase (A/B, cur).
+static void enqueue_step(lbm* h) {
+  cudaStream_t S0 = h->stream, S1 = h->chain, S2 = h->side;
+  const bool fork = S1 != S0;
+  const bool pdl = h->use_pdl != 0;
+  const int sp = h->cur;   // step parity: which newborn counter / repulsion grid this step uses
+  if (h->np > 0) {
+    { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h, S1, pdl); }
+    note_chain_node(h, S1);
+    if (fork) {
+      cudaEventRecord(h->ev_bb, S1);
+      cudaStreamWaitEvent(S0, h->ev_bb, 0);
+    }
+  }
+  if (fork || h->np == 0) {
+    Timed tm(h, K_STREAM_COLLIDE, S0);
+    launch_stream_collide(h);
+  }
+  if (h->np > 0) {
+    if (fork) cudaEventRecord(h->ev_sc, S0);
+    { Timed tm(h, K_MOVE, S1); launch_move(h, S1, pdl); }
+    note_chain_node(h, S1);
+    { Timed tm(h, K_COVER, S1); launch_cover(h, sp ^ 1, S1, pdl); }
+    note_chain_node(h, S1);
+    if (fork) {
+      cudaEventRecord(h->ev_cov, S1);
+      cudaStreamWaitEvent(S2, h->ev_cov, 0);
+    }
+    { Timed tm(h, K_REFILL, S2); launch_refill(h, S2); }
+    note_chain_node(h, S2);
+    if (fork) cudaEventRecord(h->ev_ref, S2);
+    { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h, sp ^ 1, S1, pdl && fork); }
+    note_chain_node(h, S1);
+    h->cur ^= 1;
+    if (fork) {
+      cudaStreamWaitEvent(S1, h->ev_sc, 0);
+      cudaStreamWaitEvent(S1, h->ev_ref, 0);
+    } else {
+      Timed tm(h, K_STREAM_COLLIDE, S0);
+      launch_stream_collide(h);
+    }
+    { Timed tm(h, K_REFILL_COMMIT, S1); launch_refill_commit(h, sp, S1, pdl); }
+    note_chain_node(h, S1);
+  }
+  std::swap(h->A, h->B);
+}
+
+// Both ends of a run of steps: the chain stream starts after everything already on the caller's
+// stream, and the caller's stream continues after the last refill commit.
+static void join_in(lbm* h) {
+  if (h->np == 0 || h->chain == h->stream) return;
+  cudaEventRecord(h->ev_in, h->stream);
+  cudaStreamWaitEvent(h->chain, h->ev_in, 0);
+}
+static void join_out(lbm* h) {
+  if (h->np == 0 || h->chain == h->stream) return;
+  cudaEventRecord(h->ev_out, h->chain);
+  cudaStreamWaitEvent(h->stream, h->ev_out, 0);
+}
+
+static void drop_graphs(lbm* h) {
+  for (int k = 0; k < h->n_graphs; ++k) cudaGraphExecDestroy(h->graphs[k].exec);
+  h->n_graphs = 0;
+}
+
+// The graph of `steps` (even) time steps starting in the handle's current phase: looked up, or
+// captured now.  Capture runs on the library's own stream pair (the caller's stream may be the
+// legacy default stream, which cannot capture); the fork / join events turn into graph edges.
+// Returns nullptr if capture is not possible (the caller then launches directly).
+static lbm::StepGraph* step_graph(lbm* h, int steps) {
+  for (int k = 0; k < h->n_graphs; ++k) {
+    lbm::StepGraph& g = h->graphs[k];
+    if (g.A == h->A && g.cur == h->cur && g.steps == steps && g.overlap == h->overlap &&
+        g.chain_ctas == h->chain_ctas)
+      return &g;
+  }
+  if (h->n_graphs == LBM_MAX_GRAPHS) drop_graphs(h);
+  cudaStream_t user = h->stream, chain = h->chain;
+  double *A0 = h->A, *B0 = h->B;
+  const int cur0 = h->cur;
+  const long long l0 = h->launches;
+  cudaStream_t side = h->side;
+  h->stream = h->cap_stream;
+  if (chain == user) h->chain = h->side = h->cap_stream;
+  cudaGraph_t graph = nullptr;
+  std::vector<cudaGraphNode_t> chain_nodes;
+  cudaError_t e = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeRelaxed);
+  if (e == cudaSuccess) {
+    if (h->chain != h->stream) h->cap_nodes = &chain_nodes;
+    join_in(h);
+    for (int s = 0; s < steps; ++s) enqueue_step(h);
+    join_out(h);
+    h->cap_nodes = nullptr;
+    e = cudaStreamEndCapture(h->cap_stream, &graph);
+  }
+  // The chain's kernel nodes get the chain stream's priority explicitly: without it the chain
+  // would start in the lattice kernel's tail.
+  if (e == cudaSuccess)
+    for (cudaGraphNode_t nd : chain_nodes) {
+      cudaGraphNodeType ty;
+      if (cudaGraphNodeGetType(nd, &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+      cudaLaunchAttributeValue v;
+      std::memset(&v, 0, sizeof v);
+      v.priority = h->chain_priority;
+      cudaGraphKernelNodeSetAttribute(nd, cudaLaunchAttributePriority, &v);
+    }
+  cudaGetLastError();
+  const long long per = h->launches - l0;
+  h->launches = l0;
+  h->stream = user;
+  h->chain = chain;
+  h->side = side;
+  h->A = A0;
+  h->B = B0;
+  h->cur = cur0;
+  cudaGraphExec_t exec = nullptr;
+  // per-node priorities are honoured only on request (otherwise every node runs at the priority
+  // of the stream the graph is launched into)
+  if (e == cudaSuccess) e = cudaGraphInstantiateWithFlags(&exec, graph, cudaGraphInstantiateFlagUseNodePriority);
+  if (graph) cudaGraphDestroy(graph);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    h->use_graph = 0;   // not available here: direct launches from now on
+    return nullptr;
+  }
+  lbm::StepGraph& g = h->graphs[h->n_graphs++];
+  g.exec = exec;
+  g.A = h->A;
+  g.cur = h->cur;
+  g.steps = steps;
+  g.overlap = h->overlap;
+  g.chain_ctas = h->chain_ctas;
+  g.launches = per;
+  return &g;
+}
+
 int lbm_step(lbm_t* h, int nsteps) {
   if (!h) return LBM_E_ARG;
   if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
+  DeviceGuard dg(h);
   if (nsteps > 0) {
     prime(h);
     ensure_links(h);
   }
-  cudaStream_t S0 = h->stream, S1 = h->chain;
-  for (int s = 0; s < nsteps; ++s) {
+  int s = 0;
+  // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
+  // launch while that many remain, then 2), the odd last step directly; event profiling needs
+  // the direct launches
+  if (h->np > 0 && h->use_graph && !h->prof_on) {
+    while (nsteps - s >= 2) {
+      const int unit = nsteps - s >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : 2;
+      lbm::StepGraph* g = step_graph(h, unit);
+      if (!g) break;
+      CUDA_OK(h, cudaGraphLaunch(g->exec, h->stream));
+      h->launches += g->launches;
+      h->steps_done += unit;
+      s += unit;
+    }
+  }
+  if (s < nsteps) join_in(h);
+  const bool direct = s < nsteps;
+  for (; s < nsteps; ++s) {
     if (h->np == 0 && h->two_step && nsteps - s >= 2) {
       // particle-free lattice: two time steps per pass over the populations (A -> B)
-      { Timed tm(h, K_STREAM_COLLIDE_2STEP, S0); launch_stream_collide_2step(h); }
+      { Timed tm(h, K_STREAM_COLLIDE_2STEP, h->stream); launch_stream_collide_2step(h); }
       std::swap(h->A, h->B);
       h->steps_done += 2;
       ++s;
       continue;
     }
-    if (h->np > 0) {
-      { Timed tm(h, K_BOUNCE_BACK, S0); launch_bounce_back(h); }
-      if (S1 != S0) {
-        cudaEventRecord(h->ev_fork, S0);
-        cudaStreamWaitEvent(S1, h->ev_fork, 0);
-      }
-      { Timed tm(h, K_INTEGRATE, S1); launch_integrate(h); }
-      { Timed tm(h, K_UNCOVER, S1); launch_uncover(h); }
-      { Timed tm(h, K_COVER, S1); launch_cover(h, h->cur ^ 1, S1); }
-      { Timed tm(h, K_REFILL, S1); launch_refill(h, S1); }
-      { Timed tm(h, K_BUILD_LINKS, S1); launch_build_links(h, h->cur ^ 1, S1); }
-      h->cur ^= 1;
-      if (S1 != S0) cudaEventRecord(h->ev_join, S1);
-    }
-    { Timed tm(h, K_STREAM_COLLIDE, S0); launch_stream_collide(h); }
-    if (h->np > 0) {
-      if (S1 != S0) cudaStreamWaitEvent(S0, h->ev_join, 0);
-      { Timed tm(h, K_REFILL_COMMIT, S0); launch_refill_commit(h); }
-    }
-    std::swap(h->A, h->B);
+    enqueue_step(h);
     h->steps_done++;
   }
+  if (direct) join_out(h);
   return check_status(h);
+}
+
+int lbm_set_graph(lbm_t* h, int on) {
+  if (!h) return LBM_E_ARG;
+  h->use_graph = (on && h->cap_stream) ? 1 : 0;
+  return LBM_OK;
 }
 
 int lbm_set_two_step(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
-  h->two_step = on ? 1 : 0;
+  h->two_step = (on && h->two_step_ok) ? 1 : 0;
   return LBM_OK;
 }
 
 int lbm_set_overlap(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
+  DeviceGuard dg(h);
   cudaStreamSynchronize(h->stream);
   if (h->chain_own) cudaStreamSynchronize(h->chain_own);
+  if (h->side_own) cudaStreamSynchronize(h->side_own);
   h->overlap = (on && h->chain_own) ? 1 : 0;
   h->chain = h->overlap ? h->chain_own : h->stream;
+  h->side = h->overlap ? h->side_own : h->stream;
   return LBM_OK;
 }
 
 int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, double* f, double* g,
                    unsigned char* flag) {
   if (!h) return LBM_E_ARG;
+  DeviceGuard dg(h);
   const size_t n = (size_t)h->nx * h->ny;
   if (rho || ux || uy || T) {
     // B is dead between steps: use four of its planes as dense scratch
@@ -619,6 +815,7 @@ int lbm_get_particles(lbm_t* h, int* n, double* x, double* y, double* theta, dou
   if (!h || !n) return h ? fail(h, LBM_E_ARG, "get_particles: n is NULL") : LBM_E_ARG;
   *n = h->np;
   if (h->np == 0) return LBM_OK;
+  DeviceGuard dg(h);
   const int c = h->cur;
   const size_t b = (size_t)h->np * sizeof(double);
   auto down = [&](double* dst, const double* src) {
@@ -642,6 +839,7 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
   const long long capacity = *n;
   *n = 0;
   if (h->np == 0) return LBM_OK;
+  DeviceGuard dg(h);
   ensure_links(h);
   std::vector<int> count(h->np);
   CUDA_OK(h, cudaMemcpyAsync(count.data(), h->la.count, h->np * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -674,6 +872,7 @@ int lbm_get_links(lbm_t* h, long long* n, int* pid, int* i, int* j, int* alpha, 
 
 int lbm_profile_enable(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
+  DeviceGuard dg(h);
   if (on) {
     for (int k = 0; k < K_COUNT; ++k) {
       if (!h->ev0[k]) {
@@ -699,8 +898,10 @@ const char* lbm_profile_kernel_name(int kernel_id) {
 
 int lbm_profile_get(lbm_t* h, int kernel_id, double* total_ms, long long* launches) {
   if (!h || kernel_id < 0 || kernel_id >= K_COUNT) return LBM_E_ARG;
+  DeviceGuard dg(h);
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   if (h->chain != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->chain));
+  if (h->side != h->stream) CUDA_OK(h, cudaStreamSynchronize(h->side));
   double tot = 0.0;
   const int n = h->ev0[kernel_id] ? h->ev_n[kernel_id] : 0;
   for (int s = 0; s < n; ++s) {
@@ -717,12 +918,16 @@ long long lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : -1; }
 
 int lbm_destroy(lbm_t* h) {
   if (!h) return LBM_OK;
+  DeviceGuard dg(h);
   cudaStreamSynchronize(h->stream);
+  drop_graphs(h);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   if (h->chain_own) {
     cudaStreamSynchronize(h->chain_own);
     cudaStreamDestroy(h->chain_own);
-    cudaEventDestroy(h->ev_fork);
-    cudaEventDestroy(h->ev_join);
+    if (h->side_own) cudaStreamDestroy(h->side_own);
+    cudaEvent_t evs[6] = {h->ev_in, h->ev_out, h->ev_bb, h->ev_sc, h->ev_cov, h->ev_ref};
+    for (cudaEvent_t e : evs) cudaEventDestroy(e);
   }
   for (int k = 0; k < K_COUNT; ++k)
     if (h->ev0[k]) {

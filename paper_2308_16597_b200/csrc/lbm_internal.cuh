@@ -21,6 +21,7 @@
 #define CELL_CAP 32          // particle centres per repulsion-grid cell
 #define MIN_CELL 16.0        // smallest repulsion-grid cell edge (workspace is sized for it)
 #define NEWBORN_PER_PARTICLE 32
+#define LBM_MAX_GRAPHS 8
 
 // status bits written by kernels, read once per lbm_step call
 #define ST_NONFINITE 1
@@ -29,7 +30,7 @@
 #define ST_NEWBORN_OVERFLOW 8
 
 enum {
-  K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_INTEGRATE, K_UNCOVER, K_COVER, K_REFILL,
+  K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_MOVE, K_COVER, K_REFILL,
   K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_COUNT
 };
 
@@ -39,14 +40,6 @@ enum {
 // bounce-back kernel needs no dependent flag loads.
 #define LINK_DIR_MASK 0x0f
 #define LINK_BEHIND_SHIFT 4
-
-// effective zone of PAPER.md:258 (the narrower reading of DESIGN.md): [INT(xc-r)-1, INT(xc+r)+1]^2
-__device__ __forceinline__ void zone_of(double xc, double yc, double r, int& i0, int& i1, int& j0, int& j1) {
-  i0 = (int)floor(__dsub_rn(xc, r)) - 1;
-  i1 = (int)floor(__dadd_rn(xc, r)) + 1;
-  j0 = (int)floor(__dsub_rn(yc, r)) - 1;
-  j1 = (int)floor(__dadd_rn(yc, r)) + 1;
-}
 
 // double index of f_k / g_k of node x inside one copy of the populations
 __host__ __device__ __forceinline__ long long f_at(int k, long long x, long long ps) {
@@ -98,9 +91,11 @@ struct lbm {
   lbm_params P;
   LbmConst C;
   cudaStream_t stream;       // the caller's stream: bounce-back, lattice kernel, refill, set-up, read-out
-  cudaStream_t chain;        // particle update chain (integrator, flags, next step's links)
+  cudaStream_t chain;        // the serial chain: bounce-back, particle update, flags, links, refill commit
+  cudaStream_t side;         // refill (beside the link builder)
   cudaStream_t chain_own;    // the stream we created (NULL if creation failed)
-  cudaEvent_t ev_fork, ev_join;
+  cudaStream_t side_own;     // refill runs here, beside the link builder
+  cudaEvent_t ev_in, ev_out, ev_bb, ev_sc, ev_cov, ev_ref;
   int overlap;               // 1: chain runs on `chain_own` concurrently with the lattice kernel
   int chain_ctas;            // CTAs per chain kernel while it runs under the lattice kernel (0 = one per item)
   int sm_count;
@@ -115,14 +110,14 @@ struct lbm {
   int np;                    // particles added
   int n_ell;                 // of which ellipses (a != b): selects the kernel instantiations
   double d_max;              // largest diameter (sizes the repulsion grid)
-  int* cell_count;
-  int* cell_items;
+  int* cell_count[2];        // repulsion grid, double-buffered by the particle buffer index
+  int* cell_items[2];
   int ncx, ncy;
   double cell;               // cell edge
   int max_cells;
   int* newborn_node;
   int* newborn_pid;
-  int* newborn_count;
+  int* newborn_count;        // two counters, [step parity = cur at the start of the step]
   double* stash;             // 14 refilled populations per newborn-list entry
   int newborn_cap;
   int* status_dev;
@@ -130,6 +125,24 @@ struct lbm {
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
   long long steps_done;
   long long launches;        // kernels launched (lbm_kernel_launches)
+  int device;                // the device the handle was created on (every entry point selects it)
+  int two_step_ok;           // the two-step kernel's attributes could be set
+  // CUDA graphs: a period of the schedule -- an even number of steps,
+  // after which A/B and the particle buffer index are back where they started -- is captured once
+  // per (phase, length, schedule) and replayed; the fork/join onto the chain stream is part of
+  // the capture.  The single-GPU analogue of the paper's async(n) queues.
+  int use_graph;
+  int use_pdl;               // programmatic dependent launch along the chain (LBM_PDL=0 turns it off)
+  cudaStream_t cap_stream;   // capture happens here (the caller's stream may be the legacy stream)
+  void* cap_nodes;           // during capture: std::vector<cudaGraphNode_t>* of the chain's kernel nodes
+  int chain_priority;        // priority of the chain stream, given to those nodes
+  struct StepGraph {
+    cudaGraphExec_t exec;
+    const double* A;         // phase the graph was captured in
+    int cur, steps, overlap, chain_ctas;
+    long long launches;      // kernels per replay
+  } graphs[LBM_MAX_GRAPHS];
+  int n_graphs;
   // profiling
   int prof_on;
   cudaEvent_t* ev0[K_COUNT];
@@ -137,6 +150,33 @@ struct lbm {
   int ev_n[K_COUNT];
   char err[512];
 };
+
+// ---- programmatic dependent launch (PDL).  Every kernel of the step's serial chain starts with
+// pdl_wait(): launched with the programmatic-serialisation attribute it may begin while its
+// predecessor in the stream still runs, and this is where it waits for that kernel to have
+// completed and flushed; launched normally the instruction returns at once.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+#ifdef __CUDACC__
+#include <utility>
+// <<<grid, block, smem, st>>> with the PDL attribute on request
+template <typename... KArgs, typename... Args>
+inline void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                     bool pdl, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+#endif
 
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
@@ -149,12 +189,13 @@ void launch_set_equilibrium(lbm* h);
 void launch_export(lbm* h, double* f_dense, double* g_dense);    // dense f[9][n], g[5][n], device
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
 // particles.cu (compiled with -fmad=false)
-void launch_build_links(lbm* h, int which_buffer, cudaStream_t st);
-void launch_integrate(lbm* h);             // on h->chain
+// `pdl`: launch with the programmatic-serialisation attribute (the kernel then waits for its
+// predecessor in `st` itself, see pdl_wait)
+void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
+void launch_move(lbm* h, cudaStream_t st, bool pdl);   // integrator + uncover, buffer cur -> cur ^ 1
 int particles_configure(lbm* h);           // per-handle kernel attributes (0 = ok)
-void launch_uncover(lbm* h);               // on h->chain
-void launch_cover(lbm* h, int which_buffer, cudaStream_t st);
+void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
 // bounce_back.cu
-void launch_bounce_back(lbm* h);            // on h->stream
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl);
 void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped
-void launch_refill_commit(lbm* h);          // on h->stream: stash -> B, newborn flags cleared
+void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl);  // stash -> B, newborn flags cleared

@@ -166,7 +166,9 @@ template <bool ELL>
 __global__ void __launch_bounds__(LB_T)
 k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag,
               const int* __restrict__ owner, LinkArrays la, int np, int max_rows,
-              int* __restrict__ status, const LbmConst c) {
+              int* __restrict__ status, int early, const LbmConst c) {
+  if (early) pdl_launch_dependents();
+  pdl_wait();
   extern __shared__ int s_node[];                           // la.cap packed nodes, la.cap dir bytes,
   unsigned char* s_dir = (unsigned char*)(s_node + la.cap); // then the row tables
   int* s_off = s_node + la.cap + (la.cap + 3) / 4;          // max_rows + 1: candidates before row t
@@ -416,23 +418,20 @@ __device__ __forceinline__ double repulsion_mag(double C, const LbmConst& c, dou
 // U' = U + F/M, x' = x + (U + U')/2 (DESIGN.md reading), same for Omega, theta.
 // One WARP per particle: the lanes fetch the candidates of the 3 x 3 cell neighbourhood in
 // parallel (one round of dependent loads instead of a serial walk), each lane evaluates one pair,
-// and the non-zero contributions are added in ascending particle id (warp min-reduction picks the
-// next one), so the sum order is fixed whatever order the cell slots were filled in.
-constexpr int IW = 4;   // warps (particles) per CTA
+// the non-zero contributions of all batches are collected and then added in ascending particle id
+// (warp min-reduction picks the next one), so the sum order is fixed whatever order the cell slots
+// were filled in and however many candidates the nine cells hold.
+// Called by warp 0 of the particle's CTA (k_move); s_cid / s_cfx / s_cfy: 32 entries each.
 template <bool ELL>
-__global__ void __launch_bounds__(IW * 32)
-k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
-            const int* __restrict__ cell_count, const int* __restrict__ cell_items,
-            int* __restrict__ status, int* __restrict__ nb_count, const LbmConst c) {
+__device__ __forceinline__ void integrate_particle(const ParticleArrays& pa, int cur, int ia, double cell,
+                                                   int ncx, int ncy, const int* __restrict__ cell_count,
+                                                   const int* __restrict__ cell_items,
+                                                   int* __restrict__ status, const LbmConst& c,
+                                                   int* s_cid, double* s_cfx, double* s_cfy) {
   const int lane = threadIdx.x & 31;
-  // the newborn list of the previous step has been consumed (refill, then the bounce-back kernel
-  // of this step cleared its flags; both precede this kernel)
-  if (blockIdx.x == 0 && threadIdx.x == 0) *nb_count = 0;
   const unsigned FULL = 0xffffffffu;
   const int nxt = cur ^ 1;
   const double PI = 3.14159265358979323846;
-  // grid-size agnostic: warp w of the grid takes particles w, w + (warps in the grid), ...
-  for (int ia = blockIdx.x * IW + (threadIdx.x >> 5); ia < np; ia += gridDim.x * IW) {
   const Shape SA = load_shape<ELL>(pa, cur, ia);
   const double ax = SA.x, ay = SA.y, ar = SA.r, ratio = pa.rho_ratio[ia];
   const double Ca = PI * SA.a * SA.b * (ratio * c.rho0 - c.rho0) * c.g;   // area pi a b
@@ -457,6 +456,7 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
     if (lane >= d) incl += v;
   }
   const int total = __shfl_sync(FULL, incl, 8);
+  int ncontrib = 0;
   for (int base = 0; base < total; base += 32) {
     const int k = base + lane;   // candidate number k lives in the cell whose prefix range holds it
     int id = 0x7fffffff;
@@ -495,8 +495,32 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
         }
       }
     }
-    // contributions of this batch in ascending id (batches themselves are rare beyond the first:
-    // 32 candidates already cover 9 cells of edge >= d_max + s)
+    // the non-zero contributions are parked in the warp's shared list (batch after batch, in slot
+    // order); the sum itself waits until every batch has been seen
+    const unsigned hm = __ballot_sync(FULL, has);
+    if (has) {
+      const int slot = ncontrib + __popc(hm & ((1u << lane) - 1u));
+      if (slot < 32) {
+        s_cid[slot] = id;
+        s_cfx[slot] = fx;
+        s_cfy[slot] = fy;
+      }
+    }
+    ncontrib += __popc(hm);
+  }
+  // Sum in ascending particle id over ALL neighbours, whatever batch or cell slot they came from
+  // (the slot order is the atomicAdd order of k_cover and varies from run to run): the oracle's
+  // order, and the same bits on every run.  A disc has at most a handful of neighbours within the
+  // repulsion range; more than 32 is reported as a capacity error.
+  if (ncontrib > 32) {
+    if (lane == 0) atomicOr(status, ST_CELL_OVERFLOW);
+    ncontrib = 32;
+  }
+  __syncwarp();
+  if (ncontrib > 0) {
+    bool has = lane < ncontrib;
+    const int id = has ? s_cid[lane] : 0x7fffffff;
+    const double fx = has ? s_cfx[lane] : 0.0, fy = has ? s_cfy[lane] : 0.0;
     while (__any_sync(FULL, has)) {
       const int m = __reduce_min_sync(FULL, has ? id : 0x7fffffff);
       const int src = __ffs(__ballot_sync(FULL, has && id == m)) - 1;
@@ -505,7 +529,7 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
       if (lane == src) has = false;
     }
   }
-  if (lane != 0) continue;
+  if (lane != 0) return;
   double ahx, ahy;
   half_extents(SA, ahx, ahy);
   if (!c.periodic_x) {
@@ -556,7 +580,6 @@ k_integrate(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   pa.omega[nxt][ia] = om;
   if (!(isfinite(x) && isfinite(y) && isfinite(th) && isfinite(ux) && isfinite(uy) && isfinite(om)))
     atomicOr(status, ST_NONFINITE);
-  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -572,18 +595,35 @@ __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const L
   }
 }
 
-// Phase A: nodes owned by p that the disc at its NEW position no longer covers become newborn
-// candidates (flag 2, owner NONE) and are appended to the newborn list.
+// a5 + first half of a6 in ONE kernel, one CTA per particle (grid-size agnostic): warp 0 integrates
+// the particle (it needs only the OLD positions of its neighbours, the repulsion grid of this step
+// and the particle's own force), then the whole CTA sweeps the particle's old zone:
+// Phase A of the flag update: nodes owned by p that the disc at its NEW position no longer covers
+// become newborn candidates (flag 2, owner NONE) and are appended to the newborn list.
+// The repulsion grid and the newborn counter are double-buffered by the particle buffer index, so
+// that nothing this kernel resets is still being read inside it: it zeroes the grid of buffer
+// cur ^ 1 (last read by the previous step's integration; k_cover of this step refills it with the
+// new positions) and appends to the newborn counter of this step (zeroed by the previous step's
+// k_refill_commit).
 template <bool ELL>
 __global__ void __launch_bounds__(PT)
-k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, int* __restrict__ owner,
-          int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
-          int* __restrict__ status, int* __restrict__ cell_count, int ncells, const LbmConst c) {
-  // the repulsion grid of this step has been consumed by k_integrate: zero it; k_cover refills it
-  // with the new positions for the next step
-  for (int k = blockIdx.x * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count[k] = 0;
+k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
+       const int* __restrict__ cell_count_cur, const int* __restrict__ cell_items_cur,
+       int* __restrict__ cell_count_nxt, int ncells,
+       unsigned char* __restrict__ flag, int* __restrict__ owner,
+       int* __restrict__ nb_node, int* __restrict__ nb_pid, int* __restrict__ nb_count, int nb_cap,
+       int* __restrict__ status, int early, const LbmConst c) {
+  __shared__ int s_cid[32];
+  __shared__ double s_cfx[32], s_cfy[32];
+  if (early) pdl_launch_dependents();
+  pdl_wait();
+  for (int k = blockIdx.x * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count_nxt[k] = 0;
   const int nxt = cur ^ 1;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
+  if (threadIdx.x < 32)
+    integrate_particle<ELL>(pa, cur, p, cell, ncx, ncy, cell_count_cur, cell_items_cur, status, c,
+                            s_cid, s_cfx, s_cfy);
+  __syncthreads();   // the new state (global memory, written by lane 0) is visible to the CTA
   if (pa.fixed[p]) continue;
   const Shape So = load_shape<ELL>(pa, cur, p), Sn = load_shape<ELL>(pa, nxt, p);
   int i0, i1, j0, j1;
@@ -617,12 +657,14 @@ k_uncover(ParticleArrays pa, int cur, int np, unsigned char* __restrict__ flag, 
 // (and every particle at set-up, `all` = 1) sweeps its whole disc, which also re-claims nodes
 // another particle has just uncovered.
 // Thread 0 also enters the particle into the repulsion grid of the step that will use this
-// position (k_uncover has zeroed the counts).
+// position (the grid of buffer `buf`; k_move has zeroed its counts).
 template <bool ELL>
 __global__ void __launch_bounds__(PT)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
-        int* __restrict__ cell_items, int* __restrict__ status, const LbmConst c) {
+        int* __restrict__ cell_items, int* __restrict__ status, int early, const LbmConst c) {
+  if (early) pdl_launch_dependents();
+  pdl_wait();
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const Shape Sn = load_shape<ELL>(pa, buf, p);
   const double xn = Sn.x, yn = Sn.y;
@@ -665,6 +707,14 @@ static int chain_grid(const lbm* h, int items, cudaStream_t st) {
   return items;
 }
 
+// Programmatic dependent launch along the chain: a kernel that is NOT throttled (few particles,
+// the launch-latency-bound case) lets its successor's CTAs come up at once -- they wait in
+// griddepcontrol.wait -- so that only the kernel bodies remain on the critical path.  A throttled
+// chain (large lattices) does not: waiting CTAs would hold SM slots the lattice kernel needs.
+static int chain_early(const lbm* h, cudaStream_t st) {
+  return (st == h->chain_own && h->chain_ctas > 0) ? 0 : 1;
+}
+
 // rows of the largest effective zone the capacity admits (12N - 12 <= cap) and the
 // dynamic shared memory of the link builder: the compacted list + four row tables
 static int link_rows(const lbm* h) { return (h->la.cap + 12) / 12 + 2; }
@@ -672,44 +722,51 @@ static size_t link_smem(const lbm* h) {
   return ((size_t)h->la.cap + ((size_t)h->la.cap + 3) / 4 + 4 * (size_t)link_rows(h) + 4) * sizeof(int);
 }
 
-void launch_build_links(lbm* h, int which_buffer, cudaStream_t st) {
+void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
   const int max_rows = link_rows(h);
-  (h->n_ell ? k_build_links<true> : k_build_links<false>)<<<chain_grid(h, h->np, st), LB_T, link_smem(h), st>>>(
-      h->pa, which_buffer, h->flag, h->owner, h->la, h->np, max_rows, h->status_dev, h->C);
+  launch_k(h->n_ell ? k_build_links<true> : k_build_links<false>, dim3(chain_grid(h, h->np, st)), dim3(LB_T),
+           link_smem(h), st, pdl, h->pa, which_buffer, (const unsigned char*)h->flag, (const int*)h->owner,
+           h->la, h->np, max_rows, h->status_dev, chain_early(h, st), h->C);
 }
 
+// The dynamic shared memory limit of the link builder is a per-function (per-device) attribute:
+// it is only ever raised, to the largest need any live handle on this device has had, so a later
+// handle with a smaller index array cannot take it away from an earlier one.
 int particles_configure(lbm* h) {
+  static size_t raised[64] = {0};
   const size_t smem = link_smem(h);
-  if (smem > 48 * 1024 &&
-      (cudaFuncSetAttribute(k_build_links<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-       cudaFuncSetAttribute(k_build_links<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess))
+  const int dev = (h->device >= 0 && h->device < 64) ? h->device : 0;
+  if (smem <= 48 * 1024 || smem <= raised[dev]) return 0;
+  if (cudaFuncSetAttribute(k_build_links<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_build_links<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    cudaGetLastError();
     return -1;
+  }
+  raised[dev] = smem;
   return 0;
 }
 
-void launch_integrate(lbm* h) {
+// integrator + phase A of the flag update for the particle buffer h->cur -> h->cur ^ 1
+void launch_move(lbm* h, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
-  (h->n_ell ? k_integrate<true> : k_integrate<false>)<<<chain_grid(h, (h->np + IW - 1) / IW, h->chain), IW * 32, 0, h->chain>>>(h->pa, h->cur, h->np, h->cell, h->ncx, h->ncy,
-                                             h->cell_count, h->cell_items, h->status_dev,
-                                             h->newborn_count, h->C);
-}
-
-void launch_uncover(lbm* h) {
-  if (h->np == 0) return;
-  h->launches++;
-  (h->n_ell ? k_uncover<true> : k_uncover<false>)<<<chain_grid(h, h->np, h->chain), PT, 0, h->chain>>>(h->pa, h->cur, h->np, h->flag, h->owner, h->newborn_node,
-                                         h->newborn_pid, h->newborn_count, h->newborn_cap,
-                                         h->status_dev, h->cell_count, h->ncx * h->ncy, h->C);
+  const int c = h->cur;
+  launch_k(h->n_ell ? k_move<true> : k_move<false>, dim3(chain_grid(h, h->np, st)), dim3(PT), 0, st, pdl,
+           h->pa, c, h->np, h->cell, h->ncx, h->ncy, (const int*)h->cell_count[c],
+           (const int*)h->cell_items[c], h->cell_count[c ^ 1], h->ncx * h->ncy, h->flag, h->owner,
+           h->newborn_node, h->newborn_pid, h->newborn_count + c, h->newborn_cap, h->status_dev,
+           chain_early(h, st), h->C);
 }
 
 // after add_particles every particle (fixed ones too) is rasterised with a full sweep; during
 // stepping the fixed ones never move
-void launch_cover(lbm* h, int which_buffer, cudaStream_t st) {
+void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
-  (h->n_ell ? k_cover<true> : k_cover<false>)<<<chain_grid(h, h->np, st), PT, 0, st>>>(h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell,
-                                h->ncx, h->ncy, h->cell_count, h->cell_items, h->status_dev, h->C);
+  launch_k(h->n_ell ? k_cover<true> : k_cover<false>, dim3(chain_grid(h, h->np, st)), dim3(PT), 0, st, pdl,
+           h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell, h->ncx, h->ncy,
+           h->cell_count[which_buffer], h->cell_items[which_buffer], h->status_dev,
+           chain_early(h, st), h->C);
 }

@@ -232,6 +232,67 @@ def test_heat_flow_from_a_hot_cylinder_matches_the_shape_factor_on_the_gpu(gpu, 
         assert abs(q / expected - 1.0) < 0.01, (d, W, q, expected)
 
 
+def test_coupling_closed_forms_on_the_gpu(gpu, ob, wl):
+    """The closed forms that pin the rotational / geometric half of the coupling in the oracle
+    (tests/test_oracle_coupling_pins.py), asserted on the CUDA path directly: circular Couette
+    torque on a spinning cylinder; one-step dU = F/M, dOmega = T_z/I with M, I from quadrature
+    (disc and 3 : 1 ellipse); Eq. (15) against each of the four walls; the ellipse pair gap through
+    the support functions and the wall gap at the vertex of an upright ellipse."""
+    import math
+    import test_oracle_coupling_pins as pins
+
+    class AsOracle:                       # the pins' set-up helpers build "ob.OracleSim"s
+        OracleSim = gpu.Simulation
+    # (a) Couette
+    r, L, nu, rim = 9.0, 64, 1.0 / 6.0, 0.01
+    g = pins.spinning_cylinder(AsOracle, wl, r, L=L, nu=nu, rim_speed=rim, steps=5000)
+    P = g.particles()
+    expected = -4.0 * math.pi * nu * (rim / r) * r * r / (1.0 - (r / (0.5 * L)) ** 2)
+    assert -0.035 < P["Tz"][0] / expected - 1.0 < 0.005, (P["Tz"][0], expected)
+    # (b) mass and inertia as the step uses them
+    for a, b, theta in ((5.3, 5.3, None), (9.0, 3.0, 0.5)):
+        ratio = 1.6
+        Mq, Iq = pins.quadrature_mass_inertia(a, b, ratio)
+        p = pins.base_params(wl, 1, 2 * a, g=0.0, gbeta=0.0, nu=0.05)
+        parts = dict(x=np.array([40.3]), y=np.array([31.7]), diam=np.array([2 * a]),
+                     rho_ratio=np.array([ratio]), T_w=np.array([0.0]), ux=np.array([0.02]),
+                     uy=np.array([0.015]), omega=np.array([0.003]))
+        if theta is not None:
+            parts.update(minor=np.array([2 * b]), theta=np.array([theta]))
+        s = gpu.Simulation.from_workload(wl.Workload("kick", 80, 64, p, 1, 1, particles=parts))
+        s.step(5)
+        dux, duy, dom, Fx, Fy, Tz = pins.one_step_increments(s)
+        assert abs(Fx) > 1e-3 and abs(Tz) > 1e-4
+        assert dux == pytest.approx(Fx / Mq, rel=3e-3) and duy == pytest.approx(Fy / Mq, rel=3e-3)
+        assert dom == pytest.approx(Tz / Iq, rel=3e-3)
+        M = ratio * math.pi * a * b
+        assert dux == pytest.approx(Fx / M, rel=1e-10)
+        assert dom == pytest.approx(Tz / (0.25 * M * (a * a + b * b)), rel=1e-10)
+    # (c), (d): the pins themselves, run with the CUDA path standing in for the oracle
+    pins.test_repulsion_from_each_of_the_four_walls_in_closed_form(AsGpu(gpu), wl)
+    pins.test_ellipse_pair_gap_is_taken_through_the_support_functions(AsGpu(gpu), wl)
+    pins.test_upright_ellipse_is_repelled_by_the_bottom_wall_at_its_vertex(AsGpu(gpu), wl)
+    # Eq. (14) with a moving wall on a fixed disc (the pin's brute-force case): parity of F, T_z
+    r, xc, yc, U, V, Om = 6.3, 24.3, 21.8, 0.08, -0.05, 0.012
+    p = pins.base_params(wl, 1, 2 * r, g=0.0, gbeta=0.0, nu=0.02)
+    parts = dict(x=np.array([xc]), y=np.array([yc]), diam=np.array([2 * r]),
+                 rho_ratio=np.array([2.0]), T_w=np.array([0.0]), ux=np.array([U]),
+                 uy=np.array([V]), omega=np.array([Om]), fixed=np.array([1], dtype=np.uint8))
+    run_and_compare(gpu, ob, wl.Workload("arm", 48, 44, p, 61, 61, particles=parts), [61], r_min=6.3)
+
+
+class AsGpu:
+    """Lets a pin written against the oracle binding run against the CUDA binding: the same
+    constructor and method names, `OracleSim(nx, ny, params)` included."""
+
+    def __init__(self, gpu):
+        class Sim(gpu.Simulation):
+            def add_particles(self, **kw):
+                super().add_particles(**{k: (None if v is None else np.asarray(v, dtype=np.uint8 if k == "fixed" else np.float64))
+                                         for k, v in kw.items()})
+        self.OracleSim = Sim
+
+
 def test_paper_repulsion_variant(gpu, ob, wl):
     """Eq. (15) as the paper prints it: quadratic, s = 3, eps_w = 1e-3; two
     particles approaching head-on and one falling onto the bottom wall."""
@@ -413,6 +474,93 @@ def test_chain_grid_size_does_not_change_results(gpu, wl, monkeypatch):
         La, Lb = a.links(), b.links()
         for k in Lb:
             assert np.array_equal(np.asarray(La[k]), np.asarray(Lb[k])), k
+
+
+def assert_same_bits(a, b):
+    fa, fb = a.fields(populations=True), b.fields(populations=True)
+    fluid = fa["flag"] == 0
+    assert np.array_equal(fa["flag"], fb["flag"])
+    for k in ("f", "g"):
+        assert np.array_equal(fa[k][:, fluid], fb[k][:, fluid]), k
+    pa, pb = a.particles(), b.particles()
+    for k in pa:
+        assert np.array_equal(pa[k], pb[k]), k
+
+
+def test_graph_replay_equals_direct_launches_bitwise(gpu, wl):
+    """lbm_step replays whole periods of the schedule as CUDA graphs (8 steps per launch, then 2,
+    an odd last step directly).  Every mix of those must give the bits of the direct launches, in
+    the overlapped and in the sequential schedule, from either phase of the A/B swap."""
+    w = wl.sedimentation(300, 260, 14, seed=9, y_frac_lo=0.2, d_lo=12.0, d_hi=24.0, name="graph")
+    a = gpu.Simulation.from_workload(w)              # graphs, overlapped
+    b = gpu.Simulation.from_workload(w)
+    b.set_graph(False)                               # direct launches, overlapped
+    c = gpu.Simulation.from_workload(w)
+    c.set_overlap(False)                             # graphs, sequential
+    for n in (1, 2, 7, 16, 33, 8, 101):
+        counts = []
+        for s in (a, b, c):
+            l0 = s.kernel_launches()
+            s.step(n)
+            counts.append(s.kernel_launches() - l0)
+        assert counts[0] == counts[1] == counts[2] > 0      # replayed kernels are counted
+        assert_same_bits(a, b)
+        assert_same_bits(c, b)
+
+
+def dense_pack(wl, n_side=10, d=12.0, gap=1.95, big=True):
+    """A hexagonal pack of d = 12 discs at surface gap 1.95 (every disc has six neighbours just
+    inside the repulsion range s = 2) next to one d = 30 disc, which makes the repulsion cells 32
+    wide: the 3 x 3 cells around a disc of the pack then hold more than 40 centres."""
+    pitch = d + gap
+    xs, ys = [], []
+    for r in range(n_side):
+        for c in range(n_side):
+            xs.append(20.0 + c * pitch + (0.5 * pitch if r % 2 else 0.0))
+            ys.append(20.0 + r * pitch * np.sqrt(3.0) / 2.0)
+    ds = [d] * len(xs)
+    if big:
+        xs.append(200.0)
+        ys.append(60.0)
+        ds.append(30.0)
+    n = len(xs)
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=n,
+             max_links_per_particle=wl.max_links_for_diameter(30.0))
+    parts = dict(x=np.array(xs), y=np.array(ys), diam=np.array(ds), rho_ratio=np.full(n, 1.5),
+                 T_w=np.full(n, 1.0))
+    return wl.Workload("dense_pack", 240, 170, p, 20, 20, particles=parts)
+
+
+def test_repulsion_sum_is_order_deterministic_with_many_candidates(gpu, ob, wl):
+    """More than 32 candidates in the 3 x 3 repulsion cells (the integrator's batch size): the
+    contributions must still be added in ascending particle id, as the oracle does, whatever
+    order the cell slots were filled in (atomicAdd order of the flag update, different from run
+    to run).  20 repeated runs and both schedules give identical bits; the oracle agrees."""
+    w = dense_pack(wl)
+    P = w.particles
+    cell = 32.0
+    ci, cj = np.floor(P["x"] / cell), np.floor(P["y"] / cell)
+    k = 44                                            # a disc in the middle of the pack
+    cand = int(((np.abs(ci - ci[k]) <= 1) & (np.abs(cj - cj[k]) <= 1)).sum())
+    assert cand >= 40, cand
+    ref = gpu.Simulation.from_workload(w)
+    ref.set_overlap(False)
+    ref.step(20)
+    pr = ref.particles()
+    assert np.abs(pr["ux"]).max() > 1e-3              # the pack is really pushing itself apart
+    for rep in range(20):
+        s = gpu.Simulation.from_workload(w)
+        if rep % 2:
+            s.set_graph(False)
+        s.step(20)
+        ps = s.particles()
+        for key in pr:
+            assert np.array_equal(ps[key], pr[key]), (rep, key)
+    o = ob.OracleSim.from_workload(w)
+    o.step(20)
+    assert_particles_close(pr, o.particles(), r_min=6.0, steps=20)
+    assert_fields_close(ref.fields(populations=True), o.fields(populations=True))
 
 
 # ------------------------------------------------------------------ boundary behaviour
