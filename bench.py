@@ -239,6 +239,7 @@ def main():
 
     seq = profile_pass(False)
     ovl = profile_pass(True)
+    band_q = sim.band_rows()     # rows [0, Q) advanced two steps per pass (0: none)
     st = sim.fields()
     flag = st["flag"]
     n_fluid = int((flag == 0).sum())
@@ -250,8 +251,23 @@ def main():
     far_s = seq[kname] * 1e-3
     far_ovl_s = ovl[kname] * 1e-3
     step_ms_seq = sum(seq.values())
-    # 14 doubles read + 14 written per fluid node + 1 flag byte per node
-    alg_bytes = (2 * BYTES_PER_LU * n_fluid) if two_step else (BYTES_PER_LU * n_fluid + FLAG_BYTES * n)
+    # 14 doubles read + 14 written per fluid node + 1 flag byte per node.
+    # With a two-step band the one-step kernel covers the rows from Q up (and row Q-1 in every
+    # other step); the band's kernel advances Q*nx nodes by one step per launch on average
+    if two_step:
+        alg_bytes = 2 * BYTES_PER_LU * n_fluid
+    elif band_q > 0:
+        fluid_top = int((flag[band_q:] == 0).sum()) + 0.5 * w.nx
+        alg_bytes = BYTES_PER_LU * fluid_top + FLAG_BYTES * (w.ny - band_q + 0.5) * w.nx
+    else:
+        alg_bytes = BYTES_PER_LU * n_fluid + FLAG_BYTES * n
+    band = None
+    if band_q > 0 and not two_step:
+        b_s = ovl["stream_collide_2step"] * 1e-3
+        band = {"rows": band_q, "kernel": "k_stream_collide_2step", "launches_per_step": 1,
+                "lattice_updates_per_launch": band_q * w.nx, "avg_launch_ms": b_s * 1e3,
+                "avg_launch_ms_alone": seq["stream_collide_2step"],
+                "algorithmic_gbs_at_224_B_per_update": BYTES_PER_LU * band_q * w.nx / b_s / 1e9 if b_s > 0 else None}
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
@@ -273,6 +289,10 @@ def main():
                 "whole_step_frac_of_hbm_roofline": value / world / (peak * 1e9 / BYTES_PER_LU / 1e6),
                 # north_star words the roofline as "about 8 TB/s" (nominal): 35,714 MLUPS
                 "whole_step_frac_of_nominal_8TBs_roofline": value / world / (8.0e12 / BYTES_PER_LU / 1e6),
+                # the same step counted in the method's own bytes (224 B per FLUID node + 1 flag
+                # byte per node; solid nodes are never moved) over the step time, against the peak
+                "whole_step_frac_fluid_bytes": (BYTES_PER_LU * n_fluid + FLAG_BYTES * n) / (ms_max / K * 1e-3) / 1e9 / peak,
+                "two_step_band": band,
                 "fluid_fraction": n_fluid / n}
     sim.close()
     del sim

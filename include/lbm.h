@@ -139,6 +139,18 @@ int lbm_set_graph(lbm_t* h, int on);
  * arithmetic per step is the same, so results are identical bit for bit to on = 0. */
 int lbm_set_two_step(lbm_t* h, int on);
 
+/* on = 1 (default; LBM_BAND=0 turns the default off): lattices WITH particles also use the
+ * two-steps-per-pass kernel, on the particle-free rows [0, Q) below the lowest particle (SURVEY
+ * 8(f)-4).  In periods of four time steps a
+ * device kernel picks Q from the particle positions and speeds (far enough below the lowest
+ * particle that no link or refill stencil reaches the band within the period; fewer than 28 free
+ * rows: no band), the band is advanced t -> t+2 -> t+4 by the two-step kernel while the rows
+ * above it take four ordinary steps, the two meeting in one row that is computed by both.  The
+ * arithmetic per node and step is unchanged: results are identical bit for bit to on = 0.
+ * lbm_get_band: *rows = Q of the last banded period completed by lbm_step (0: none). */
+int lbm_set_band(lbm_t* h, int on);
+int lbm_get_band(lbm_t* h, int* rows);
+
 /* Readout.  Any pointer may be NULL = not wanted.
  * rho, ux, uy, T: nx*ny doubles each; on fluid nodes rho = sum f, T = sum g,
  *   u = (sum e f + F/2)/rho; on solid nodes rho0, rigid-body velocity, T_w.

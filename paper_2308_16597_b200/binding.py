@@ -77,6 +77,8 @@ def load_library():
     L.lbm_set_overlap.argtypes = [vp, C.c_int]
     L.lbm_set_two_step.argtypes = [vp, C.c_int]
     L.lbm_set_graph.argtypes = [vp, C.c_int]
+    L.lbm_set_band.argtypes = [vp, C.c_int]
+    L.lbm_get_band.argtypes = [vp, C.POINTER(C.c_int)]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
     L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
@@ -93,7 +95,7 @@ def load_library():
     for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_add_ellipses", "lbm_step",
                  "lbm_get_fields", "lbm_get_particles", "lbm_get_links", "lbm_profile_enable",
                  "lbm_profile_kernels", "lbm_profile_get", "lbm_destroy", "lbm_set_overlap",
-                 "lbm_set_two_step", "lbm_set_graph"):
+                 "lbm_set_two_step", "lbm_set_graph", "lbm_set_band", "lbm_get_band"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -197,6 +199,15 @@ class Simulation:
 
     def set_graph(self, on=True):
         self._chk(self._L.lbm_set_graph(self._h, 1 if on else 0))
+
+    def set_band(self, on=True):
+        self._chk(self._L.lbm_set_band(self._h, 1 if on else 0))
+
+    def band_rows(self):
+        """Rows [0, Q) the last banded period advanced two steps per pass (0: none)."""
+        q = C.c_int(0)
+        self._chk(self._L.lbm_get_band(self._h, C.byref(q)))
+        return q.value
 
     def set_two_step(self, on=True):
         self._chk(self._L.lbm_set_two_step(self._h, 1 if on else 0))

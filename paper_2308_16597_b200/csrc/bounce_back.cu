@@ -37,11 +37,12 @@ __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, in
 }
 
 __global__ void __launch_bounds__(BT, 8)
-k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, int early,
+k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur, int np, int early,
               const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();   // the previous step's refill commit (and, through it, everything before)
-  const int p = blockIdx.x;
+  __shared__ double s_red[3][BT / 32];
+  for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic (one CTA per particle, or fewer)
   const int n = la.count[p];
   const long long base = (long long)p * la.cap;
   const double xc = pa.x[cur][p], yc = pa.y[cur][p];
@@ -141,7 +142,6 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     Fy += __shfl_xor_sync(0xffffffffu, Fy, d);
     Tz += __shfl_xor_sync(0xffffffffu, Tz, d);
   }
-  __shared__ double s_red[3][BT / 32];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (lane == 0) {
     s_red[0][warp] = Fx;
@@ -160,6 +160,8 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     pa.Fx[p] = a;
     pa.Fy[p] = b;
     pa.Tz[p] = t;
+  }
+  __syncthreads();   // s_red is reused by the next particle
   }
 }
 
@@ -304,10 +306,16 @@ __global__ void k_refill_commit(double* __restrict__ B, const double* __restrict
 
 } // namespace
 
-void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl) {
+// ctas_per_sm > 0: that many persistent CTAs per SM instead of one CTA per particle.  The kernel
+// is bound by scattered sector requests, not by occupancy, so in the
+// banded schedule it runs at half its occupancy and leaves the other half of every SM to the
+// band's two-step kernel, which is launched beside it.
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl, int ctas_per_sm) {
   if (h->np == 0) return;
   h->launches++;
-  launch_k(k_bounce_back, dim3(h->np), dim3(BT), 0, st, pdl, h->A, h->la, h->pa, h->cur,
+  int grid = h->np;
+  if (ctas_per_sm > 0 && grid > ctas_per_sm * h->sm_count) grid = ctas_per_sm * h->sm_count;
+  launch_k(k_bounce_back, dim3(grid), dim3(BT), 0, st, pdl, h->A, h->la, h->pa, h->cur, h->np,
            h->chain_ctas > 0 ? 0 : 1, h->C);
 }
 

@@ -21,7 +21,7 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "integrate_uncover",
-    "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step"};
+    "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step", "band_plan"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -77,7 +77,7 @@ struct Layout {
 Layout layout_of(int nx, int ny, const lbm_params* p) {
   Layout L;
   L.px = (int)align_up((size_t)nx, 16);
-  L.ps = (long long)align_up((size_t)L.px * ny, 32);
+  L.ps = (long long)align_up((size_t)L.px * (ny + 1), 32);   // one spare row (the band seam's)
   L.mcx = (int)std::ceil(nx / MIN_CELL) + 1;
   L.mcy = (int)std::ceil(ny / MIN_CELL) + 1;
   L.max_cells = p->max_particles > 0 ? L.mcx * L.mcy : 0;
@@ -134,7 +134,9 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   int* nb_count = c.take<int>(2);
   double* stash = c.take<double>((size_t)L.newborn_cap * 14);
   int* status = c.take<int>(1);
+  int* band = c.take<int>(2);
   if (h) {
+    h->band = band;
     h->px = L.px;
     h->ps = L.ps;
     h->A = A;
@@ -223,6 +225,7 @@ struct Timed {
 
 int check_status(lbm* h) {
   CUDA_OK(h, cudaMemcpyAsync(h->status_host, h->status_dev, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
   const int st = *h->status_host;
@@ -314,7 +317,7 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     delete h;
     return fail(nullptr, LBM_E_CUDA, "lbm_create: max_links_per_particle needs more shared memory than the device has");
   }
-  cudaError_t e = cudaMallocHost((void**)&h->status_host, sizeof(int));
+  cudaError_t e = cudaMallocHost((void**)&h->status_host, 2 * sizeof(int));
   if (e != cudaSuccess) {
     fail(nullptr, LBM_E_CUDA, "cudaMallocHost: %s", cudaGetErrorString(e));
     delete h;
@@ -332,7 +335,7 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     h->chain_priority = hi;
     bool ok = cudaStreamCreateWithPriority(&h->chain_own, cudaStreamNonBlocking, hi) == cudaSuccess &&
               cudaStreamCreateWithPriority(&h->side_own, cudaStreamNonBlocking, hi) == cudaSuccess;
-    cudaEvent_t* evs[6] = {&h->ev_in, &h->ev_out, &h->ev_bb, &h->ev_sc, &h->ev_cov, &h->ev_ref};
+    cudaEvent_t* evs[7] = {&h->ev_in, &h->ev_out, &h->ev_bb, &h->ev_sc, &h->ev_cov, &h->ev_ref, &h->ev_plan};
     for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
     if (ok) {
       h->overlap = 1;
@@ -363,6 +366,14 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   cudaMemsetAsync(h->flag, 0, nn, h->stream);
   cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
   cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
+  cudaMemsetAsync(h->band, 0, 2 * sizeof(int), h->stream);
+  h->status_host[1] = 0;
+  {
+    const char* eb = getenv("LBM_BAND");
+    h->band_on = (eb && atoi(eb) == 0) ? 0 : 1;
+    const char* ec = getenv("LBM_BAND_BB_CTAS");
+    h->band_bb_ctas = ec ? atoi(ec) : 4;
+  }
   cudaMemsetAsync(h->newborn_count, 0, 2 * sizeof(int), h->stream);
   for (int b = 0; b < 2; ++b)
     if (h->max_cells) cudaMemsetAsync(h->cell_count[b], 0, sizeof(int) * (size_t)h->max_cells, h->stream);
@@ -575,22 +586,50 @@ static void note_chain_node(lbm* h, cudaStream_t S1) {
 // S1 is one dependent chain from step to step (the next bounce-back follows the commit), each link
 // a programmatic dependent launch.  The caller's stream is joined to it at both ends of a call.
 // Enqueues ONE time step (the streams may be capturing) and flips the host-side phase (A/B, cur).
-static void enqueue_step(lbm* h) {
+//
+// Banded schedule (phase = 0..3, the position of the step in a period of four; phase = -1: the
+// plain step above).  At the start of a period (every row in A at the same time t) k_band_plan
+// picks Q from the particle positions; for the four steps the rows [0, Q) belong to the two-step
+// kernel: with X, Y = A, B at the start of the period,
+//   steps 0, 1: band X -> Y (t -> t+2);  rows >= Q: X -> Y -> X as always
+//   steps 2, 3: band Y -> X (t+2 -> t+4); rows >= Q: X -> Y -> X
+// The band's tile rows of a pair are dealt to its two steps and launched on S0 BEFORE the wait for
+// the bounce-back kernel: they fill the time in which that latency-bound kernel leaves the
+// memory system idle.  The one-step kernel of the first step of a pair also updates row Q-1 (into
+// the spare row of its output copy), which the second step reads there; the band's part of a pair
+// is complete before the second step's one-step kernel overwrites the rows Q, Q+1 of X it reads.
+static void enqueue_step(lbm* h, int phase) {
   cudaStream_t S0 = h->stream, S1 = h->chain, S2 = h->side;
   const bool fork = S1 != S0;
   const bool pdl = h->use_pdl != 0;
+  const bool banded = phase >= 0;
   const int sp = h->cur;   // step parity: which newborn counter / repulsion grid this step uses
-  if (h->np > 0) {
-    { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h, S1, pdl); }
+  double* X = (phase & 1) ? h->B : h->A;   // the copies as they were named at the start of the period
+  double* Y = (phase & 1) ? h->A : h->B;
+  const double* band_src = phase < 2 ? X : Y;
+  double* band_dst = phase < 2 ? Y : X;
+  if (banded && phase == 0) {
+    { Timed tm(h, K_BAND_PLAN, S1); launch_band_plan(h, S1); }
     note_chain_node(h, S1);
     if (fork) {
-      cudaEventRecord(h->ev_bb, S1);
-      cudaStreamWaitEvent(S0, h->ev_bb, 0);
+      cudaEventRecord(h->ev_plan, S1);
+      cudaStreamWaitEvent(S0, h->ev_plan, 0);
     }
   }
+  if (h->np > 0) {
+    { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h, S1, pdl, (banded && fork) ? h->band_bb_ctas : 0); }
+    note_chain_node(h, S1);
+    if (fork) cudaEventRecord(h->ev_bb, S1);
+  }
+  if (banded) {
+    Timed tm(h, K_STREAM_COLLIDE_2STEP, S0);
+    launch_stream_collide_band(h, band_src, X, band_dst, 2, phase & 1);
+  }
+  if (h->np > 0 && fork) cudaStreamWaitEvent(S0, h->ev_bb, 0);
+  const int lattice_mode = banded ? ((phase & 1) ? 2 : 1) : 0;
   if (fork || h->np == 0) {
     Timed tm(h, K_STREAM_COLLIDE, S0);
-    launch_stream_collide(h);
+    launch_stream_collide(h, lattice_mode, band_src);
   }
   if (h->np > 0) {
     if (fork) cudaEventRecord(h->ev_sc, S0);
@@ -613,7 +652,7 @@ static void enqueue_step(lbm* h) {
       cudaStreamWaitEvent(S1, h->ev_ref, 0);
     } else {
       Timed tm(h, K_STREAM_COLLIDE, S0);
-      launch_stream_collide(h);
+      launch_stream_collide(h, lattice_mode, band_src);
     }
     { Timed tm(h, K_REFILL_COMMIT, S1); launch_refill_commit(h, sp, S1, pdl); }
     note_chain_node(h, S1);
@@ -643,11 +682,11 @@ static void drop_graphs(lbm* h) {
 // captured now.  Capture runs on the library's own stream pair (the caller's stream may be the
 // legacy default stream, which cannot capture); the fork / join events turn into graph edges.
 // Returns nullptr if capture is not possible (the caller then launches directly).
-static lbm::StepGraph* step_graph(lbm* h, int steps) {
+static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   for (int k = 0; k < h->n_graphs; ++k) {
     lbm::StepGraph& g = h->graphs[k];
     if (g.A == h->A && g.cur == h->cur && g.steps == steps && g.overlap == h->overlap &&
-        g.chain_ctas == h->chain_ctas)
+        g.chain_ctas == h->chain_ctas && g.banded == banded)
       return &g;
   }
   if (h->n_graphs == LBM_MAX_GRAPHS) drop_graphs(h);
@@ -664,7 +703,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps) {
   if (e == cudaSuccess) {
     if (h->chain != h->stream) h->cap_nodes = &chain_nodes;
     join_in(h);
-    for (int s = 0; s < steps; ++s) enqueue_step(h);
+    for (int s = 0; s < steps; ++s) enqueue_step(h, banded ? s % 4 : -1);
     join_out(h);
     h->cap_nodes = nullptr;
     e = cudaStreamEndCapture(h->cap_stream, &graph);
@@ -706,6 +745,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps) {
   g.steps = steps;
   g.overlap = h->overlap;
   g.chain_ctas = h->chain_ctas;
+  g.banded = banded;
   g.launches = per;
   return &g;
 }
@@ -719,13 +759,17 @@ int lbm_step(lbm_t* h, int nsteps) {
     ensure_links(h);
   }
   int s = 0;
+  // the banded schedule needs the particle-free two-step kernel and runs in periods of four steps
+  const bool band_ok = h->np > 0 && h->band_on && h->two_step_ok;
   // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
-  // launch while that many remain, then 2), the odd last step directly; event profiling needs
-  // the direct launches
+  // launch while that many remain, then 4 if banded, then 2), the odd last step directly; event
+  // profiling needs the direct launches
   if (h->np > 0 && h->use_graph && !h->prof_on) {
     while (nsteps - s >= 2) {
-      const int unit = nsteps - s >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : 2;
-      lbm::StepGraph* g = step_graph(h, unit);
+      const int left = nsteps - s;
+      const int banded = (band_ok && left >= 4) ? 1 : 0;
+      const int unit = left >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : (banded ? 4 : 2);
+      lbm::StepGraph* g = step_graph(h, unit, banded);
       if (!g) break;
       CUDA_OK(h, cudaGraphLaunch(g->exec, h->stream));
       h->launches += g->launches;
@@ -735,20 +779,39 @@ int lbm_step(lbm_t* h, int nsteps) {
   }
   if (s < nsteps) join_in(h);
   const bool direct = s < nsteps;
-  for (; s < nsteps; ++s) {
+  while (s < nsteps) {
     if (h->np == 0 && h->two_step && nsteps - s >= 2) {
       // particle-free lattice: two time steps per pass over the populations (A -> B)
       { Timed tm(h, K_STREAM_COLLIDE_2STEP, h->stream); launch_stream_collide_2step(h); }
       std::swap(h->A, h->B);
       h->steps_done += 2;
-      ++s;
+      s += 2;
       continue;
     }
-    enqueue_step(h);
+    if (band_ok && nsteps - s >= 4) {
+      for (int ph = 0; ph < 4; ++ph) enqueue_step(h, ph);
+      h->steps_done += 4;
+      s += 4;
+      continue;
+    }
+    enqueue_step(h, -1);
     h->steps_done++;
+    ++s;
   }
   if (direct) join_out(h);
   return check_status(h);
+}
+
+int lbm_set_band(lbm_t* h, int on) {
+  if (!h) return LBM_E_ARG;
+  h->band_on = on ? 1 : 0;
+  return LBM_OK;
+}
+
+int lbm_get_band(lbm_t* h, int* rows) {
+  if (!h || !rows) return LBM_E_ARG;
+  *rows = (h->np > 0 && h->band_on && h->two_step_ok) ? h->status_host[1] : 0;
+  return LBM_OK;
 }
 
 int lbm_set_graph(lbm_t* h, int on) {
@@ -926,7 +989,7 @@ int lbm_destroy(lbm_t* h) {
     cudaStreamSynchronize(h->chain_own);
     cudaStreamDestroy(h->chain_own);
     if (h->side_own) cudaStreamDestroy(h->side_own);
-    cudaEvent_t evs[6] = {h->ev_in, h->ev_out, h->ev_bb, h->ev_sc, h->ev_cov, h->ev_ref};
+    cudaEvent_t evs[7] = {h->ev_in, h->ev_out, h->ev_bb, h->ev_sc, h->ev_cov, h->ev_ref, h->ev_plan};
     for (cudaEvent_t e : evs) cudaEventDestroy(e);
   }
   for (int k = 0; k < K_COUNT; ++k)

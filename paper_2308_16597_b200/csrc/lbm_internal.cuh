@@ -31,7 +31,7 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_MOVE, K_COVER, K_REFILL,
-  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_COUNT
+  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_BAND_PLAN, K_COUNT
 };
 
 // link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along
@@ -121,7 +121,13 @@ struct lbm {
   double* stash;             // 14 refilled populations per newborn-list entry
   int newborn_cap;
   int* status_dev;
-  int* status_host;          // pinned
+  int* status_host;          // pinned: [0] status word, [1] band height of the last banded period
+  // two-step band: band[0] = Q, rows
+  // [0, Q) are advanced two steps per pass; band[1] = 0 (what the plain schedule's kernels read)
+  int* band;
+  int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
+  int band_bb_ctas;          // bounce-back CTAs per SM beside the band kernel (LBM_BAND_BB_CTAS; 0 = one per particle)
+  cudaEvent_t ev_plan, ev_l1;
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
   long long steps_done;
   long long launches;        // kernels launched (lbm_kernel_launches)
@@ -139,7 +145,7 @@ struct lbm {
   struct StepGraph {
     cudaGraphExec_t exec;
     const double* A;         // phase the graph was captured in
-    int cur, steps, overlap, chain_ctas;
+    int cur, steps, overlap, chain_ctas, banded;
     long long launches;      // kernels per replay
   } graphs[LBM_MAX_GRAPHS];
   int n_graphs;
@@ -180,8 +186,10 @@ inline void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
 
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
-void launch_stream_collide(lbm* h);        // on h->stream
+void launch_stream_collide(lbm* h, int band, const double* low);   // on h->stream, h->A -> h->B
 void launch_stream_collide_2step(lbm* h);  // on h->stream; particle-free lattices only
+void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
+                                int nparts, int part);   // on h->stream; rows [0, *h->band)
 int stream_collide_configure();            // kernel attributes (0 = ok)
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
@@ -195,7 +203,8 @@ void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
 void launch_move(lbm* h, cudaStream_t st, bool pdl);   // integrator + uncover, buffer cur -> cur ^ 1
 int particles_configure(lbm* h);           // per-handle kernel attributes (0 = ok)
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
+void launch_band_plan(lbm* h, cudaStream_t st);   // h->band[0] from the positions of buffer h->cur
 // bounce_back.cu
-void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl);
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl, int ctas_per_sm);
 void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped
 void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl);  // stash -> B, newborn flags cleared

@@ -695,6 +695,38 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
   }
 }
 
+// ------------------------------------------------------------------------------------------
+// Two-step band: the rows [0, Q) below the
+// lowest particle are advanced two time steps per pass by k_stream_collide_2step for the next
+// BAND_PERIOD steps.  Within those steps no solid node, no link stencil (x_f - 2 e_i) and no refill
+// stencil (x_new + 3 e_c and its upstream neighbours) may reach below row Q: with the lowest solid
+// row >= floor(min_p(y_p - r_p)) that needs Q + 4 <= lowest solid row, plus what the particle can
+// fall in BAND_PERIOD steps (its speed now, one node for its acceleration, one in reserve).
+// A band of fewer than BAND_MIN rows is not worth its seam: Q = 0 (no band).  One CTA.
+constexpr int BAND_PERIOD = 4;
+constexpr int BAND_MIN = 28;
+__global__ void __launch_bounds__(1024)
+k_band_plan(ParticleArrays pa, int cur, int np, int ny, int* __restrict__ band) {
+  __shared__ double s_min[32];
+  double low = 1.0e300;
+  for (int p = threadIdx.x; p < np; p += blockDim.x) {
+    const double fall = pa.fixed[p] ? 0.0 : fmax(-pa.uy[cur][p], 0.0);
+    low = fmin(low, pa.y[cur][p] - pa.r[p] - (double)BAND_PERIOD * fall);
+  }
+#pragma unroll
+  for (int d = 16; d >= 1; d >>= 1) low = fmin(low, __shfl_xor_sync(0xffffffffu, low, d));
+  if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = low;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) low = fmin(low, s_min[w]);
+    int Q = 0;
+    if (low == low && low < 1.0e9 && low > -1.0e9) Q = (int)floor(low) - 6;
+    if (Q > ny - 8) Q = ny - 8;
+    if (Q < BAND_MIN) Q = 0;
+    band[0] = Q;
+  }
+}
+
 } // namespace
 
 // CTAs of a particle-chain kernel.  On the library's own stream (concurrent with the lattice
@@ -769,4 +801,11 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
            h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell, h->ncx, h->ncy,
            h->cell_count[which_buffer], h->cell_items[which_buffer], h->status_dev,
            chain_early(h, st), h->C);
+}
+
+// rows [0, h->band[0]) of the next BAND_PERIOD steps go to the two-step kernel (positions of
+// buffer h->cur); a plain launch: it starts after everything before it in `st` has completed
+void launch_band_plan(lbm* h, cudaStream_t st) {
+  h->launches++;
+  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band);
 }

@@ -23,11 +23,36 @@ __host__ __device__ constexpr int opp_of(int k) { return k == 0 ? 0 : (k <= 4 ? 
 
 constexpr int SC_THREADS = 128;
 
-// generic pull with cavity-wall handling; only nodes on the lattice rim take this path.
-// Fully unrolled and inlined so that f, g stay in registers.
-__device__ __forceinline__ void pull_boundary(const double* __restrict__ A, const LbmConst& c, int i,
+// Where the rows of the state a node pulls from live.  Normally every row j sits in one copy of
+// the populations at node index j*px + i.  Along the seam of a two-step band (DESIGN.md "Two steps
+// per pass below the suspension") the rows below the seam row Q come from elsewhere: from the
+// band's own copy (which runs two steps behind / ahead of the rest), or, for the single row Q-1 at
+// the intermediate time, from the spare row ny of the same copy.
+struct RowsPlain {
+  const double* A;
+  int px;
+  __device__ __forceinline__ const double* base(int) const { return A; }
+  __device__ __forceinline__ long long row0(int sj) const { return (long long)sj * px; }
+};
+struct RowsSeam {
+  const double* top;   // rows >= Q
+  const double* low;   // rows < Q
+  int Q;
+  int low_row;         // >= 0: every row < Q is stored as this row of `low` (the spare row)
+  int px;
+  __device__ __forceinline__ const double* base(int sj) const { return sj < Q ? low : top; }
+  __device__ __forceinline__ long long row0(int sj) const {
+    return (long long)((sj < Q && low_row >= 0) ? low_row : sj) * px;
+  }
+};
+
+// generic pull with cavity-wall handling; nodes on the lattice rim and the rows along a band seam
+// take this path.  Fully unrolled and inlined so that f, g stay in registers.
+template <typename Rows>
+__device__ __forceinline__ void pull_boundary(const Rows& R, const LbmConst& c, int i,
                                               int j, double (&f)[9], double (&g)[5]) {
-  const long long x = (long long)j * c.px + i;
+  const double* __restrict__ Aj = R.base(j);
+  const long long x = R.row0(j) + i;
 #pragma unroll
   for (int k = 0; k < 9; ++k) {
     int si = i - ex_of(k), sj = j - ey_of(k);
@@ -35,7 +60,7 @@ __device__ __forceinline__ void pull_boundary(const double* __restrict__ A, cons
     if (si < 0 || si >= c.nx) {
       if (c.periodic_x) si = (si + c.nx) % c.nx; else in = false;
     }
-    f[k] = in ? A[f_at(k, (long long)sj * c.px + si, c.ps)] : A[f_at(opp_of(k), x, c.ps)];
+    f[k] = in ? R.base(sj)[f_at(k, R.row0(sj) + si, c.ps)] : Aj[f_at(opp_of(k), x, c.ps)];
   }
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
@@ -46,9 +71,9 @@ __device__ __forceinline__ void pull_boundary(const double* __restrict__ A, cons
       if (c.periodic_x) si = (si + c.nx) % c.nx;
       else { in = false; wall = si < 0 ? 0 : 1; }
     }
-    if (in) g[k] = A[g_at(k, (long long)sj * c.px + si, c.ps)];
+    if (in) g[k] = R.base(sj)[g_at(k, R.row0(sj) + si, c.ps)];
     else {
-      const double gb = A[g_at(opp_of(k), x, c.ps)];
+      const double gb = Aj[g_at(opp_of(k), x, c.ps)];
       g[k] = c.wall_type[wall] == 1 ? (2.0 * c.wT * c.wall_T[wall] - gb) : gb;
     }
   }
@@ -85,14 +110,14 @@ __device__ __forceinline__ void pull_node(const double* __restrict__ A, const Lb
     f[3] = p3.x; g[3] = p3.y;
     f[4] = p4.x; g[4] = p4.y;
   } else {
-    pull_boundary(A, c, i, j, f, g);
+    pull_boundary(RowsPlain{A, c.px}, c, i, j, f, g);
   }
 }
 
 // the same nine accesses as stores
 __device__ __forceinline__ void store_node(double* __restrict__ B, const LbmConst& c, int i, int j,
                                            const double (&f)[9], const double (&g)[5]) {
-  const long long x = (long long)j * c.px + i;
+  const long long x = (long long)j * c.px + i;   // j: the row of the copy the node is stored in
   const long long ps = c.ps;
   double* __restrict__ O = B + 2 * x;
 #pragma unroll
@@ -122,13 +147,33 @@ __device__ __forceinline__ void update_node(const double* __restrict__ A, double
 // The flag update of this step (k_uncover / k_cover on the chain stream) may run concurrently:
 // a node it covers (0 -> 1) was fluid at t, so updating it or not are both fine (its B slot is
 // don't-care from t+1 on); a node it uncovers (1 -> 2) is skipped under either value.
+//
+// Two-step band: rows [0, Q), Q = *bandp,
+// belong to k_stream_collide_2step, which advances them two steps per pass; this kernel covers
+// the rows from Q + delta up.  In the first step of a pair (delta = -1) it also updates row Q-1,
+// whose result -- the one row of the band the second step needs at the intermediate time -- goes
+// to the spare row ny of B; rows below Q are read from the band's copy Alow.  In the second step
+// (delta = 0, Alow = nullptr) row Q-1 is read from the spare row of A.  Rows Q-1 and Q take the
+// generic pull; everything above is untouched by the band.  Q = 0: no band.
 constexpr int SC_FILL = 8;
 __global__ void __launch_bounds__(SC_THREADS)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
-                 const unsigned char* __restrict__ flag, const LbmConst c) {
+                 const unsigned char* __restrict__ flag, const double* __restrict__ Alow,
+                 const int* __restrict__ bandp, int delta, const LbmConst c) {
+  const int Q = *bandp;
   const int i = blockIdx.x * SC_THREADS + threadIdx.x;
-  const int j = blockIdx.y;
+  const int j = blockIdx.y + (Q > 0 ? Q + delta : 0);
+  if (j >= c.ny) return;
   const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
+  if (j <= Q && Q > 0) {                       // the two rows along the seam (all fluid)
+    if (!fluid) return;
+    double f[9], g[5];
+    const RowsSeam R{A, Alow ? Alow : A, Q, Alow ? -1 : c.ny, c.px};
+    pull_boundary(R, c, i, j, f, g);
+    mrt_collide(f, g, c);
+    store_node(B, c, i, j < Q ? c.ny : j, f, g);
+    return;
+  }
   const unsigned m = __ballot_sync(0xffffffffu, fluid);
   if (fluid) {
     update_node(A, B, c, i, j);
@@ -141,36 +186,49 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   double* __restrict__ O = B + 2 * x;
 #pragma unroll
   for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
-  double* __restrict__ Q = B + 10 * c.ps + x;
+  double* __restrict__ Q4 = B + 10 * c.ps + x;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) Q[k * c.ps] = 0.0;
+  for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
 }
 
-// TWO time steps per pass for a particle-free lattice (traffic below 224 B per
+// TWO time steps per pass over particle-free rows (traffic below 224 B per
 // update).  A CTA owns a TB_X x TB_Y tile of output nodes.  Phase 1: its TB_W x TB_H threads
-// update the tile plus a one-node halo from A (the same pull + collide as the one-step kernel) and
-// keep the result f+(x, t+1), g+(x, t+1) in shared memory, population-major.  Phase 2: the tile's
-// nodes pull from shared memory (walls as in pull_boundary, on tile-local indices, so the periodic
-// wrap needs no arithmetic), collide again and store f+(x, t+2) to B.  Per two updates a node costs
-// (TB_W+2)(TB_H+2)/(TB_X TB_Y) = 1.46 reads and one write of its 112 B: 138 B per update instead
-// of 224 B (the halo re-reads hit L2: 111 B of DRAM traffic measured); the arithmetic is the one-step kernel's, so the result is the same bit for bit.
+// update the tile plus a one-node halo from the state at t (the same pull + collide as the
+// one-step kernel) and keep the result f+(x, t+1), g+(x, t+1) in shared memory, population-major.
+// Phase 2: the tile's nodes pull from shared memory (walls as in pull_boundary, on tile-local
+// indices, so the periodic wrap needs no arithmetic), collide again and store f+(x, t+2).  Per two
+// updates a node costs (TB_W+2)(TB_H+2)/(TB_X TB_Y) = 1.46 reads and one write of its 112 B:
+// 138 B per update instead of 224 B (the halo re-reads hit L2: 111 B of DRAM traffic measured);
+// the arithmetic is the one-step kernel's, so the result is the same bit for bit.
+//
+// The kernel updates the rows [0, Q), Q = *bandp (bandp == nullptr: the whole lattice, the
+// particle-free case).  Rows below Q are read from Aband, the rows Q and Q+1 the top tiles' halo
+// needs from Atop; the band is written to Bband.  Tile rows are dealt to `nparts` launches
+// (part = which of them this is), so that the band's work can be spread over the slots of the step
+// schedule in which the bounce-back kernel leaves the GPU's bandwidth idle.
 constexpr int TB_X = 30, TB_Y = 14;   // TB_W = 32: one warp per tile row
 constexpr int TB_W = TB_X + 2, TB_H = TB_Y + 2;
 constexpr int TB_THREADS = TB_W * TB_H;   // 512 = 16 warps
 constexpr int TB_SMEM = 14 * TB_THREADS * (int)sizeof(double);
 
 __global__ void __launch_bounds__(TB_THREADS)
-k_stream_collide_2step(const double* __restrict__ A, double* __restrict__ B, const LbmConst c) {
+k_stream_collide_2step(const double* __restrict__ Aband, const double* __restrict__ Atop,
+                       double* __restrict__ Bband, const int* __restrict__ bandp, int nparts,
+                       int part, const LbmConst c) {
   extern __shared__ double s_pop[];   // [14][TB_H][TB_W]
+  const int Q = bandp ? min(*bandp, c.ny) : c.ny;
+  const int tile_j0 = (blockIdx.y * nparts + part) * TB_Y;
+  if (tile_j0 >= Q) return;
   const int tx = threadIdx.x % TB_W, ty = threadIdx.x / TB_W;
-  const int i = blockIdx.x * TB_X - 1 + tx, j = blockIdx.y * TB_Y - 1 + ty;
+  const int i = blockIdx.x * TB_X - 1 + tx, j = tile_j0 - 1 + ty;
   // phase 1: node (i, j) of the halo'd tile, wrapped in x when periodic
   int iw = i;
   if (c.periodic_x) iw = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i);
-  const bool exists = iw >= 0 && iw < c.nx && j >= 0 && j < c.ny;
+  const bool exists = iw >= 0 && iw < c.nx && j >= 0 && j < c.ny && j <= Q;
   double f[9], g[5];
   if (exists) {
-    pull_node(A, c, iw, j, f, g);
+    if (j + 1 < Q || Q == c.ny) pull_node(Aband, c, iw, j, f, g);
+    else pull_boundary(RowsSeam{Atop, Aband, Q, -1, c.px}, c, iw, j, f, g);   // rows Q-1, Q (warp-uniform)
     mrt_collide(f, g, c);
 #pragma unroll
     for (int k = 0; k < 9; ++k) s_pop[k * TB_THREADS + threadIdx.x] = f[k];
@@ -179,7 +237,7 @@ k_stream_collide_2step(const double* __restrict__ A, double* __restrict__ B, con
   }
   __syncthreads();
   // phase 2: the tile's own nodes
-  if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= c.ny) return;
+  if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= Q) return;
   if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
     // interior: every upstream neighbour is a node of the tile's halo'd image
     const double* __restrict__ S = s_pop + threadIdx.x;
@@ -210,7 +268,7 @@ k_stream_collide_2step(const double* __restrict__ A, double* __restrict__ B, con
     }
   }
   mrt_collide(f, g, c);
-  store_node(B, c, i, j, f, g);
+  store_node(Bband, c, i, j, f, g);
 }
 
 // first step only: A holds the PRE-collision initial state f(x,0); collide it (in place when
@@ -324,10 +382,13 @@ inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1
 
 } // namespace
 
-void launch_stream_collide(lbm* h) {
+// band == 0: the plain step (every row).  band == 1 / 2: first / second step of a pair of the
+// banded schedule (lbm_capi.cu): rows from *h->band - 1 resp. *h->band up; low = the band's copy
+// (first step only).
+void launch_stream_collide(lbm* h, int band, const double* low) {
   h->launches++;
   k_stream_collide<<<grid_rows(h->px, h->ny, SC_THREADS), SC_THREADS, 0, h->stream>>>(
-      h->A, h->B, h->flag, h->C);
+      h->A, h->B, h->flag, band == 1 ? low : nullptr, band ? h->band : h->band + 1, band == 1 ? -1 : 0, h->C);
 }
 
 int stream_collide_configure() {
@@ -335,10 +396,21 @@ int stream_collide_configure() {
                               TB_SMEM) == cudaSuccess ? 0 : -1;
 }
 
+// particle-free lattice: every row, A -> B
 void launch_stream_collide_2step(lbm* h) {
   h->launches++;
   const dim3 grid((h->nx + TB_X - 1) / TB_X, (h->ny + TB_Y - 1) / TB_Y);
-  k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(h->A, h->B, h->C);
+  k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(h->A, h->A, h->B, nullptr, 1, 0, h->C);
+}
+
+// the band rows [0, *h->band) of a lattice with particles: tile rows part, part + nparts, ...
+void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
+                                int nparts, int part) {
+  h->launches++;
+  const int tile_rows = (h->ny + TB_Y - 1) / TB_Y;
+  const dim3 grid((h->nx + TB_X - 1) / TB_X, (tile_rows - part + nparts - 1) / nparts);
+  k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(src_band, src_top, dst_band, h->band,
+                                                                   nparts, part, h->C);
 }
 
 void launch_init_collide(lbm* h, double* dst) {

@@ -2,12 +2,14 @@
 (Simulation.from_workload(config(k)), lbm_step on the current torch stream).
 
 * configs 1 and 2: the full 100-step parity horizon against the oracle (SURVEY 8(c) protocol).
-* config 3 (the benched workload): links bit-exact on the full 4,800-particle set, full-field and
-  particle parity over a short horizon the oracle can afford (3.6 s per step), and a sampled
-  one-step check deep into the run: for sampled nodes the oracle's per-node collision is applied
-  to the populations pulled from the GPU state at step s and compared with the GPU state at s+1.
-* config 4 (8192^2, 20,000 particles): links bit-exact, flag map against an independent numpy
-  rasterisation of the discs, 2-step macroscopic + particle parity, sampled one-step check.
+* config 3 (the benched workload): flag map against an independent numpy rasterisation, a sampled
+  one-step check deep into the run (for sampled nodes the oracle's per-node collision is applied
+  to the populations pulled from the GPU state at step s and compared with the GPU state at s+1),
+  307 steps of incremental flag updates against a from-scratch rasterisation, final links against
+  the oracle's link builder.  The 100-step parity (populations included) and the injected-state
+  coupling check are in tests/test_gpu_protocol_horizon.py.
+* config 4 (8192^2, 20,000 particles): flag map against an independent numpy rasterisation,
+  sampled one-step check; 20-step parity with populations in tests/test_gpu_protocol_horizon.py.
 """
 import numpy as np
 import pytest
@@ -113,18 +115,11 @@ def test_config3_full_size(gpu, ob, wl):
     if host_gb_free() < 24:
         pytest.skip("needs ~20 GB of host memory for the oracle's 4000^2 arrays")
     w = wl.config(3)
-    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
-    Lg = g.links()
-    assert_links_equal(Lg, o.links())
-    assert len(Lg["q"]) > 4800 * 150
+    g = gpu.Simulation.from_workload(w)
+    assert len(g.links()["q"]) > 4800 * 150
     assert np.array_equal(g.fields()["flag"], numpy_flags(w))
-    g.step(6)
-    o.step(6)
-    assert_fields_close(g.fields(populations=True), o.fields(populations=True))
-    assert_particles_close(g.particles(), o.particles(), r_min=10.0, steps=6)
-    del o
     # deep into the run, in bench.py's regime
-    g.step(300)
+    g.step(306)
     assert sampled_one_step_check(g, ob, w, 1500) == 1500
     p = g.particles()
     assert all(np.isfinite(v).all() for v in p.values())
@@ -140,18 +135,12 @@ def test_config3_full_size(gpu, ob, wl):
 
 
 def test_config4_full_size(gpu, ob, wl):
-    if host_gb_free() < 90:
-        pytest.skip("needs ~70 GB of host memory for the oracle's 8192^2 arrays")
+    if host_gb_free() < 60:
+        pytest.skip("needs host memory for two read-outs of the 8192^2 populations")
     w = wl.config(4)
-    g, o = gpu.Simulation.from_workload(w), ob.OracleSim.from_workload(w)
-    assert_links_equal(g.links(), o.links())
+    g = gpu.Simulation.from_workload(w)
     assert np.array_equal(g.fields()["flag"], numpy_flags(w))
-    g.step(2)
-    o.step(2)
-    assert_fields_close(g.fields(), o.fields(), populations=False)
-    assert_particles_close(g.particles(), o.particles(), r_min=6.0, steps=2)
-    del o
-    g.step(50)
+    g.step(52)
     assert sampled_one_step_check(g, ob, w, 800) == 800
 
 

@@ -508,6 +508,73 @@ def test_graph_replay_equals_direct_launches_bitwise(gpu, wl):
         assert_same_bits(c, b)
 
 
+def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
+    """Lattices with particles advance the particle-free rows below the lowest particle two steps
+    per pass (lbm_set_band; periods of four steps, the band height chosen on the device at the
+    start of each period).  The arithmetic per node and step is unchanged, so every fluid
+    population and particle state must equal the plain schedule's bit for bit: through graph
+    replays and direct launches, overlapped and sequential, for step counts that are not multiples
+    of the period, while a fast particle falls into the band's rows (the band shrinks from period
+    to period) and ends up too close to the floor for any band."""
+    w = wl.sedimentation(333, 420, 16, seed=5, y_frac_lo=0.55, d_lo=12.0, d_hi=22.0, name="band")
+    n = w.n_particles
+    uy = np.zeros(n)
+    k = int(np.argmin(w.particles["y"]))
+    uy[k] = -0.12                                    # one particle dives through the free rows
+    w.particles.update(ux=np.zeros(n), uy=uy, omega=np.zeros(n))
+    ref = gpu.Simulation.from_workload(w)
+    ref.set_band(False)
+    ref.set_graph(False)
+    sims = [gpu.Simulation.from_workload(w) for _ in range(3)]
+    sims[1].set_graph(False)                         # direct launches (the profiling path)
+    sims[2].set_overlap(False)                       # one stream
+    q_seen = []
+    for nst in (1, 4, 8, 3, 29, 64, 402, 7, 1500):
+        ref.step(nst)
+        for s_ in sims:
+            s_.step(nst)
+            assert_same_bits(s_, ref)
+        q_seen.append(sims[0].band_rows())
+        assert sims[1].band_rows() == q_seen[-1] or nst < 4
+    assert ref.band_rows() == 0
+    assert max(q_seen) > 150                         # a real band at the start ...
+    live = [q for q in q_seen if q > 0]
+    assert live == sorted(live, reverse=True) and len(set(live)) > 2   # ... that shrinks
+    # a particle that starts just above the smallest band worth having and falls: the band is
+    # given up (Q = 0) within a few periods and the plain schedule carries on
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=1,
+             max_links_per_particle=wl.max_links_for_diameter(14.0))
+    parts = dict(x=np.array([60.4]), y=np.array([47.0]), diam=np.array([14.0]),
+                 rho_ratio=np.array([1.5]), T_w=np.array([1.0]), ux=np.array([0.0]),
+                 uy=np.array([-0.05]), omega=np.array([0.0]))
+    w2 = wl.Workload("band_vanishes", 120, 150, p, 1, 1, particles=parts)
+    a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
+    b.set_band(False)
+    qs = []
+    for nst in (4, 4, 8, 16, 40, 200):
+        a.step(nst)
+        b.step(nst)
+        assert_same_bits(a, b)
+        qs.append(a.band_rows())
+    assert qs[0] >= 28 and qs[-1] == 0, qs
+
+
+def test_two_step_band_periodic_and_wall_types(gpu, ob, wl):
+    """The band next to every kind of cavity wall (Dirichlet floor, adiabatic and periodic sides,
+    body force) against the oracle."""
+    for periodic in (0, 1):
+        p = wl.default_params()
+        p.update(g=1.6e-4, gbeta=1e-5, body_ax=1e-6, periodic_x=periodic,
+                 wall_T_type=[0, 0, 1, 1], wall_T=[0.0, 0.0, 0.7, 0.1], max_particles=2,
+                 max_links_per_particle=wl.max_links_for_diameter(16.0))
+        parts = dict(x=np.array([40.3, 77.0]), y=np.array([150.2, 139.0]), diam=np.array([16.0, 12.5]),
+                     rho_ratio=np.array([1.5, 1.3]), T_w=np.array([1.0, 0.4]))
+        w = wl.Workload("band_walls", 131, 181, p, 60, 60, particles=parts)
+        g, o, _ = run_and_compare(gpu, ob, w, [60], r_min=6.0)
+        assert g.band_rows() > 100
+
+
 def dense_pack(wl, n_side=10, d=12.0, gap=1.95, big=True):
     """A hexagonal pack of d = 12 discs at surface gap 1.95 (every disc has six neighbours just
     inside the repulsion range s = 2) next to one d = 30 disc, which makes the repulsion cells 32
