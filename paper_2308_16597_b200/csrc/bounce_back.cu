@@ -306,16 +306,10 @@ __global__ void k_refill_commit(double* __restrict__ B, const double* __restrict
 
 } // namespace
 
-// ctas_per_sm > 0: that many persistent CTAs per SM instead of one CTA per particle.  The kernel
-// is bound by scattered sector requests, not by occupancy, so in the
-// banded schedule it runs at half its occupancy and leaves the other half of every SM to the
-// band's two-step kernel, which is launched beside it.
-void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl, int ctas_per_sm) {
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
-  int grid = h->np;
-  if (ctas_per_sm > 0 && grid > ctas_per_sm * h->sm_count) grid = ctas_per_sm * h->sm_count;
-  launch_k(k_bounce_back, dim3(grid), dim3(BT), 0, st, pdl, h->A, h->la, h->pa, h->cur, h->np,
+  launch_k(k_bounce_back, dim3(h->np), dim3(BT), 0, st, pdl, h->A, h->la, h->pa, h->cur, h->np,
            h->chain_ctas > 0 ? 0 : 1, h->C);
 }
 

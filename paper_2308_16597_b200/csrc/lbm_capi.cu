@@ -216,6 +216,15 @@ struct Timed {
     }
   }
   ~Timed() {
+    static const int dbg = getenv("LBM_DEBUG_SYNC") ? atoi(getenv("LBM_DEBUG_SYNC")) : 0;
+    if (dbg) {
+      cudaError_t e = cudaDeviceSynchronize();
+      if (e != cudaSuccess) {
+        fprintf(stderr, "[lbm debug] %s failed at step %lld: %s\n", kKernelNames[k], h->steps_done, cudaGetErrorString(e));
+        fflush(stderr);
+        abort();
+      }
+    }
     if (on) {
       cudaEventRecord(h->ev1[k][h->ev_n[k]], st);
       h->ev_n[k]++;
@@ -367,14 +376,17 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   cudaMemsetAsync(h->owner, 0x7f, nn * sizeof(int), h->stream);   // OWNER_NONE = 0x7f7f7f7f
   cudaMemsetAsync(h->status_dev, 0, sizeof(int), h->stream);
   cudaMemsetAsync(h->band, 0, 2 * sizeof(int), h->stream);
+  cudaMemsetAsync(h->newborn_count, 0, 2 * sizeof(int), h->stream);
   h->status_host[1] = 0;
   {
     const char* eb = getenv("LBM_BAND");
     h->band_on = (eb && atoi(eb) == 0) ? 0 : 1;
-    const char* ec = getenv("LBM_BAND_BB_CTAS");
-    h->band_bb_ctas = ec ? atoi(ec) : 4;
+    if (cudaEventCreateWithFlags(&h->ev_p2, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      h->band_on = 0;
+      h->ev_p2 = nullptr;
+    }
   }
-  cudaMemsetAsync(h->newborn_count, 0, 2 * sizeof(int), h->stream);
   for (int b = 0; b < 2; ++b)
     if (h->max_cells) cudaMemsetAsync(h->cell_count[b], 0, sizeof(int) * (size_t)h->max_cells, h->stream);
   cudaMemsetAsync(h->B, 0, sizeof(double) * 14 * (size_t)h->ps, h->stream);
@@ -617,13 +629,19 @@ static void enqueue_step(lbm* h, int phase) {
     }
   }
   if (h->np > 0) {
-    { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h, S1, pdl, (banded && fork) ? h->band_bb_ctas : 0); }
+    { Timed tm(h, K_BOUNCE_BACK, S1); launch_bounce_back(h, S1, pdl); }
     note_chain_node(h, S1);
     if (fork) cudaEventRecord(h->ev_bb, S1);
   }
   if (banded) {
-    Timed tm(h, K_STREAM_COLLIDE_2STEP, S0);
-    launch_stream_collide_band(h, band_src, X, band_dst, 2, phase & 1);
+    { Timed tm(h, K_STREAM_COLLIDE_2STEP, S0); launch_stream_collide_band(h, band_src, X, band_dst, 2, phase & 1); }
+    // the particle chain holds register space the band kernel's large CTAs need (measured: the band
+    // part takes 115 us beside the bounce-back kernel alone, 190 us beside the chain): the chain
+    // starts after the band's part and still has the whole one-step kernel to hide under
+    if (fork) {
+      cudaEventRecord(h->ev_p2, S0);
+      cudaStreamWaitEvent(S1, h->ev_p2, 0);
+    }
   }
   if (h->np > 0 && fork) cudaStreamWaitEvent(S0, h->ev_bb, 0);
   const int lattice_mode = banded ? ((phase & 1) ? 2 : 1) : 0;
@@ -686,7 +704,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   for (int k = 0; k < h->n_graphs; ++k) {
     lbm::StepGraph& g = h->graphs[k];
     if (g.A == h->A && g.cur == h->cur && g.steps == steps && g.overlap == h->overlap &&
-        g.chain_ctas == h->chain_ctas && g.banded == banded)
+        g.chain_ctas == h->chain_ctas && g.banded == banded && (!banded || g.band_hint == h->band_hint))
       return &g;
   }
   if (h->n_graphs == LBM_MAX_GRAPHS) drop_graphs(h);
@@ -746,6 +764,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   g.overlap = h->overlap;
   g.chain_ctas = h->chain_ctas;
   g.banded = banded;
+  g.band_hint = h->band_hint;
   g.launches = per;
   return &g;
 }
@@ -761,6 +780,9 @@ int lbm_step(lbm_t* h, int nsteps) {
   int s = 0;
   // the banded schedule needs the particle-free two-step kernel and runs in periods of four steps
   const bool band_ok = h->np > 0 && h->band_on && h->two_step_ok;
+  // grid of the one-step kernel in banded steps: the band height at the end of the previous call
+  // less a margin, in steps of 64 rows (each value is its own graph)
+  h->band_hint = band_ok ? std::max(0, ((h->status_host[1] - 96) / 64) * 64) : 0;
   // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
   // launch while that many remain, then 4 if banded, then 2), the odd last step directly; event
   // profiling needs the direct launches
@@ -985,6 +1007,7 @@ int lbm_destroy(lbm_t* h) {
   cudaStreamSynchronize(h->stream);
   drop_graphs(h);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->ev_p2) cudaEventDestroy(h->ev_p2);
   if (h->chain_own) {
     cudaStreamSynchronize(h->chain_own);
     cudaStreamDestroy(h->chain_own);

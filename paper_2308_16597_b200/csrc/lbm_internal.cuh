@@ -125,8 +125,9 @@ struct lbm {
   // two-step band: band[0] = Q, rows
   // [0, Q) are advanced two steps per pass; band[1] = 0 (what the plain schedule's kernels read)
   int* band;
+  int band_hint;             // rows certainly inside the band as the host last saw it (sizes the one-step grid; 0 = unknown)
   int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
-  int band_bb_ctas;          // bounce-back CTAs per SM beside the band kernel (LBM_BAND_BB_CTAS; 0 = one per particle)
+  cudaEvent_t ev_p2;         // the band kernel's part of a step has been issued (the particle chain follows it)
   cudaEvent_t ev_plan, ev_l1;
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
   long long steps_done;
@@ -145,7 +146,7 @@ struct lbm {
   struct StepGraph {
     cudaGraphExec_t exec;
     const double* A;         // phase the graph was captured in
-    int cur, steps, overlap, chain_ctas, banded;
+    int cur, steps, overlap, chain_ctas, banded, band_hint;
     long long launches;      // kernels per replay
   } graphs[LBM_MAX_GRAPHS];
   int n_graphs;
@@ -205,6 +206,6 @@ int particles_configure(lbm* h);           // per-handle kernel attributes (0 = 
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
 void launch_band_plan(lbm* h, cudaStream_t st);   // h->band[0] from the positions of buffer h->cur
 // bounce_back.cu
-void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl, int ctas_per_sm);
+void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl);
 void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped
 void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl);  // stash -> B, newborn flags cleared

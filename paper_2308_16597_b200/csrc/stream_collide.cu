@@ -156,39 +156,43 @@ __device__ __forceinline__ void update_node(const double* __restrict__ A, double
 // (delta = 0, Alow = nullptr) row Q-1 is read from the spare row of A.  Rows Q-1 and Q take the
 // generic pull; everything above is untouched by the band.  Q = 0: no band.
 constexpr int SC_FILL = 8;
-__global__ void __launch_bounds__(SC_THREADS)
+__global__ void __launch_bounds__(SC_THREADS, 9)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
                  const unsigned char* __restrict__ flag, const double* __restrict__ Alow,
                  const int* __restrict__ bandp, int delta, const LbmConst c) {
   const int Q = *bandp;
   const int i = blockIdx.x * SC_THREADS + threadIdx.x;
-  const int j = blockIdx.y + (Q > 0 ? Q + delta : 0);
-  if (j >= c.ny) return;
-  const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
-  if (j <= Q && Q > 0) {                       // the two rows along the seam (all fluid)
-    if (!fluid) return;
-    double f[9], g[5];
-    const RowsSeam R{A, Alow ? Alow : A, Q, Alow ? -1 : c.ny, c.px};
-    pull_boundary(R, c, i, j, f, g);
-    mrt_collide(f, g, c);
-    store_node(B, c, i, j < Q ? c.ny : j, f, g);
-    return;
-  }
-  const unsigned m = __ballot_sync(0xffffffffu, fluid);
-  if (fluid) {
-    update_node(A, B, c, i, j);
-    return;
-  }
-  const unsigned lane = threadIdx.x & 31u;
-  const unsigned grp = (m >> (lane & ~(unsigned)(SC_FILL - 1))) & ((1u << SC_FILL) - 1u);
-  if (grp == 0u || i >= c.px) return;
-  const long long x = (long long)j * c.px + i;
-  double* __restrict__ O = B + 2 * x;
+  // The grid has one CTA row per lattice row the host EXPECTS this launch to cover (it knows the
+  // band height of the previous lbm_step call); the loop takes care of a band that has shrunk
+  // since (normally it runs once).
+  for (int j = blockIdx.y + (Q > 0 ? Q + delta : 0); j < c.ny; j += gridDim.y) {
+    const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
+    if (j <= Q && Q > 0) {                       // the two rows along the seam (all fluid)
+      if (fluid) {
+        double f[9], g[5];
+        const RowsSeam R{A, Alow ? Alow : A, Q, Alow ? -1 : c.ny, c.px};
+        pull_boundary(R, c, i, j, f, g);
+        mrt_collide(f, g, c);
+        store_node(B, c, i, j < Q ? c.ny : j, f, g);
+      }
+      continue;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, fluid);
+    if (fluid) {
+      update_node(A, B, c, i, j);
+      continue;
+    }
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned grp = (m >> (lane & ~(unsigned)(SC_FILL - 1))) & ((1u << SC_FILL) - 1u);
+    if (grp == 0u || i >= c.px) continue;
+    const long long x = (long long)j * c.px + i;
+    double* __restrict__ O = B + 2 * x;
 #pragma unroll
-  for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
-  double* __restrict__ Q4 = B + 10 * c.ps + x;
+    for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
+    double* __restrict__ Q4 = B + 10 * c.ps + x;
 #pragma unroll
-  for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
+    for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
+  }
 }
 
 // TWO time steps per pass over particle-free rows (traffic below 224 B per
@@ -203,9 +207,9 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
 //
 // The kernel updates the rows [0, Q), Q = *bandp (bandp == nullptr: the whole lattice, the
 // particle-free case).  Rows below Q are read from Aband, the rows Q and Q+1 the top tiles' halo
-// needs from Atop; the band is written to Bband.  Tile rows are dealt to `nparts` launches
-// (part = which of them this is), so that the band's work can be spread over the slots of the step
-// schedule in which the bounce-back kernel leaves the GPU's bandwidth idle.
+// needs from Atop; the band is written to Bband.  The tile rows are split into `nparts` contiguous
+// shares, one per launch (part = which of them this is), so that the band's work can be spread
+// over the steps of the pair it advances.
 constexpr int TB_X = 30, TB_Y = 14;   // TB_W = 32: one warp per tile row
 constexpr int TB_W = TB_X + 2, TB_H = TB_Y + 2;
 constexpr int TB_THREADS = TB_W * TB_H;   // 512 = 16 warps
@@ -217,7 +221,11 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
                        int part, const LbmConst c) {
   extern __shared__ double s_pop[];   // [14][TB_H][TB_W]
   const int Q = bandp ? min(*bandp, c.ny) : c.ny;
-  const int tile_j0 = (blockIdx.y * nparts + part) * TB_Y;
+  // part p owns the p-th contiguous share of the band's tile rows (neighbouring tile rows of one
+  // launch share their halo rows through L2)
+  const int per_part = ((Q + TB_Y - 1) / TB_Y + nparts - 1) / nparts;
+  if ((int)blockIdx.y >= per_part) return;
+  const int tile_j0 = (part * per_part + blockIdx.y) * TB_Y;
   if (tile_j0 >= Q) return;
   const int tx = threadIdx.x % TB_W, ty = threadIdx.x / TB_W;
   const int i = blockIdx.x * TB_X - 1 + tx, j = tile_j0 - 1 + ty;
@@ -387,7 +395,10 @@ inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1
 // (first step only).
 void launch_stream_collide(lbm* h, int band, const double* low) {
   h->launches++;
-  k_stream_collide<<<grid_rows(h->px, h->ny, SC_THREADS), SC_THREADS, 0, h->stream>>>(
+  // banded steps: one CTA row per lattice row above the band as the host last saw it
+  // (h->band_hint, 0 = unknown); the kernel's row loop covers whatever the band has lost since
+  const int rows = band ? h->ny - h->band_hint : h->ny;
+  k_stream_collide<<<grid_rows(h->px, rows, SC_THREADS), SC_THREADS, 0, h->stream>>>(
       h->A, h->B, h->flag, band == 1 ? low : nullptr, band ? h->band : h->band + 1, band == 1 ? -1 : 0, h->C);
 }
 
@@ -403,12 +414,12 @@ void launch_stream_collide_2step(lbm* h) {
   k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(h->A, h->A, h->B, nullptr, 1, 0, h->C);
 }
 
-// the band rows [0, *h->band) of a lattice with particles: tile rows part, part + nparts, ...
+// the band rows [0, *h->band) of a lattice with particles: the part-th of nparts contiguous shares
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part) {
   h->launches++;
   const int tile_rows = (h->ny + TB_Y - 1) / TB_Y;
-  const dim3 grid((h->nx + TB_X - 1) / TB_X, (tile_rows - part + nparts - 1) / nparts);
+  const dim3 grid((h->nx + TB_X - 1) / TB_X, (tile_rows + nparts - 1) / nparts);
   k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(src_band, src_top, dst_band, h->band,
                                                                    nparts, part, h->C);
 }

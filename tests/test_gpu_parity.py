@@ -575,6 +575,32 @@ def test_two_step_band_periodic_and_wall_types(gpu, ob, wl):
         assert g.band_rows() > 100
 
 
+def test_results_do_not_depend_on_what_the_workspace_held_before(gpu, wl, monkeypatch):
+    """The caller's workspace is arbitrary memory (PyTorch hands freed blocks out again, with the
+    previous simulation's populations still in them): every array the path reads must have been
+    initialised by the library.  Three workspaces pre-filled with 0x00, 0xFF and 0x3F bytes (the
+    last reads as large positive ints and as doubles of order 5e-4) must give identical bits."""
+    import torch
+    w = wl.sedimentation(260, 300, 10, seed=13, y_frac_lo=0.45, d_lo=12.0, d_hi=20.0, name="poison")
+    real_empty = torch.empty
+    sims = []
+    for fill in (0x00, 0xFF, 0x3F):
+        def filled(*a, fill=fill, **kw):
+            t = real_empty(*a, **kw)
+            if kw.get("dtype") == torch.uint8 and t.is_cuda:
+                t.fill_(fill)
+            return t
+        monkeypatch.setattr(torch, "empty", filled)
+        sims.append(gpu.Simulation.from_workload(w))
+    monkeypatch.setattr(torch, "empty", real_empty)
+    for n in (1, 8, 31):
+        for s_ in sims:
+            s_.step(n)
+        assert_same_bits(sims[1], sims[0])
+        assert_same_bits(sims[2], sims[0])
+    assert sims[0].band_rows() > 50
+
+
 def dense_pack(wl, n_side=10, d=12.0, gap=1.95, big=True):
     """A hexagonal pack of d = 12 discs at surface gap 1.95 (every disc has six neighbours just
     inside the repulsion range s = 2) next to one d = 30 disc, which makes the repulsion cells 32
