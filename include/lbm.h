@@ -141,8 +141,9 @@ int lbm_set_two_step(lbm_t* h, int on);
 
 /* on = 1 (default; LBM_BAND=0 turns the default off): lattices WITH particles also use the
  * two-steps-per-pass kernel, on the particle-free rows [0, Q) below the lowest particle (SURVEY
- * 8(f)-4).  In periods of four time steps a
- * device kernel picks Q from the particle positions and speeds (far enough below the lowest
+ * 8(f)-4), in lbm_step calls of at least 16
+ * steps (such a call plans the band once on entry to size its grids: one more synchronisation).
+ * In periods of four time steps a device kernel picks Q from the particle positions and speeds (far enough below the lowest
  * particle that no link or refill stencil reaches the band within the period; fewer than 28 free
  * rows: no band), the band is advanced t -> t+2 -> t+4 by the two-step kernel while the rows
  * above it take four ordinary steps, the two meeting in one row that is computed by both.  The

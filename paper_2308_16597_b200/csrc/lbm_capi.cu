@@ -40,6 +40,7 @@ int fail(lbm* h, int code, const char* fmt, ...) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+constexpr int LBM_BAND_MIN_STEPS = 16;   // shortest lbm_step call that uses the two-step band
 constexpr int LBM_GRAPH_STEPS = 8;   // time steps per graph launch (an even number: one or more periods)
 
 // Every entry point runs on the device the handle was created on, whatever device is current in
@@ -242,6 +243,7 @@ int check_status(lbm* h) {
   if (st & ST_LINK_OVERFLOW) return fail(h, LBM_E_CAPACITY, "a particle has more links than max_links_per_particle");
   if (st & ST_CELL_OVERFLOW) return fail(h, LBM_E_CAPACITY, "more than %d particle centres in one repulsion cell", CELL_CAP);
   if (st & ST_NEWBORN_OVERFLOW) return fail(h, LBM_E_CAPACITY, "newborn-node list overflow");
+  if (st & ST_BAND_REACHED) return fail(h, LBM_E_STATE, "a particle came within 4 rows of the two-step band (lbm_set_band(h, 0) runs without it)");
   return LBM_OK;
 }
 
@@ -610,17 +612,18 @@ static void note_chain_node(lbm* h, cudaStream_t S1) {
 // memory system idle.  The one-step kernel of the first step of a pair also updates row Q-1 (into
 // the spare row of its output copy), which the second step reads there; the band's part of a pair
 // is complete before the second step's one-step kernel overwrites the rows Q, Q+1 of X it reads.
-static void enqueue_step(lbm* h, int phase) {
+static void enqueue_step(lbm* h, int phase, bool plan = true) {
   cudaStream_t S0 = h->stream, S1 = h->chain, S2 = h->side;
   const bool fork = S1 != S0;
   const bool pdl = h->use_pdl != 0;
   const bool banded = phase >= 0;
+  h->band_live = banded ? 1 : 0;
   const int sp = h->cur;   // step parity: which newborn counter / repulsion grid this step uses
   double* X = (phase & 1) ? h->B : h->A;   // the copies as they were named at the start of the period
   double* Y = (phase & 1) ? h->A : h->B;
   const double* band_src = phase < 2 ? X : Y;
   double* band_dst = phase < 2 ? Y : X;
-  if (banded && phase == 0) {
+  if (banded && phase == 0 && plan) {   // one plan serves two periods (k_band_plan allows for 8 steps of motion)
     { Timed tm(h, K_BAND_PLAN, S1); launch_band_plan(h, S1); }
     note_chain_node(h, S1);
     if (fork) {
@@ -704,7 +707,8 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   for (int k = 0; k < h->n_graphs; ++k) {
     lbm::StepGraph& g = h->graphs[k];
     if (g.A == h->A && g.cur == h->cur && g.steps == steps && g.overlap == h->overlap &&
-        g.chain_ctas == h->chain_ctas && g.banded == banded && (!banded || g.band_hint == h->band_hint))
+        g.chain_ctas == h->chain_ctas && g.banded == banded &&
+        (!banded || (g.band_hint == h->band_hint && g.band_cap == h->band_cap)))
       return &g;
   }
   if (h->n_graphs == LBM_MAX_GRAPHS) drop_graphs(h);
@@ -721,7 +725,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   if (e == cudaSuccess) {
     if (h->chain != h->stream) h->cap_nodes = &chain_nodes;
     join_in(h);
-    for (int s = 0; s < steps; ++s) enqueue_step(h, banded ? s % 4 : -1);
+    for (int s = 0; s < steps; ++s) enqueue_step(h, banded ? s % 4 : -1, s == 0);
     join_out(h);
     h->cap_nodes = nullptr;
     e = cudaStreamEndCapture(h->cap_stream, &graph);
@@ -765,6 +769,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   g.chain_ctas = h->chain_ctas;
   g.banded = banded;
   g.band_hint = h->band_hint;
+  g.band_cap = h->band_cap;
   g.launches = per;
   return &g;
 }
@@ -778,11 +783,28 @@ int lbm_step(lbm_t* h, int nsteps) {
     ensure_links(h);
   }
   int s = 0;
-  // the banded schedule needs the particle-free two-step kernel and runs in periods of four steps
-  const bool band_ok = h->np > 0 && h->band_on && h->two_step_ok;
-  // grid of the one-step kernel in banded steps: the band height at the end of the previous call
-  // less a margin, in steps of 64 rows (each value is its own graph)
-  h->band_hint = band_ok ? std::max(0, ((h->status_host[1] - 96) / 64) * 64) : 0;
+  // The banded schedule needs the particle-free two-step kernel, runs in periods of four steps and
+  // is worth one extra synchronisation per call only for calls of some length: the band is planned
+  // once here, on the caller's stream, so that the host can size the grids -- the one-step kernel
+  // gets one CTA row per lattice row above (the planned band less a margin, in steps of 32 rows),
+  // the band kernel's grid covers (the planned band plus a margin, in steps of 16 rows); each pair
+  // of values is its own graph.  The per-period plans on the device stay below the cap; a band that shrinks faster than
+  // the margin is caught by the one-step kernel's row loop.
+  bool band_ok = h->np > 0 && h->band_on && h->two_step_ok && nsteps >= LBM_BAND_MIN_STEPS;
+  if (band_ok) {
+    h->band_cap = h->ny;
+    launch_band_plan(h, h->stream);
+    CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaStreamSynchronize(h->stream));
+    const int q0 = h->status_host[1];
+    if (q0 <= 0) band_ok = false;
+    else {
+      const char* eh = getenv("LBM_HINT_SLACK");
+      const int hs = eh ? atoi(eh) : 96, hq = hs >= 64 ? 64 : 32;
+      h->band_hint = std::max(0, ((q0 - hs) / hq) * hq);
+      h->band_cap = std::min(h->ny, ((q0 + 8 + 15) / 16) * 16);
+    }
+  }
   // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
   // launch while that many remain, then 4 if banded, then 2), the odd last step directly; event
   // profiling needs the direct launches
@@ -801,6 +823,7 @@ int lbm_step(lbm_t* h, int nsteps) {
   }
   if (s < nsteps) join_in(h);
   const bool direct = s < nsteps;
+  int direct_periods = 0;   // a band plan serves two periods
   while (s < nsteps) {
     if (h->np == 0 && h->two_step && nsteps - s >= 2) {
       // particle-free lattice: two time steps per pass over the populations (A -> B)
@@ -811,7 +834,8 @@ int lbm_step(lbm_t* h, int nsteps) {
       continue;
     }
     if (band_ok && nsteps - s >= 4) {
-      for (int ph = 0; ph < 4; ++ph) enqueue_step(h, ph);
+      for (int ph = 0; ph < 4; ++ph) enqueue_step(h, ph, (direct_periods & 1) == 0);
+      ++direct_periods;
       h->steps_done += 4;
       s += 4;
       continue;

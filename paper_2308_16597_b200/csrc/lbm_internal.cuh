@@ -28,6 +28,7 @@
 #define ST_LINK_OVERFLOW 2
 #define ST_CELL_OVERFLOW 4
 #define ST_NEWBORN_OVERFLOW 8
+#define ST_BAND_REACHED 16
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_MOVE, K_COVER, K_REFILL,
@@ -126,6 +127,8 @@ struct lbm {
   // [0, Q) are advanced two steps per pass; band[1] = 0 (what the plain schedule's kernels read)
   int* band;
   int band_hint;             // rows certainly inside the band as the host last saw it (sizes the one-step grid; 0 = unknown)
+  int band_live;             // the step being enqueued belongs to a banded period (k_cover checks the margin)
+  int band_cap;              // most rows the band may have in this call (sizes the band kernel's grid)
   int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
   cudaEvent_t ev_p2;         // the band kernel's part of a step has been issued (the particle chain follows it)
   cudaEvent_t ev_plan, ev_l1;
@@ -146,7 +149,7 @@ struct lbm {
   struct StepGraph {
     cudaGraphExec_t exec;
     const double* A;         // phase the graph was captured in
-    int cur, steps, overlap, chain_ctas, banded, band_hint;
+    int cur, steps, overlap, chain_ctas, banded, band_hint, band_cap;
     long long launches;      // kernels per replay
   } graphs[LBM_MAX_GRAPHS];
   int n_graphs;

@@ -662,13 +662,18 @@ template <bool ELL>
 __global__ void __launch_bounds__(PT)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
-        int* __restrict__ cell_items, int* __restrict__ status, int early, const LbmConst c) {
+        int* __restrict__ cell_items, int* __restrict__ status, const int* __restrict__ bandp,
+        int early, const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();
+  const int Q = *bandp;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const Shape Sn = load_shape<ELL>(pa, buf, p);
   const double xn = Sn.x, yn = Sn.y;
   if (threadIdx.x == 0) {
+    // safety net of the two-step band: no solid node within 4 rows of it (k_band_plan's margins
+    // make this unreachable for any |U|, dU the method is stable at)
+    if (Q > 0 && (int)floor(yn - Sn.r) < Q + 4) atomicOr(status, ST_BAND_REACHED);
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
     ci = min(max(ci, 0), ncx - 1);
     cj = min(max(cj, 0), ncy - 1);
@@ -698,15 +703,16 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
 // ------------------------------------------------------------------------------------------
 // Two-step band: the rows [0, Q) below the
 // lowest particle are advanced two time steps per pass by k_stream_collide_2step for the next
-// BAND_PERIOD steps.  Within those steps no solid node, no link stencil (x_f - 2 e_i) and no refill
+// BAND_PERIOD steps (two periods of the banded schedule).  Within those steps no solid node, no link stencil (x_f - 2 e_i) and no refill
 // stencil (x_new + 3 e_c and its upstream neighbours) may reach below row Q: with the lowest solid
 // row >= floor(min_p(y_p - r_p)) that needs Q + 4 <= lowest solid row, plus what the particle can
-// fall in BAND_PERIOD steps (its speed now, one node for its acceleration, one in reserve).
+// fall in BAND_PERIOD steps (its speed now, two nodes for its acceleration -- the stiffest
+// repulsion of Eq. 15 gives 32 a = 1.7 -- one in reserve); k_cover checks it every step.
 // A band of fewer than BAND_MIN rows is not worth its seam: Q = 0 (no band).  One CTA.
-constexpr int BAND_PERIOD = 4;
+constexpr int BAND_PERIOD = 8;
 constexpr int BAND_MIN = 28;
 __global__ void __launch_bounds__(1024)
-k_band_plan(ParticleArrays pa, int cur, int np, int ny, int* __restrict__ band) {
+k_band_plan(ParticleArrays pa, int cur, int np, int ny, int qcap, int* __restrict__ band) {
   __shared__ double s_min[32];
   double low = 1.0e300;
   for (int p = threadIdx.x; p < np; p += blockDim.x) {
@@ -720,8 +726,9 @@ k_band_plan(ParticleArrays pa, int cur, int np, int ny, int* __restrict__ band) 
   if (threadIdx.x == 0) {
     for (int w = 1; w < (int)(blockDim.x >> 5); ++w) low = fmin(low, s_min[w]);
     int Q = 0;
-    if (low == low && low < 1.0e9 && low > -1.0e9) Q = (int)floor(low) - 6;
+    if (low == low && low < 1.0e9 && low > -1.0e9) Q = (int)floor(low) - 7;
     if (Q > ny - 8) Q = ny - 8;
+    if (Q > qcap) Q = qcap;        // the band kernel's grid was sized for at most this many rows
     if (Q < BAND_MIN) Q = 0;
     band[0] = Q;
   }
@@ -800,12 +807,12 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   launch_k(h->n_ell ? k_cover<true> : k_cover<false>, dim3(chain_grid(h, h->np, st)), dim3(PT), 0, st, pdl,
            h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell, h->ncx, h->ncy,
            h->cell_count[which_buffer], h->cell_items[which_buffer], h->status_dev,
-           chain_early(h, st), h->C);
+           (const int*)(h->band_live ? h->band : h->band + 1), chain_early(h, st), h->C);
 }
 
 // rows [0, h->band[0]) of the next BAND_PERIOD steps go to the two-step kernel (positions of
 // buffer h->cur); a plain launch: it starts after everything before it in `st` has completed
 void launch_band_plan(lbm* h, cudaStream_t st) {
   h->launches++;
-  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band);
+  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_cap, h->band);
 }

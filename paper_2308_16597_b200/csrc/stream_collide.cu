@@ -12,6 +12,8 @@
 // kernel needs no link awareness.  Only the cavity walls are handled here: halfway bounce-back
 // f_k(x,t+1) = f+_kbar(x,t); thermal g_k(x,t+1) = -g+_kbar(x,t) + 2 w_k T_wall (Dirichlet) or
 // g+_kbar(x,t) (adiabatic)  (DESIGN.md readings; the paper only says "no-slip").
+#include <algorithm>
+
 #include "collide.cuh"
 
 namespace {
@@ -160,6 +162,10 @@ __global__ void __launch_bounds__(SC_THREADS, 9)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
                  const unsigned char* __restrict__ flag, const double* __restrict__ Alow,
                  const int* __restrict__ bandp, int delta, const LbmConst c) {
+  // programmatic dependent launch along the caller's stream: the next lattice kernel's CTAs may
+  // come up as this grid's last wave drains; every kernel waits here for its predecessor's data
+  pdl_launch_dependents();
+  pdl_wait();
   const int Q = *bandp;
   const int i = blockIdx.x * SC_THREADS + threadIdx.x;
   // The grid has one CTA row per lattice row the host EXPECTS this launch to cover (it knows the
@@ -220,6 +226,8 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
                        double* __restrict__ Bband, const int* __restrict__ bandp, int nparts,
                        int part, const LbmConst c) {
   extern __shared__ double s_pop[];   // [14][TB_H][TB_W]
+  pdl_launch_dependents();
+  pdl_wait();
   const int Q = bandp ? min(*bandp, c.ny) : c.ny;
   // part p owns the p-th contiguous share of the band's tile rows (neighbouring tile rows of one
   // launch share their halo rows through L2)
@@ -398,8 +406,9 @@ void launch_stream_collide(lbm* h, int band, const double* low) {
   // banded steps: one CTA row per lattice row above the band as the host last saw it
   // (h->band_hint, 0 = unknown); the kernel's row loop covers whatever the band has lost since
   const int rows = band ? h->ny - h->band_hint : h->ny;
-  k_stream_collide<<<grid_rows(h->px, rows, SC_THREADS), SC_THREADS, 0, h->stream>>>(
-      h->A, h->B, h->flag, band == 1 ? low : nullptr, band ? h->band : h->band + 1, band == 1 ? -1 : 0, h->C);
+  launch_k(k_stream_collide, grid_rows(h->px, rows, SC_THREADS), dim3(SC_THREADS), 0, h->stream, h->use_pdl != 0,
+           (const double*)h->A, h->B, (const unsigned char*)h->flag, band == 1 ? low : (const double*)nullptr,
+           (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->C);
 }
 
 int stream_collide_configure() {
@@ -411,17 +420,20 @@ int stream_collide_configure() {
 void launch_stream_collide_2step(lbm* h) {
   h->launches++;
   const dim3 grid((h->nx + TB_X - 1) / TB_X, (h->ny + TB_Y - 1) / TB_Y);
-  k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(h->A, h->A, h->B, nullptr, 1, 0, h->C);
+  launch_k(k_stream_collide_2step, grid, dim3(TB_THREADS), TB_SMEM, h->stream, h->use_pdl != 0,
+           (const double*)h->A, (const double*)h->A, h->B, (const int*)nullptr, 1, 0, h->C);
 }
 
 // the band rows [0, *h->band) of a lattice with particles: the part-th of nparts contiguous shares
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part) {
   h->launches++;
-  const int tile_rows = (h->ny + TB_Y - 1) / TB_Y;
+  // CTAs of this kernel are expensive to launch even when they exit at once (512 threads, 57 KB):
+  // the grid covers the band as the host last saw it plus a margin (k_band_plan keeps Q below it)
+  const int tile_rows = (std::min(h->band_cap, h->ny) + TB_Y - 1) / TB_Y;
   const dim3 grid((h->nx + TB_X - 1) / TB_X, (tile_rows + nparts - 1) / nparts);
-  k_stream_collide_2step<<<grid, TB_THREADS, TB_SMEM, h->stream>>>(src_band, src_top, dst_band, h->band,
-                                                                   nparts, part, h->C);
+  launch_k(k_stream_collide_2step, grid, dim3(TB_THREADS), TB_SMEM, h->stream, h->use_pdl != 0, src_band, src_top,
+           dst_band, (const int*)h->band, nparts, part, h->C);
 }
 
 void launch_init_collide(lbm* h, double* dst) {

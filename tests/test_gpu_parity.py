@@ -552,7 +552,7 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
     a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
     b.set_band(False)
     qs = []
-    for nst in (4, 4, 8, 16, 40, 200):
+    for nst in (16, 16, 24, 40, 200):         # (calls shorter than 16 steps never use the band)
         a.step(nst)
         b.step(nst)
         assert_same_bits(a, b)
