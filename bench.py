@@ -133,10 +133,23 @@ def oracle_sample_workload(wl, cfg, edge):
                             name=f"config{cfg}_sample_{edge}")
 
 
+def host_gb_free():
+    try:
+        import psutil
+        return psutil.virtual_memory().available / 2 ** 30
+    except ImportError:
+        return 0.0
+
+
+# host memory the oracle needs for a full config (three copies of f, g + fields), GB
+ORACLE_FULL_GB = {0: 0.1, 1: 1.0, 2: 1.0, 3: 8.0, 4: 32.0, 5: 8.0}
+
+
 def time_oracle(wl, cfg, edge, steps, warmup):
+    """edge = 0: the full config; else a square sample of that edge."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle_binding as ob
-    w = oracle_sample_workload(wl, cfg, edge)
+    w = wl.config(cfg) if edge == 0 else oracle_sample_workload(wl, cfg, edge)
     o = ob.OracleSim.from_workload(w)
     if warmup:
         o.step(warmup)
@@ -151,18 +164,27 @@ def run_reference(args, wl):
     if rank != 0:
         return
     total = args.steps + args.warmup
-    # size the sample so that the whole run ends within ~2 minutes at ~1.5 MLUPS (measured)
-    edge = int(math.sqrt(max(1.0, 120.0 * 1.5e6 / max(total, 1))))
-    edge = max(96, min(1000, edge))
+    full = wl.config(args.config)
+    # the FULL config whenever the oracle can finish it in a few minutes (about 5 MLUPS on one
+    # core: 3.3 s per step of config 3) and the host has the memory; else a bounded sample sized
+    # so that the whole run ends within ~2 minutes
+    full_seconds = full.nx * full.ny * total / 4.5e6
+    if full_seconds <= 240.0 and host_gb_free() >= ORACLE_FULL_GB.get(args.config, 8.0) + 4.0:
+        edge = 0
+    else:
+        edge = int(math.sqrt(max(1.0, 120.0 * 1.5e6 / max(total, 1))))
+        edge = max(96, min(1000, edge))
     w, val, dt = time_oracle(wl, args.config, edge, args.steps, args.warmup)
-    sample = (f"{w.nx}x{w.ny} sample of config {args.config} ({w.n_particles} particles, same "
+    what = "the full config" if edge == 0 else f"{w.nx}x{w.ny} sample of config {args.config}"
+    sample = (f"{what} ({w.nx}x{w.ny}, {w.n_particles} particles; samples keep the "
               f"density/diameters/physics/placement recipe), {args.steps} steps after "
               f"{args.warmup} warm-up, single thread")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "MLUPS",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": dt / max(args.steps, 1) * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"config{args.config}", "sample": sample},
+            "config": {"workload": w.name if edge == 0 else f"config{args.config}", "sample": sample,
+                       "same_config": edge == 0},
             "cpu_baseline": {"value": val, "unit": "MLUPS", "cores": 1, "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": val, "unit": "MLUPS", "h2d_bytes_per_step": 0,
@@ -334,13 +356,18 @@ def main():
     # ---------------- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        edge = 600 if args.config >= 2 else (512 if args.config == 1 else 0)
-        steps_cpu = 200 if args.config >= 1 else 4000    # about 15 s of single-thread work
+        # about 15-25 s of single-thread work: the full config where a handful of steps fit
+        # (config 3: 5 steps of 3.3 s; configs 0-2: more steps), a sample only for config 4
+        if args.config in (0, 1, 2, 3, 5) and host_gb_free() >= ORACLE_FULL_GB[args.config] + 4.0:
+            edge = 0
+            steps_cpu = {0: 4000, 1: 60, 2: 60, 3: 5, 5: 5}[args.config]
+        else:
+            edge, steps_cpu = 600, 200
         wc, v, dt = time_oracle(wl, args.config, edge, steps_cpu, 1)
+        what = "the full config" if edge == 0 else f"{wc.nx}x{wc.ny} sample of config {args.config}"
         cpu = {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle",
-               "sample": f"{wc.nx}x{wc.ny} sample of config {args.config} ({wc.n_particles} "
-                         f"particles, same recipe), {steps_cpu} steps, {dt:.1f} s, single thread "
-                         f"of {os.cpu_count()} host cores"}
+               "sample": f"{what} ({wc.nx}x{wc.ny}, {wc.n_particles} particles), {steps_cpu} steps "
+                         f"after 1, {dt:.1f} s, single thread of {os.cpu_count()} host cores"}
 
     # BASELINE.md holds a published number only for the paper's own workload (config 5): 1750 MLUPS
     # on 1x A100 (Table 5) -- another machine's, context rather than target
