@@ -51,6 +51,10 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--profile-steps", type=int, default=200)
+    ap.add_argument("--slabs", action="store_true",
+                    help="cut the lattice into one y-slab per rank (strong scaling: halo rows and the "
+                         "force combine cross NVLink every step) instead of independent replicas; "
+                         "north_star keeps the headline on one GPU, so this is not the default")
     ap.add_argument("--edge", type=int, default=0,
                     help="config 1 only: particle-free lattice of this edge instead of 1024 "
                          "(same physics and initial-state recipe)")
@@ -204,6 +208,9 @@ def main():
     import numpy as np
     import torch
     from paper_2308_16597_b200 import binding, replicas
+    if args.slabs:
+        run_slabs(args, wl)
+        return
 
     rank, world, local = replicas.rank_info()
     if not torch.cuda.is_available():
@@ -387,6 +394,56 @@ def main():
                 "context": {"paper_single_gpu_mlups": 1750, "paper_hardware": "1x A100, OpenACC "
                             "(PAPER.md:271-281; d=40, Pr=5 workload: context, not like-for-like)"}}
         print(json.dumps(line))
+    replicas.shutdown()
+
+
+def run_slabs(args, wl):
+    """One y-slab per rank (paper_2308_16597_b200/slabs.py, include/lbm.h "y-slabs"): the same
+    metric on a lattice cut along y; per step one all-reduce of 3 doubles per particle and one
+    send / recv of `halo` rows x 14 populations with each neighbour."""
+    import torch
+    from paper_2308_16597_b200 import replicas, slabs
+    rank, world, local = replicas.rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hot path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    replicas.init("nccl", dev)
+    K, W = args.steps, max(args.warmup, 3)
+    w = wl.config(args.config)
+    sr = slabs.SlabRank(w, rank, world, dev)
+    stream = torch.cuda.current_stream(dev)
+    sr.step(W)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    clocks = ClockSampler(local)
+    clocks.start()
+    time.sleep(0.3)
+    replicas.barrier(dev)
+    l0 = sr.sim.kernel_launches()
+    t0 = time.perf_counter()
+    ev0.record(stream)
+    sr.step(K)
+    ev1.record(stream)
+    replicas.barrier(dev)
+    t1 = time.perf_counter()
+    launches = sr.sim.kernel_launches() - l0
+    ms_max = replicas.max_over_ranks(ev0.elapsed_time(ev1), dev)
+    clk = clocks.stop(t0, t1)
+    value = w.nx * w.ny * K / (ms_max * 1e-3) / 1e6          # one lattice, all ranks together
+    if rank == 0:
+        j0, j1 = sr.ranges[0]
+        line = {"metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "particles": w.n_particles,
+                           "parallelism": f"{world} y-slabs of ~{j1 - j0} rows, {sr.halo} ghost rows "
+                                          "per face, direct launches (no graphs, no band)",
+                           "l2": "inputs larger than L2" if 2 * 14 * 8 * w.nx * w.ny / world > 252e6
+                                 else "working set fits L2"},
+                "clocks": clk, "e2e": None, "gpu_launches": launches, "roofline": None,
+                "cpu_baseline": None}
+        print(json.dumps(line))
+    sr.close()
     replicas.shutdown()
 
 

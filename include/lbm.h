@@ -152,6 +152,49 @@ int lbm_set_two_step(lbm_t* h, int on);
 int lbm_set_band(lbm_t* h, int on);
 int lbm_get_band(lbm_t* h, int* rows);
 
+/* ---- y-slabs: domain decomposition along y (PAPER.md:287-291 ghost layers,
+ * 303-321 domain lists, 347-355 schedule).  BASELINE.json's north_star keeps the measured path on
+ * one GPU; this is the library side of the next step, testable on one device.
+ *
+ * A slab handle stores and updates the rows [j0, j1) of a cavity ny_global rows high (its OWN rows)
+ * plus `halo` ghost rows on every side that is not a cavity wall.  Every slab holds EVERY particle
+ * (lbm_add_particles with the same arrays on each; coordinates are global) and advances all of
+ * them identically; which slab does what for a particle follows from positions alone (the paper's
+ * domain lists): each slab rasterises, builds links and runs the bounce-back for whatever part of
+ * a particle lies in its stored rows (that parks the values its own rows pull); the slab whose own
+ * rows hold the particle's centre sees all of its links -- the halo must be at least d/2 + 8 rows,
+ * checked by lbm_add_particles -- and its force sum, in the single domain's order, is the
+ * particle's force.  Results on own rows and all particle states are bit-identical to one
+ * lbm_create domain (tests/test_gpu_slabs.py).
+ *
+ * One time step, for all slabs:
+ *   lbm_slab_forces(h)      bounce-back + momentum exchange; the slab's share of F, T_z (zeros for
+ *                           particles it does not own) is left in lbm_slab_force_buffer
+ *   -- force combine: element-wise sum of the slabs' buffers (3 * n doubles: Fx[n], Fy[n], Tz[n]),
+ *      written back to every slab's buffer.  One process: lbm_slab_combine_forces; ranks: an
+ *      all-reduce (the sum is exact: one non-zero term per entry)
+ *   lbm_slab_advance(h)     particle update from the combined forces, flags, refill, links, lattice
+ *                           kernel on the own rows
+ *   -- halo exchange: lbm_slab_pack(h, side, buf) / lbm_slab_unpack(h, side, buf) with
+ *      lbm_slab_halo_doubles values per face (14 populations x halo rows), or, in one process,
+ *      lbm_slab_exchange_halos (direct copies, peer copies between devices)
+ * lbm_slab_check reads the device status word (one synchronisation; same errors as lbm_step).
+ * lbm_step refuses slab handles.  lbm_set_temperature takes the STORED rows (own + ghost:
+ * global rows [j0 - halo, j1 + halo) clipped to the cavity), lbm_get_fields returns the OWN rows.
+ * Errors: LBM_E_ARG (halo < 4, a slab lower than its halo, ranges that do not adjoin), LBM_E_STATE. */
+size_t lbm_slab_workspace_bytes(int nx, int ny_global, int j0, int j1, int halo, const lbm_params* p);
+int lbm_create_slab(int nx, int ny_global, int j0, int j1, int halo, const lbm_params* p,
+                    void* dev_workspace, size_t bytes, void* cuda_stream, lbm_t** out);
+int lbm_slab_forces(lbm_t* h);
+int lbm_slab_force_buffer(lbm_t* h, double** dev_buf, int* count);   /* DEVICE pointer, 3 * n doubles */
+int lbm_slab_advance(lbm_t* h);
+int lbm_slab_check(lbm_t* h);
+int lbm_slab_halo_doubles(const lbm_t* h, long long* doubles);
+int lbm_slab_pack(lbm_t* h, int side, double* dev_buf);           /* side 0: lowest own rows, 1: highest */
+int lbm_slab_unpack(lbm_t* h, int side, const double* dev_buf);   /* side 0: ghost rows below, 1: above */
+int lbm_slab_exchange_halos(lbm_t** slabs, int n);                /* ascending row ranges, one process */
+int lbm_slab_combine_forces(lbm_t** slabs, int n);                /* same, one device */
+
 /* Readout.  Any pointer may be NULL = not wanted.
  * rho, ux, uy, T: nx*ny doubles each; on fluid nodes rho = sum f, T = sum g,
  *   u = (sum e f + F/2)/rho; on solid nodes rho0, rigid-body velocity, T_w.

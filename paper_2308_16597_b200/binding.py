@@ -79,6 +79,18 @@ def load_library():
     L.lbm_set_graph.argtypes = [vp, C.c_int]
     L.lbm_set_band.argtypes = [vp, C.c_int]
     L.lbm_get_band.argtypes = [vp, C.POINTER(C.c_int)]
+    L.lbm_slab_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P]
+    L.lbm_slab_workspace_bytes.restype = sz
+    L.lbm_create_slab.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, vp, sz, vp, C.POINTER(vp)]
+    L.lbm_slab_forces.argtypes = [vp]
+    L.lbm_slab_force_buffer.argtypes = [vp, C.POINTER(vp), C.POINTER(C.c_int)]
+    L.lbm_slab_advance.argtypes = [vp]
+    L.lbm_slab_check.argtypes = [vp]
+    L.lbm_slab_halo_doubles.argtypes = [vp, C.POINTER(ll)]
+    L.lbm_slab_pack.argtypes = [vp, C.c_int, vp]
+    L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp]
+    L.lbm_slab_exchange_halos.argtypes = [C.POINTER(vp), C.c_int]
+    L.lbm_slab_combine_forces.argtypes = [C.POINTER(vp), C.c_int]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
     L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
@@ -95,7 +107,10 @@ def load_library():
     for name in ("lbm_create", "lbm_set_temperature", "lbm_add_particles", "lbm_add_ellipses", "lbm_step",
                  "lbm_get_fields", "lbm_get_particles", "lbm_get_links", "lbm_profile_enable",
                  "lbm_profile_kernels", "lbm_profile_get", "lbm_destroy", "lbm_set_overlap",
-                 "lbm_set_two_step", "lbm_set_graph", "lbm_set_band", "lbm_get_band"):
+                 "lbm_set_two_step", "lbm_set_graph", "lbm_set_band", "lbm_get_band", "lbm_create_slab",
+                 "lbm_slab_forces", "lbm_slab_force_buffer", "lbm_slab_advance", "lbm_slab_check",
+                 "lbm_slab_halo_doubles", "lbm_slab_pack", "lbm_slab_unpack", "lbm_slab_exchange_halos",
+                 "lbm_slab_combine_forces"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -117,18 +132,31 @@ def _host(a, pinned_ok=True):
 class Simulation:
     """One particle-resolved thermal LBM simulation on one B200 (calls follow include/lbm.h)."""
 
-    def __init__(self, nx, ny, params, device="cuda:0", stream=None):
+    def __init__(self, nx, ny, params, device="cuda:0", stream=None, slab=None):
+        """slab = (j0, j1, halo): a y-slab of the nx x ny cavity (include/lbm.h "y-slabs"): the handle
+        stores the rows [j0 - halo, j1 + halo) clipped to the cavity and owns [j0, j1); `ny`, `n` and
+        the arrays of fields() then refer to the OWN rows, `rows_stored` to what set_temperature takes."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the lattice Boltzmann hot path has no CPU fallback")
         self._torch = torch
         self._L = load_library()
         self.nx, self.ny, self.n = int(nx), int(ny), int(nx) * int(ny)
+        self.ny_global, self.slab = int(ny), None
         self.params = dict(params)
         self._P = LbmParams.from_dict(params)
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        nbytes = self._L.lbm_workspace_bytes(self.nx, self.ny, C.byref(self._P))
+        if slab is not None:
+            j0, j1, halo = (int(v) for v in slab)
+            self.slab = (j0, j1, halo)
+            lo, hi = (0 if j0 == 0 else j0 - halo), (int(ny) if j1 == int(ny) else j1 + halo)
+            self.rows_stored = (lo, hi)
+            self.ny, self.n = j1 - j0, int(nx) * (j1 - j0)
+            nbytes = self._L.lbm_slab_workspace_bytes(self.nx, self.ny_global, j0, j1, halo, C.byref(self._P))
+        else:
+            self.rows_stored = (0, int(ny))
+            nbytes = self._L.lbm_workspace_bytes(self.nx, self.ny, C.byref(self._P))
         if nbytes == 0:
             raise LbmError(LBM_E_ARG, "lbm_workspace_bytes: bad size or parameter")
         self.workspace_bytes = int(nbytes)
@@ -136,9 +164,14 @@ class Simulation:
         base = (self._ws.data_ptr() + 255) // 256 * 256
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._h = C.c_void_p()
-        rc = self._L.lbm_create(self.nx, self.ny, C.byref(self._P), C.c_void_p(base),
-                                C.c_size_t(int(nbytes)), C.c_void_p(self.stream.cuda_stream),
-                                C.byref(self._h))
+        if slab is not None:
+            rc = self._L.lbm_create_slab(self.nx, self.ny_global, j0, j1, halo, C.byref(self._P),
+                                         C.c_void_p(base), C.c_size_t(int(nbytes)),
+                                         C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
+        else:
+            rc = self._L.lbm_create(self.nx, self.ny, C.byref(self._P), C.c_void_p(base),
+                                    C.c_size_t(int(nbytes)), C.c_void_p(self.stream.cuda_stream),
+                                    C.byref(self._h))
         if rc:
             raise LbmError(rc, self._L.lbm_last_error(None).decode())
 
@@ -170,7 +203,7 @@ class Simulation:
     # ---- set-up ----
     def set_temperature(self, T):
         T = _host(T).reshape(-1)
-        assert T.size == self.n
+        assert T.size == self.nx * (self.rows_stored[1] - self.rows_stored[0])
         self._chk(self._L.lbm_set_temperature(self._h, _d(T)))
 
     def add_particles(self, x, y, diam, rho_ratio, T_w, ux=None, uy=None, omega=None, fixed=None,
@@ -211,6 +244,34 @@ class Simulation:
 
     def set_two_step(self, on=True):
         self._chk(self._L.lbm_set_two_step(self._h, 1 if on else 0))
+
+    # ---- y-slabs: the two halves of a step and the exchanges' end points (slabs.py drives them) ----
+    def slab_forces(self):
+        self._chk(self._L.lbm_slab_forces(self._h))
+
+    def slab_advance(self):
+        self._chk(self._L.lbm_slab_advance(self._h))
+
+    def slab_check(self):
+        self._chk(self._L.lbm_slab_check(self._h))
+
+    def slab_force_tensor(self):
+        """The slab's force buffer (3 * n doubles on the device) as a torch view of the workspace."""
+        ptr, cnt = C.c_void_p(), C.c_int()
+        self._chk(self._L.lbm_slab_force_buffer(self._h, C.byref(ptr), C.byref(cnt)))
+        off = (ptr.value or 0) - self._ws.data_ptr()
+        return self._ws[off:off + 8 * cnt.value].view(self._torch.float64)
+
+    def slab_halo_doubles(self):
+        n = C.c_longlong()
+        self._chk(self._L.lbm_slab_halo_doubles(self._h, C.byref(n)))
+        return n.value
+
+    def slab_pack(self, side, buf):
+        self._chk(self._L.lbm_slab_pack(self._h, int(side), C.c_void_p(buf.data_ptr())))
+
+    def slab_unpack(self, side, buf):
+        self._chk(self._L.lbm_slab_unpack(self._h, int(side), C.c_void_p(buf.data_ptr())))
 
     # ---- read-out ----
     def fields(self, populations=False, out=None):

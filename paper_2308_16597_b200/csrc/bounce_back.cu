@@ -25,15 +25,17 @@ __constant__ double b_w[9] = {4.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9, 1.0 / 9,
 
 constexpr int BT = 128;
 
-// index of node (i+di, j+dj) or -1 if outside the cavity (x wraps when periodic)
+// memory index of node (i+di, j+dj), j a GLOBAL row, or -1 if it lies outside the cavity (x wraps
+// when periodic) or in a row this handle does not store (y-slabs: such a node is farther from the
+// slab's own rows than anything the slab's own results depend on)
 __device__ __forceinline__ long long node_at(const LbmConst& c, int i, int j, int di, int dj) {
   int a = i + di, b = j + dj;
-  if (b < 0 || b >= c.ny) return -1;
+  if (!row_here(c, b)) return -1;
   if (a < 0 || a >= c.nx) {
     if (!c.periodic_x) return -1;
     a = (a + c.nx) % c.nx;
   }
-  return (long long)b * c.px + a;
+  return node_index(c, a, b);
 }
 
 __global__ void __launch_bounds__(BT, 8)
@@ -56,7 +58,7 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
     const int nbehind = db >> LINK_BEHIND_SHIFT;   // fluid nodes behind x_f (link builder)
     const int ab = b_opp[al];
     const int i = nd & 0xffff, j = (int)((unsigned)nd >> 16);
-    const int xf = j * c.px + i;
+    const int xf = (int)node_index(c, i, j);
     const int ex = b_ex[al], ey = b_ey[al];
     // the populations this link's rung of the ladder needs, all requested before the first use
     // (independent loads in flight together); q <= 1/2 interpolates upstream of x_f in plane
@@ -113,7 +115,8 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
         fbb = (fi0 + tq * fa + wall) * (0.5 * rq);
       }
     }
-    const long long xb = (long long)(j + ey) * c.px + (i + ex);   // solid node of the link
+    const long long xb = node_index(c, i + ex, j + ey);   // solid node of the link
+    const bool park = row_here(c, j + ey);                // (always, except on a slab's outermost ghost row)
     if (al <= 4) {
       double cd2 = 0.0, cd4 = 1.0;
       if (nbehind >= 1) {
@@ -124,8 +127,8 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
       }
       const double gbb = (-gi0 + cd2 * gi1 + cd2 * gb0) + cd4 * (2.0 * c.wT * Tw);
       // parked for the pull at x_f: the pair (f_ibar, g_ibar) of the solid node
-      *reinterpret_cast<double2*>(A + 2 * (long long)ab * c.ps + 2 * xb) = make_double2(fbb, gbb);
-    } else {
+      if (park) *reinterpret_cast<double2*>(A + 2 * (long long)ab * c.ps + 2 * xb) = make_double2(fbb, gbb);
+    } else if (park) {
       A[(long long)(ab + 5) * c.ps + xb] = fbb;
     }
     // Eqs. (13), (14)
@@ -190,7 +193,7 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
       continue;
     }
     const int p = nb_pid[e];
-    const int i = x % c.px, j = x / c.px;
+    const int i = x % c.px, j = x / c.px + c.yoff;   // j: global row
     // state at t+1 (cur already points at the new buffer)
     const double dxn = (double)i - pa.x[cur][p], dyn = (double)j - pa.y[cur][p];
     // e_c maximises n . e_alpha/|e_alpha|, ties -> lowest alpha; separately rounded operations
@@ -228,7 +231,7 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
     if (okm & 1u) { nvalid = 1; if (okm & (1u << 9)) { nvalid = 2; if (okm & (1u << 18)) nvalid = 3; } }
     double v = 0.0;
     if (lane < 27 && st < nvalid) {
-      const int ci = (int)(snode % c.px), cj = (int)(snode / c.px);
+      const int ci = (int)(snode % c.px), cj = (int)(snode / c.px) + c.yoff;
       const long long src = node_at(c, ci, cj, -b_ex[k], -b_ey[k]);
       v = src >= 0 ? A[f_at(k, src, c.ps)] : A[f_at(b_opp[k], snode, c.ps)];
     }

@@ -75,19 +75,20 @@ struct Layout {
   int newborn_cap;
 };
 
-Layout layout_of(int nx, int ny, const lbm_params* p) {
+// ny: rows stored; NY: height of the whole cavity (the repulsion grid covers all of it)
+Layout layout_of(int nx, int ny, int NY, const lbm_params* p) {
   Layout L;
   L.px = (int)align_up((size_t)nx, 16);
   L.ps = (long long)align_up((size_t)L.px * (ny + 1), 32);   // one spare row (the band seam's)
   L.mcx = (int)std::ceil(nx / MIN_CELL) + 1;
-  L.mcy = (int)std::ceil(ny / MIN_CELL) + 1;
+  L.mcy = (int)std::ceil(NY / MIN_CELL) + 1;
   L.max_cells = p->max_particles > 0 ? L.mcx * L.mcy : 0;
   L.newborn_cap = p->max_particles * NEWBORN_PER_PARTICLE;
   return L;
 }
 
-size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
-  const Layout L = layout_of(nx, ny, p);
+size_t carve(lbm* h, void* base, int nx, int ny, int NY, const lbm_params* p) {
+  const Layout L = layout_of(nx, ny, NY, p);
   Carver c(base);
   const size_t np = (size_t)p->max_particles;
   double* A = c.take<double>(14 * (size_t)L.ps);
@@ -136,7 +137,9 @@ size_t carve(lbm* h, void* base, int nx, int ny, const lbm_params* p) {
   double* stash = c.take<double>((size_t)L.newborn_cap * 14);
   int* status = c.take<int>(1);
   int* band = c.take<int>(2);
+  double* fbuf = c.take<double>(3 * np);
   if (h) {
+    h->force_buf = fbuf;
     h->band = band;
     h->px = L.px;
     h->ps = L.ps;
@@ -173,6 +176,8 @@ void fill_const(lbm* h) {
   const lbm_params& p = h->P;
   c.nx = h->nx;
   c.ny = h->ny;
+  c.yoff = h->yoff;
+  c.NY = h->NY;
   c.px = h->px;
   c.ps = h->ps;
   c.periodic_x = p.periodic_x ? 1 : 0;
@@ -298,19 +303,21 @@ void lbm_params_default(lbm_params* p) {
 
 size_t lbm_workspace_bytes(int nx, int ny, const lbm_params* p) {
   if (!params_ok(nx, ny, p)) return 0;
-  return carve(nullptr, nullptr, nx, ny, p);
+  return carve(nullptr, nullptr, nx, ny, ny, p);
 }
 
-int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t bytes,
-               void* cuda_stream, lbm_t** out) {
+// Shared by lbm_create (a whole cavity: yoff = 0, NY = ny, no halo) and lbm_create_slab (global
+// rows [yoff, yoff + ny) of a cavity NY rows high, of which [own0, own1) are the slab's own).
+static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, int own1, int halo, const lbm_params* p,
+                       void* dev_workspace, size_t bytes, void* cuda_stream, lbm_t** out) {
   if (!out) return fail(nullptr, LBM_E_ARG, "lbm_create: out is NULL");
   *out = nullptr;
-  if (!params_ok(nx, ny, p)) return fail(nullptr, LBM_E_ARG, "lbm_create: bad size or parameter");
+  if (!params_ok(nx, ny, p) || NY > 46000) return fail(nullptr, LBM_E_ARG, "lbm_create: bad size or parameter");
   if (!dev_workspace || ((uintptr_t)dev_workspace & 255))
     return fail(nullptr, LBM_E_ARG, "lbm_create: workspace NULL or not 256-byte aligned");
-  const size_t need = carve(nullptr, nullptr, nx, ny, p);
+  const size_t need = carve(nullptr, nullptr, nx, ny, NY, p);
   if (bytes < need) return fail(nullptr, LBM_E_CAPACITY, "lbm_create: workspace %zu < %zu bytes", bytes, need);
-  if ((long long)layout_of(nx, ny, p).px * ny >= 0x7fffffffLL)
+  if ((long long)layout_of(nx, ny, NY, p).px * ny >= 0x7fffffffLL)
     return fail(nullptr, LBM_E_ARG, "lbm_create: lattice too large for 32-bit node indices");
   lbm* h = new (std::nothrow) lbm;
   if (!h) return fail(nullptr, LBM_E_ARG, "lbm_create: out of host memory");
@@ -319,7 +326,15 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
   h->ny = ny;
   h->P = *p;
   h->stream = (cudaStream_t)cuda_stream;
-  carve(h, dev_workspace, nx, ny, p);
+  h->is_slab = is_slab;
+  h->yoff = yoff;
+  h->NY = NY;
+  h->own0 = own0;
+  h->own1 = own1;
+  h->halo = halo;
+  h->row0 = own0 - yoff;
+  h->row1 = own1 - yoff;
+  carve(h, dev_workspace, nx, ny, NY, p);
   fill_const(h);
   cudaGetDevice(&h->device);
   h->two_step_ok = stream_collide_configure() == 0 ? 1 : 0;
@@ -401,8 +416,53 @@ int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t 
     delete h;
     return LBM_E_CUDA;
   }
+  if (h->is_slab) {
+    // a slab is stepped in two halves by its caller (lbm_slab_forces / lbm_slab_advance), on one
+    // stream, with direct launches; no band (its plan would need every slab's agreement)
+    h->overlap = 0;
+    h->chain = h->side = h->stream;
+    h->use_graph = 0;
+    h->band_on = 0;
+  }
   *out = h;
   return LBM_OK;
+}
+
+int lbm_create(int nx, int ny, const lbm_params* p, void* dev_workspace, size_t bytes,
+               void* cuda_stream, lbm_t** out) {
+  return create_impl(0, nx, ny, 0, ny, 0, ny, 0, p, dev_workspace, bytes, cuda_stream, out);
+}
+
+// ---- y-slabs (PAPER.md:287-291 ghost layers, 303-321 domain lists) ----
+// rows stored by the slab that owns [j0, j1): `halo` ghost rows on each side that is not a cavity wall
+static void slab_extent(int ny_global, int j0, int j1, int halo, int* yoff, int* rows) {
+  const int lo = j0 == 0 ? 0 : j0 - halo, hi = j1 == ny_global ? ny_global : j1 + halo;
+  *yoff = lo;
+  *rows = hi - lo;
+}
+
+static bool slab_ok(int nx, int ny_global, int j0, int j1, int halo) {
+  if (nx < 4 || ny_global < 4 || j0 < 0 || j1 > ny_global || j1 <= j0 || halo < 4) return false;
+  if (j0 != 0 && j0 - halo < 0) return false;                 // the slab below must be at least `halo` high
+  if (j1 != ny_global && j1 + halo > ny_global) return false;
+  return j1 - j0 >= halo;
+}
+
+size_t lbm_slab_workspace_bytes(int nx, int ny_global, int j0, int j1, int halo, const lbm_params* p) {
+  if (!slab_ok(nx, ny_global, j0, j1, halo)) return 0;
+  int yoff, rows;
+  slab_extent(ny_global, j0, j1, halo, &yoff, &rows);
+  if (!params_ok(nx, rows, p)) return 0;
+  return carve(nullptr, nullptr, nx, rows, ny_global, p);
+}
+
+int lbm_create_slab(int nx, int ny_global, int j0, int j1, int halo, const lbm_params* p,
+                    void* dev_workspace, size_t bytes, void* cuda_stream, lbm_t** out) {
+  if (!slab_ok(nx, ny_global, j0, j1, halo))
+    return fail(nullptr, LBM_E_ARG, "lbm_create_slab: bad row range or halo (need halo >= 4 and every slab at least halo rows high)");
+  int yoff, rows;
+  slab_extent(ny_global, j0, j1, halo, &yoff, &rows);
+  return create_impl(1, nx, rows, yoff, ny_global, j0, j1, halo, p, dev_workspace, bytes, cuda_stream, out);
 }
 
 int lbm_set_temperature(lbm_t* h, const double* T_host) {
@@ -463,7 +523,7 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
       hx = std::sqrt(ac * ac + bs * bs);
       hy = std::sqrt(as * as + bc * bc);
     }
-    if (!(y[k] - hy > -0.5) || !(y[k] + hy < h->ny - 0.5))
+    if (!(y[k] - hy > -0.5) || !(y[k] + hy < h->NY - 0.5))
       return fail(h, LBM_E_ARG, "add_particles: particle %d touches a y wall", k);
     if (!h->P.periodic_x) {
       if (!(x[k] - hx > -0.5) || !(x[k] + hx < h->nx - 0.5))
@@ -546,13 +606,19 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
   CUDA_OK(h, up(h->pa.Tz, nullptr));
   CUDA_OK(h, cudaMemcpyAsync(h->pa.fixed + n0, fx.data(), n, cudaMemcpyHostToDevice, h->stream));
   CUDA_OK(h, cudaMemsetAsync(h->pa.ovl + n0, 0, n, h->stream));
+  // y-slab: a particle whose centre lies in the own rows must be inside the stored rows together
+  // with its link stencils (2 rows) and the refill stencils of its newborn nodes (4 rows + the
+  // parked values those pull: 2 more), for as long as it is owned: r + 8 rows
+  if (h->is_slab && 0.5 * dmax + 8.0 > (double)h->halo)
+    return fail(h, LBM_E_ARG, "add_particles: halo of %d rows is too narrow for particles of diameter %.1f (need d/2 + 8)",
+                h->halo, dmax);
   h->np = nt;
   for (int k = n0; k < nt; ++k) h->n_ell += (SA[k] != SB[k]) ? 1 : 0;
   h->d_max = dmax;
   size_chain(h);
   h->cell = std::max(dmax + h->P.rep_s, MIN_CELL);
   h->ncx = (int)std::ceil(h->nx / h->cell) + 1;
-  h->ncy = (int)std::ceil(h->ny / h->cell) + 1;
+  h->ncy = (int)std::ceil(h->NY / h->cell) + 1;
   if ((long long)h->ncx * h->ncy > h->max_cells)
     return fail(h, LBM_E_CAPACITY, "add_particles: repulsion grid larger than the workspace allows");
   // flag and owner maps and the repulsion grid of step 0 (primed == 0: every particle, full sweep)
@@ -777,6 +843,8 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
 int lbm_step(lbm_t* h, int nsteps) {
   if (!h) return LBM_E_ARG;
   if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
+  if (h->is_slab && nsteps > 0)
+    return fail(h, LBM_E_STATE, "lbm_step on a slab: use lbm_slab_forces / lbm_slab_advance and the exchanges between them");
   DeviceGuard dg(h);
   if (nsteps > 0) {
     prime(h);
@@ -860,6 +928,151 @@ int lbm_get_band(lbm_t* h, int* rows) {
   return LBM_OK;
 }
 
+// ---- y-slabs: one time step in two halves, the two exchanges between them left to the caller ----
+// copies `rows` rows of all 14 populations: (src copy, local row sr) -> (dst copy, local row dr);
+// the planes are row-major with the same pitch in every slab of a decomposition, so a block of
+// rows is one contiguous piece per plane.  buf != nullptr: to / from a packed buffer instead.
+static int copy_rows(lbm* hd, double* dstA, int dr, const lbm* hs, const double* srcA, int sr, int rows,
+                     double* pack_to, const double* unpack_from, cudaStream_t st) {
+  const size_t px = (size_t)hs->px;
+  size_t off = 0;
+  for (int k = 0; k < 9; ++k) {
+    const bool pair = k < 5;
+    const size_t cnt = (pair ? 2 : 1) * px * rows;
+    const size_t ps_s = (size_t)hs->ps, ps_d = hd ? (size_t)hd->ps : 0;
+    const double* src = unpack_from ? unpack_from + off
+                                    : srcA + (pair ? 2 * k * ps_s + 2 * px * sr : (k + 5) * ps_s + px * sr);
+    double* dst = pack_to ? pack_to + off
+                          : dstA + (pair ? 2 * k * ps_d + 2 * px * dr : (k + 5) * ps_d + px * dr);
+    cudaError_t e;
+    if (hd && hs && hd->device != hs->device && !pack_to && !unpack_from)
+      e = cudaMemcpyPeerAsync(dst, hd->device, src, hs->device, cnt * sizeof(double), st);
+    else
+      e = cudaMemcpyAsync(dst, src, cnt * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return -1;
+    off += cnt;
+  }
+  return 0;
+}
+
+int lbm_slab_halo_doubles(const lbm_t* h, long long* doubles) {
+  if (!h || !doubles) return LBM_E_ARG;
+  *doubles = 14LL * h->halo * h->px;
+  return LBM_OK;
+}
+
+int lbm_slab_forces(lbm_t* h) {
+  if (!h) return LBM_E_ARG;
+  if (!h->is_slab) return fail(h, LBM_E_STATE, "lbm_slab_forces: not a slab handle");
+  DeviceGuard dg(h);
+  prime(h);
+  ensure_links(h);
+  launch_bounce_back(h, h->stream, false);
+  launch_slab_forces_out(h);
+  return LBM_OK;
+}
+
+int lbm_slab_force_buffer(lbm_t* h, double** dev_buf, int* count) {
+  if (!h || !dev_buf || !count) return LBM_E_ARG;
+  *dev_buf = h->force_buf;
+  *count = 3 * h->np;
+  return LBM_OK;
+}
+
+int lbm_slab_advance(lbm_t* h) {
+  if (!h) return LBM_E_ARG;
+  if (!h->is_slab) return fail(h, LBM_E_STATE, "lbm_slab_advance: not a slab handle");
+  if (!h->primed) return fail(h, LBM_E_STATE, "lbm_slab_advance before lbm_slab_forces");
+  DeviceGuard dg(h);
+  cudaStream_t S = h->stream;
+  const int sp = h->cur;
+  h->band_live = 0;
+  if (h->np > 0) {
+    launch_slab_forces_in(h);
+    launch_move(h, S, false);
+    launch_cover(h, sp ^ 1, S, false);
+    launch_refill(h, S);
+    launch_build_links(h, sp ^ 1, S, false);
+    h->cur ^= 1;
+  }
+  launch_stream_collide(h, 0, nullptr);          // the slab's own rows only (h->row0, h->row1)
+  if (h->np > 0) launch_refill_commit(h, sp, S, false);
+  std::swap(h->A, h->B);
+  h->steps_done++;
+  return LBM_OK;
+}
+
+int lbm_slab_check(lbm_t* h) {
+  if (!h) return LBM_E_ARG;
+  DeviceGuard dg(h);
+  return check_status(h);
+}
+
+// side 0: the slab's lowest `halo` own rows (what the slab below needs), 1: its highest
+int lbm_slab_pack(lbm_t* h, int side, double* dev_buf) {
+  if (!h || !dev_buf || (side != 0 && side != 1)) return LBM_E_ARG;
+  if (!h->is_slab) return fail(h, LBM_E_STATE, "lbm_slab_pack: not a slab handle");
+  DeviceGuard dg(h);
+  const int sr = side == 0 ? h->row0 : h->row1 - h->halo;
+  if (copy_rows(nullptr, nullptr, 0, h, h->A, sr, h->halo, dev_buf, nullptr, h->stream))
+    return fail(h, LBM_E_CUDA, "lbm_slab_pack: copy failed");
+  return LBM_OK;
+}
+
+// side 0: into the ghost rows below the own rows, 1: above
+int lbm_slab_unpack(lbm_t* h, int side, const double* dev_buf) {
+  if (!h || !dev_buf || (side != 0 && side != 1)) return LBM_E_ARG;
+  if (!h->is_slab) return fail(h, LBM_E_STATE, "lbm_slab_unpack: not a slab handle");
+  if ((side == 0 && h->row0 == 0) || (side == 1 && h->row1 == h->ny))
+    return fail(h, LBM_E_ARG, "lbm_slab_unpack: no ghost rows on that side (cavity wall)");
+  DeviceGuard dg(h);
+  const int dr = side == 0 ? h->row0 - h->halo : h->row1;
+  if (copy_rows(h, h->A, dr, h, nullptr, 0, h->halo, nullptr, dev_buf, h->stream))
+    return fail(h, LBM_E_CUDA, "lbm_slab_unpack: copy failed");
+  return LBM_OK;
+}
+
+// Both exchanges for slabs that live in ONE process (ascending row ranges, e.g. the GPUs of one
+// node driven by one process, or several slabs on one GPU in the tests): the halo rows go straight
+// from copy to copy (peer copies between devices); the force buffers are added in ascending slab
+// order -- each entry is non-zero in exactly one slab, so the sum is that slab's value exactly.
+int lbm_slab_exchange_halos(lbm_t** hs, int n) {
+  if (!hs || n < 1) return LBM_E_ARG;
+  for (int s = 0; s < n; ++s) {
+    if (!hs[s] || !hs[s]->is_slab) return LBM_E_ARG;
+    CUDA_OK(hs[s], cudaStreamSynchronize(hs[s]->stream));   // every slab's step has completed
+  }
+  for (int s = 0; s + 1 < n; ++s) {
+    lbm *lo = hs[s], *up = hs[s + 1];
+    if (lo->own1 != up->own0 || lo->halo != up->halo || lo->px != up->px)
+      return fail(lo, LBM_E_ARG, "lbm_slab_exchange_halos: slabs %d and %d do not adjoin", s, s + 1);
+    // the lower slab's highest own rows -> the upper slab's ghost rows below, and back
+    if (copy_rows(up, up->A, up->row0 - up->halo, lo, lo->A, lo->row1 - lo->halo, lo->halo, nullptr, nullptr, up->stream) ||
+        copy_rows(lo, lo->A, lo->row1, up, up->A, up->row0, up->halo, nullptr, nullptr, lo->stream))
+      return fail(lo, LBM_E_CUDA, "lbm_slab_exchange_halos: copy failed");
+  }
+  for (int s = 0; s < n; ++s) CUDA_OK(hs[s], cudaStreamSynchronize(hs[s]->stream));
+  return LBM_OK;
+}
+
+int lbm_slab_combine_forces(lbm_t** hs, int n) {
+  if (!hs || n < 1 || !hs[0]) return LBM_E_ARG;
+  const int cnt = 3 * hs[0]->np;
+  if (cnt == 0) return LBM_OK;
+  for (int s = 0; s < n; ++s) {
+    if (!hs[s] || !hs[s]->is_slab || hs[s]->np != hs[0]->np || hs[s]->device != hs[0]->device)
+      return LBM_E_ARG;
+    CUDA_OK(hs[s], cudaStreamSynchronize(hs[s]->stream));
+  }
+  cudaStream_t S = hs[0]->stream;
+  for (int s = 1; s < n; ++s) launch_add_buffer(hs[0]->force_buf, hs[s]->force_buf, cnt, S);
+  for (int s = 1; s < n; ++s)
+    CUDA_OK(hs[0], cudaMemcpyAsync(hs[s]->force_buf, hs[0]->force_buf, cnt * sizeof(double),
+                                   cudaMemcpyDeviceToDevice, S));
+  CUDA_OK(hs[0], cudaStreamSynchronize(S));
+  return LBM_OK;
+}
+
 int lbm_set_graph(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
   h->use_graph = (on && h->cap_stream) ? 1 : 0;
@@ -888,7 +1101,10 @@ int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, dou
                    unsigned char* flag) {
   if (!h) return LBM_E_ARG;
   DeviceGuard dg(h);
-  const size_t n = (size_t)h->nx * h->ny;
+  // a slab hands out its OWN rows only (nx * (j1 - j0) values per field, global row j0 first)
+  const size_t n = (size_t)h->nx * h->ny;                 // nodes stored
+  const size_t m = (size_t)h->nx * (h->row1 - h->row0);   // nodes handed out
+  const size_t o0 = (size_t)h->nx * h->row0;
   if (rho || ux || uy || T) {
     // B is dead between steps: use four of its planes as dense scratch
     double* s0 = h->B;
@@ -896,10 +1112,10 @@ int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, dou
     double* s2 = h->B + 2 * h->ps;
     double* s3 = h->B + 3 * h->ps;
     launch_macroscopic(h, s0, s1, s2, s3);
-    if (rho) CUDA_OK(h, cudaMemcpyAsync(rho, s0, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    if (ux) CUDA_OK(h, cudaMemcpyAsync(ux, s1, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    if (uy) CUDA_OK(h, cudaMemcpyAsync(uy, s2, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    if (T) CUDA_OK(h, cudaMemcpyAsync(T, s3, n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (rho) CUDA_OK(h, cudaMemcpyAsync(rho, s0 + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (ux) CUDA_OK(h, cudaMemcpyAsync(ux, s1 + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (uy) CUDA_OK(h, cudaMemcpyAsync(uy, s2 + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (T) CUDA_OK(h, cudaMemcpyAsync(T, s3 + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
   }
   if (f || g) {
     // f, g are defined as the post-collision populations; before the first step the resident
@@ -909,11 +1125,19 @@ int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, dou
     double* fd = h->B;
     double* gd = h->B + 9 * n;
     launch_export(h, f ? fd : nullptr, g ? gd : nullptr);
-    if (f) CUDA_OK(h, cudaMemcpyAsync(f, fd, 9 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-    if (g) CUDA_OK(h, cudaMemcpyAsync(g, gd, 5 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (m == n) {
+      if (f) CUDA_OK(h, cudaMemcpyAsync(f, fd, 9 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      if (g) CUDA_OK(h, cudaMemcpyAsync(g, gd, 5 * n * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    } else {
+      for (int k = 0; f && k < 9; ++k)
+        CUDA_OK(h, cudaMemcpyAsync(f + k * m, fd + k * n + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      for (int k = 0; g && k < 5; ++k)
+        CUDA_OK(h, cudaMemcpyAsync(g + k * m, gd + k * n + o0, m * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    }
   }
   if (flag)
-    CUDA_OK(h, cudaMemcpy2DAsync(flag, h->nx, h->flag, h->px, h->nx, h->ny, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_OK(h, cudaMemcpy2DAsync(flag, h->nx, h->flag + (size_t)h->row0 * h->px, h->px, h->nx,
+                                 h->row1 - h->row0, cudaMemcpyDeviceToHost, h->stream));
   CUDA_OK(h, cudaStreamSynchronize(h->stream));
   CUDA_OK(h, cudaGetLastError());
   return LBM_OK;

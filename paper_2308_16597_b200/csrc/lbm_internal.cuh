@@ -52,7 +52,11 @@ __host__ __device__ __forceinline__ long long g_at(int k, long long x, long long
 
 // constants every kernel needs; passed by value (lands in the constant bank)
 struct LbmConst {
-  int nx, ny, px;          // lattice size, row pitch (doubles)
+  int nx, ny, px;          // lattice size (rows this handle stores), row pitch (doubles)
+  // y-slabs: the handle stores the global rows [yoff, yoff + ny)
+  // of a cavity NY rows high.  Particle coordinates, link nodes and every row index the particle
+  // kernels compute with are GLOBAL; only memory indices are local.  Single domain: 0, ny.
+  int yoff, NY;
   long long ps;            // plane stride (doubles)
   int periodic_x;
   // D2Q9 MRT (DESIGN.md readings): relaxation rates and the (1 - s/2) forcing factors
@@ -87,7 +91,11 @@ struct LinkArrays {          // the paper's fixed index array: segment p = [p*ca
 };
 
 struct lbm {
-  int nx, ny, px;
+  int nx, ny, px;            // ny: rows stored by this handle
+  // y-slab (lbm_create_slab): global rows [yoff, yoff + ny) of a cavity NY rows high are stored,
+  // the own rows [own0, own1) (global) are updated, `halo` ghost rows on each interior side.
+  // row0, row1: the own rows as LOCAL indices.  A single domain: 0, ny, 0, ny, halo 0.
+  int is_slab, yoff, NY, own0, own1, halo, row0, row1;
   long long ps;
   lbm_params P;
   LbmConst C;
@@ -126,6 +134,7 @@ struct lbm {
   // two-step band: band[0] = Q, rows
   // [0, Q) are advanced two steps per pass; band[1] = 0 (what the plain schedule's kernels read)
   int* band;
+  double* force_buf;         // y-slabs: 3 * max_particles doubles (Fx, Fy, Tz), the slab's share of the force combine
   int band_hint;             // rows certainly inside the band as the host last saw it (sizes the one-step grid; 0 = unknown)
   int band_live;             // the step being enqueued belongs to a banded period (k_cover checks the margin)
   int band_cap;              // most rows the band may have in this call (sizes the band kernel's grid)
@@ -160,6 +169,14 @@ struct lbm {
   int ev_n[K_COUNT];
   char err[512];
 };
+
+// global row j of the cavity: is it stored by this handle, and where
+__host__ __device__ __forceinline__ bool row_here(const LbmConst& c, int j) {
+  return j >= c.yoff && j < c.yoff + c.ny;
+}
+__host__ __device__ __forceinline__ long long node_index(const LbmConst& c, int i, int j) {
+  return (long long)(j - c.yoff) * c.px + i;
+}
 
 // ---- programmatic dependent launch (PDL).  Every kernel of the step's serial chain starts with
 // pdl_wait(): launched with the programmatic-serialisation attribute it may begin while its
@@ -207,7 +224,10 @@ void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
 void launch_move(lbm* h, cudaStream_t st, bool pdl);   // integrator + uncover, buffer cur -> cur ^ 1
 int particles_configure(lbm* h);           // per-handle kernel attributes (0 = ok)
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
-void launch_band_plan(lbm* h, cudaStream_t st);   // h->band[0] from the positions of buffer h->cur
+void launch_band_plan(lbm* h, cudaStream_t st);
+void launch_slab_forces_out(lbm* h);   // owned particles' F, T_z -> h->force_buf (zeros for the others)
+void launch_slab_forces_in(lbm* h);    // h->force_buf (combined over the slabs) -> F, T_z
+void launch_add_buffer(double* dst, const double* src, int n, cudaStream_t st);   // h->band[0] from the positions of buffer h->cur
 // bounce_back.cu
 void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl);
 void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped

@@ -200,8 +200,8 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
       int a1 = 0, n1 = 0, a2 = 0, n2 = 0;
       const double dy = (double)j - yc, dy2 = dy * dy;
       if (S.ell) {                                // first version: every column of the zone row
-        if (j >= 0 && j < c.ny && ihi >= ilo) { a1 = ilo; n1 = ihi - ilo + 1; }
-      } else if (j >= 0 && j < c.ny && dy2 <= rfar) {
+        if (row_here(c, j) && ihi >= ilo) { a1 = ilo; n1 = ihi - ilo + 1; }
+      } else if (row_here(c, j) && dy2 <= rfar) {
         const double wo = sqrt(rfar - dy2);
         const int oa = max((int)floor(xc - wo) - 1, ilo), ob = min((int)floor(xc + wo) + 2, ihi);
         int ha = ob + 1, hb = ob;                 // hole = columns certainly inside the disc
@@ -266,7 +266,7 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
       const double xi = (double)i, yj = (double)j;
       if (S.ell) {
         if (inside_ellipse(xi, yj, S)) continue;
-        const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.ny - 1;
+        const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.NY - 1;
         unsigned m = 0;
         if (ei && inside_ellipse(xi + 1.0, yj, S)) m |= 1u << 1;
         if (no && inside_ellipse(xi, yj + 1.0, S)) m |= 1u << 2;
@@ -287,7 +287,7 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
       const double dxm = (xi - 1.0) - xc, dxp = (xi + 1.0) - xc;
       const double dym = (yj - 1.0) - yc, dyp = (yj + 1.0) - yc;
       const double sxm = dxm * dxm, sxp = dxp * dxp, sym = dym * dym, syp = dyp * dyp;
-      const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.ny - 1;
+      const bool wi = i > 0, ei = i < c.nx - 1, so = j > 0, no = j < c.NY - 1;
       unsigned m = 0;
       if (ei && sxp + sy0 <= r2) m |= 1u << 1;
       if (no && sx0 + syp <= r2) m |= 1u << 2;
@@ -304,7 +304,7 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
     unsigned char fl[LB_CPT];
 #pragma unroll
     for (int k = 0; k < LB_CPT; ++k)
-      fl[k] = mask[k] ? flag[(long long)(int)((unsigned)node[k] >> 16) * c.px + (node[k] & 0xffff)] : 1;
+      fl[k] = mask[k] ? flag[node_index(c, node[k] & 0xffff, (int)((unsigned)node[k] >> 16))] : 1;
 #pragma unroll
     for (int k = 0; k < LB_CPT; ++k)
       if (fl[k] == 1) mask[k] = 0;
@@ -316,7 +316,9 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
         unsigned keep = 0;
         for (unsigned t = mask[k]; t; t &= t - 1) {
           const int al = __ffs(t) - 1;
-          if (owner[(long long)(j + p_ey[al]) * c.px + (i + p_ex[al])] == p) keep |= 1u << al;
+          // (a solid neighbour in a row this slab does not store: the link's parked value is not
+          // needed here and the particle's force is summed by the slab that owns it)
+          if (row_here(c, j + p_ey[al]) && owner[node_index(c, i + p_ex[al], j + p_ey[al])] == p) keep |= 1u << al;
         }
         mask[k] = keep;
       }
@@ -385,10 +387,10 @@ k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag
       a1 = (a1 + c.nx) % c.nx;
       a2 = (a2 + c.nx) % c.nx;
     }
-    const bool in1 = a1 >= 0 && a1 < c.nx && b1 >= 0 && b1 < c.ny;
-    const bool in2 = a2 >= 0 && a2 < c.nx && b2 >= 0 && b2 < c.ny;
-    const unsigned char f1 = in1 ? flag[(long long)b1 * c.px + a1] : 1;
-    const unsigned char f2 = in2 ? flag[(long long)b2 * c.px + a2] : 1;
+    const bool in1 = a1 >= 0 && a1 < c.nx && row_here(c, b1);
+    const bool in2 = a2 >= 0 && a2 < c.nx && row_here(c, b2);
+    const unsigned char f1 = in1 ? flag[node_index(c, a1, b1)] : 1;
+    const unsigned char f2 = in2 ? flag[node_index(c, a2, b2)] : 1;
     const int behind = f1 == 1 ? 0 : (f2 == 1 ? 1 : 2);
     la.q[base + s] = S.ell ? link_q_ellipse((double)i, (double)j, al, S)
                            : link_q((double)i, (double)j, al, xc, yc, r);
@@ -540,7 +542,7 @@ __device__ __forceinline__ void integrate_particle(const ParticleArrays& pa, int
   }
   const double dS = (ay + 0.5) - ahy;
   if (dS <= c.rep_s) Fy += repulsion_mag(Ca, c, dS);
-  const double dN = ((double)c.ny - 0.5 - ay) - ahy;
+  const double dN = ((double)c.NY - 0.5 - ay) - ahy;
   if (dN <= c.rep_s) Fy -= repulsion_mag(Ca, c, dN);
 
   double x = ax, y = ay, th = pa.theta[cur][ia];
@@ -589,7 +591,7 @@ template <typename F>
 __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const LbmConst& c, F f) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int j = j0 + warp; j <= j1; j += PT / 32) {
-    if (j < 0 || j >= c.ny) continue;
+    if (!row_here(c, j)) continue;
     for (int i = i0 + lane; i <= i1; i += 32)
       if (i >= 0 && i < c.nx) f(i, j);
   }
@@ -631,7 +633,7 @@ k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
     if (!inside_shape((double)i, (double)j, So)) return;
     if (inside_shape((double)i, (double)j, Sn)) return;
-    const long long x = (long long)j * c.px + i;
+    const long long x = node_index(c, i, j);
     if (owner[x] != p) return;
     owner[x] = OWNER_NONE;
     flag[x] = 2;
@@ -690,7 +692,7 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
   for_zone(i0, i1, j0, j1, c, [&](int i, int j) {
     if (!inside_shape((double)i, (double)j, Sn)) return;
     if (!sweep && inside_shape((double)i, (double)j, So)) return;   // already ours
-    const long long x = (long long)j * c.px + i;
+    const long long x = node_index(c, i, j);
     if (owner[x] == p) return;
     const int prev = atomicMin(&owner[x], p);
     if (prev != p) flag[x] = 1;
@@ -732,6 +734,35 @@ k_band_plan(ParticleArrays pa, int cur, int np, int ny, int qcap, int* __restric
     if (Q < BAND_MIN) Q = 0;
     band[0] = Q;
   }
+}
+
+// ------------------------------------------------------------------------------------------
+// y-slabs: the force combine.  Every slab runs the bounce-back kernel on the links it can see, but
+// only the slab whose own rows [own0, own1) hold a particle's centre sees ALL of its links (the
+// halo is wider than r + 8): that slab's sum, in the single domain's order, is the particle's
+// force; every other slab contributes zero.  buf = Fx[np], Fy[np], Tz[np].
+__global__ void k_slab_forces_out(ParticleArrays pa, int cur, int np, int own0, int own1,
+                                  double* __restrict__ buf) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  const double y = pa.y[cur][p];
+  const bool mine = y >= (double)own0 && y < (double)own1;
+  buf[p] = mine ? pa.Fx[p] : 0.0;
+  buf[np + p] = mine ? pa.Fy[p] : 0.0;
+  buf[2 * np + p] = mine ? pa.Tz[p] : 0.0;
+}
+
+__global__ void k_slab_forces_in(ParticleArrays pa, int np, const double* __restrict__ buf) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  pa.Fx[p] = buf[p];
+  pa.Fy[p] = buf[np + p];
+  pa.Tz[p] = buf[2 * np + p];
+}
+
+__global__ void k_add_buffer(double* __restrict__ dst, const double* __restrict__ src, int n) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n) dst[k] = dst[k] + src[k];
 }
 
 } // namespace
@@ -815,4 +846,20 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
 void launch_band_plan(lbm* h, cudaStream_t st) {
   h->launches++;
   k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_cap, h->band);
+}
+
+void launch_slab_forces_out(lbm* h) {
+  if (h->np == 0) return;
+  h->launches++;
+  k_slab_forces_out<<<(h->np + 255) / 256, 256, 0, h->stream>>>(h->pa, h->cur, h->np, h->own0, h->own1, h->force_buf);
+}
+
+void launch_slab_forces_in(lbm* h) {
+  if (h->np == 0) return;
+  h->launches++;
+  k_slab_forces_in<<<(h->np + 255) / 256, 256, 0, h->stream>>>(h->pa, h->np, h->force_buf);
+}
+
+void launch_add_buffer(double* dst, const double* src, int n, cudaStream_t st) {
+  if (n > 0) k_add_buffer<<<(n + 255) / 256, 256, 0, st>>>(dst, src, n);
 }

@@ -161,7 +161,7 @@ constexpr int SC_FILL = 8;
 __global__ void __launch_bounds__(SC_THREADS, 9)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
                  const unsigned char* __restrict__ flag, const double* __restrict__ Alow,
-                 const int* __restrict__ bandp, int delta, const LbmConst c) {
+                 const int* __restrict__ bandp, int delta, int row0, int row1, const LbmConst c) {
   // programmatic dependent launch along the caller's stream: the next lattice kernel's CTAs may
   // come up as this grid's last wave drains; every kernel waits here for its predecessor's data
   pdl_launch_dependents();
@@ -171,7 +171,8 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   // The grid has one CTA row per lattice row the host EXPECTS this launch to cover (it knows the
   // band height of the previous lbm_step call); the loop takes care of a band that has shrunk
   // since (normally it runs once).
-  for (int j = blockIdx.y + (Q > 0 ? Q + delta : 0); j < c.ny; j += gridDim.y) {
+  // [row0, row1): the rows this launch may update at all (the whole lattice; a y-slab: its own rows)
+  for (int j = blockIdx.y + max(row0, Q > 0 ? Q + delta : 0); j < row1; j += gridDim.y) {
     const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
     if (j <= Q && Q > 0) {                       // the two rows along the seam (all fluid)
       if (fluid) {
@@ -350,7 +351,7 @@ __global__ void k_macroscopic(const double* __restrict__ A, const unsigned char*
   if (flag[x] != 0) {
     const int p = owner[x];
     rho[o] = c.rho0;
-    ux[o] = pux[p] - pom[p] * ((double)j - py_[p]);
+    ux[o] = pux[p] - pom[p] * ((double)(j + c.yoff) - py_[p]);
     uy[o] = puy[p] + pom[p] * ((double)i - px_[p]);
     T[o] = pTw[p];
     return;
@@ -405,10 +406,10 @@ void launch_stream_collide(lbm* h, int band, const double* low) {
   h->launches++;
   // banded steps: one CTA row per lattice row above the band as the host last saw it
   // (h->band_hint, 0 = unknown); the kernel's row loop covers whatever the band has lost since
-  const int rows = band ? h->ny - h->band_hint : h->ny;
+  const int rows = band ? h->ny - h->band_hint : h->row1 - h->row0;
   launch_k(k_stream_collide, grid_rows(h->px, rows, SC_THREADS), dim3(SC_THREADS), 0, h->stream, h->use_pdl != 0,
            (const double*)h->A, h->B, (const unsigned char*)h->flag, band == 1 ? low : (const double*)nullptr,
-           (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->C);
+           (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->row0, h->row1, h->C);
 }
 
 int stream_collide_configure() {
