@@ -140,7 +140,7 @@ struct lbm {
   int band_cap;              // most rows the band may have in this call (sizes the band kernel's grid)
   int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
   cudaEvent_t ev_p2;         // the band kernel's part of a step has been issued (the particle chain follows it)
-  cudaEvent_t ev_plan, ev_l1;
+  cudaEvent_t ev_plan;       // the band plan of a period has been issued (the caller's stream follows it)
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
   long long steps_done;
   long long launches;        // kernels launched (lbm_kernel_launches)

@@ -140,11 +140,13 @@ __device__ __forceinline__ void update_node(const double* __restrict__ A, double
 
 // One thread per node, 128-thread CTAs along x.  Solid (1) and newborn (2) nodes do no lattice
 // update.  DRAM moves whole 32-byte sectors, and a partially written sector costs a read-modify-
-// write there, so a non-fluid lane whose aligned group of SC_FILL lanes (= SC_FILL * 8 bytes of
-// every plane) holds at least one fluid lane stores zeros: slots of non-fluid nodes in B are
-// don't-care (a parked value is written by the NEXT step's bounce-back kernel, a newborn node by
-// this step's refill kernel, both ordered after this kernel), and every store of the kernel then
-// covers complete sectors.
+// write there, so a non-fluid lane stores zeros into every plane in which its aligned 32-byte
+// sector (2 lanes of a pair plane, 4 lanes of a diagonal plane) also holds a fluid lane: slots of
+// non-fluid nodes in B are don't-care (a parked value is written by the NEXT step's bounce-back
+// kernel, a newborn node by this step's refill kernel, both ordered after this kernel), and every
+// store of the kernel then covers complete sectors.  Measured on config 3 (plain schedule, kernel
+// alone): no fill 572 us; groups of 8 lanes in every plane 522 us; 4 lanes 518 us; one sector per
+// plane type (2 / 4 lanes) 516 us; half a sector (1 / 2 lanes) 536 us.
 //
 // The flag update of this step (k_uncover / k_cover on the chain stream) may run concurrently:
 // a node it covers (0 -> 1) was fluid at t, so updating it or not are both fine (its B slot is
@@ -157,7 +159,8 @@ __device__ __forceinline__ void update_node(const double* __restrict__ A, double
 // to the spare row ny of B; rows below Q are read from the band's copy Alow.  In the second step
 // (delta = 0, Alow = nullptr) row Q-1 is read from the spare row of A.  Rows Q-1 and Q take the
 // generic pull; everything above is untouched by the band.  Q = 0: no band.
-constexpr int SC_FILL = 8;
+constexpr int SC_FILL_PAIR = 2;   // lanes of one 32-byte sector of a pair plane (16 B per node)
+constexpr int SC_FILL_DIAG = 4;   // lanes of one 32-byte sector of a diagonal plane (8 B per node)
 __global__ void __launch_bounds__(SC_THREADS, 9)
 k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
                  const unsigned char* __restrict__ flag, const double* __restrict__ Alow,
@@ -190,15 +193,19 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
       continue;
     }
     const unsigned lane = threadIdx.x & 31u;
-    const unsigned grp = (m >> (lane & ~(unsigned)(SC_FILL - 1))) & ((1u << SC_FILL) - 1u);
-    if (grp == 0u || i >= c.px) continue;
+    if (i >= c.px) continue;
     const long long x = (long long)j * c.px + i;
-    double* __restrict__ O = B + 2 * x;
+    // pair planes: SC_FILL_PAIR lanes x 16 B; diagonal planes: SC_FILL_DIAG lanes x 8 B
+    if ((m >> (lane & ~(unsigned)(SC_FILL_PAIR - 1))) & ((1u << SC_FILL_PAIR) - 1u)) {
+      double* __restrict__ O = B + 2 * x;
 #pragma unroll
-    for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
-    double* __restrict__ Q4 = B + 10 * c.ps + x;
+      for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
+    }
+    if ((m >> (lane & ~(unsigned)(SC_FILL_DIAG - 1))) & ((1u << SC_FILL_DIAG) - 1u)) {
+      double* __restrict__ Q4 = B + 10 * c.ps + x;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
+      for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
+    }
   }
 }
 
