@@ -139,7 +139,7 @@ int lbm_set_graph(lbm_t* h, int on);
  * arithmetic per step is the same, so results are identical bit for bit to on = 0. */
 int lbm_set_two_step(lbm_t* h, int on);
 
-/* on = 1 (default; LBM_BAND=0 turns the default off): lattices WITH particles also use the
+/* on = 1 (default; the environment variable LBM_BAND = 0 / 1 / 2 sets the default): lattices WITH particles also use the
  * two-steps-per-pass kernel, on the particle-free rows [0, Q) below the lowest particle (SURVEY
  * 8(f)-4), in lbm_step calls of at least 16
  * steps (such a call plans the band once on entry to size its grids: one more synchronisation).
@@ -148,6 +148,8 @@ int lbm_set_two_step(lbm_t* h, int on);
  * rows: no band), the band is advanced t -> t+2 -> t+4 by the two-step kernel while the rows
  * above it take four ordinary steps, the two meeting in one row that is computed by both.  The
  * arithmetic per node and step is unchanged: results are identical bit for bit to on = 0.
+ * on = 1 uses a band only if it holds at least 2^18 nodes (below that its extra launches cost more
+ * than the traffic it saves); on = 2 uses every band of at least 28 rows (the tests).
  * lbm_get_band: *rows = Q of the last banded period completed by lbm_step (0: none). */
 int lbm_set_band(lbm_t* h, int on);
 int lbm_get_band(lbm_t* h, int* rows);

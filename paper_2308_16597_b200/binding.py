@@ -234,7 +234,8 @@ class Simulation:
         self._chk(self._L.lbm_set_graph(self._h, 1 if on else 0))
 
     def set_band(self, on=True):
-        self._chk(self._L.lbm_set_band(self._h, 1 if on else 0))
+        """False / 0: off; True / 1: where it pays (bands of >= 2^18 nodes); 2: every band."""
+        self._chk(self._L.lbm_set_band(self._h, int(on)))
 
     def band_rows(self):
         """Rows [0, Q) the last banded period advanced two steps per pass (0: none)."""

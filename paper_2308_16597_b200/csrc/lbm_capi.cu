@@ -40,6 +40,7 @@ int fail(lbm* h, int code, const char* fmt, ...) {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+constexpr long long LBM_BAND_MIN_NODES = 1LL << 18;
 constexpr int LBM_BAND_MIN_STEPS = 16;   // shortest lbm_step call that uses the two-step band
 constexpr int LBM_GRAPH_STEPS = 8;   // time steps per graph launch (an even number: one or more periods)
 
@@ -397,7 +398,7 @@ static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, 
   h->status_host[1] = 0;
   {
     const char* eb = getenv("LBM_BAND");
-    h->band_on = (eb && atoi(eb) == 0) ? 0 : 1;
+    h->band_on = eb ? std::min(std::max(atoi(eb), 0), 2) : 1;   // 0 off, 1 where it pays, 2 every band
     if (cudaEventCreateWithFlags(&h->ev_p2, cudaEventDisableTiming) != cudaSuccess) {
       cudaGetLastError();
       h->band_on = 0;
@@ -865,7 +866,8 @@ int lbm_step(lbm_t* h, int nsteps) {
     CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaStreamSynchronize(h->stream));
     const int q0 = h->status_host[1];
-    if (q0 <= 0) band_ok = false;
+    // a band of less than 2^18 nodes costs more in launches than it saves in traffic (config 0)
+    if (q0 <= 0 || (h->band_on < 2 && (long long)q0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
     else {
       const char* eh = getenv("LBM_HINT_SLACK");
       const int hs = eh ? atoi(eh) : 96, hq = hs >= 64 ? 64 : 32;
@@ -918,7 +920,7 @@ int lbm_step(lbm_t* h, int nsteps) {
 
 int lbm_set_band(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
-  h->band_on = on ? 1 : 0;
+  h->band_on = (on && h->ev_p2 && !h->is_slab) ? (on >= 2 ? 2 : 1) : 0;
   return LBM_OK;
 }
 

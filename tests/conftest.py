@@ -9,6 +9,12 @@ for p in (ROOT, os.path.join(ROOT, "oracle")):
         sys.path.insert(0, p)
 
 
+# The tests' lattices are small: use the two-step band wherever there are 28 free rows, not only
+# where it pays (include/lbm.h lbm_set_band), so that every parity test below a suspension also
+# exercises the banded schedule.  The full-size configs use their bands under either setting.
+os.environ.setdefault("LBM_BAND", "2")
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
 

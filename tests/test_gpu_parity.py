@@ -526,6 +526,8 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
     ref.set_band(False)
     ref.set_graph(False)
     sims = [gpu.Simulation.from_workload(w) for _ in range(3)]
+    for s_ in sims:
+        s_.set_band(2)                               # every band, however small the lattice
     sims[1].set_graph(False)                         # direct launches (the profiling path)
     sims[2].set_overlap(False)                       # one stream
     q_seen = []
@@ -550,6 +552,7 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
                  uy=np.array([-0.05]), omega=np.array([0.0]))
     w2 = wl.Workload("band_vanishes", 120, 150, p, 1, 1, particles=parts)
     a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
+    a.set_band(2)
     b.set_band(False)
     qs = []
     for nst in (16, 16, 24, 40, 200):         # (calls shorter than 16 steps never use the band)

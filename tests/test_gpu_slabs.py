@@ -138,3 +138,25 @@ def test_one_rank_slab_runner_equals_the_single_domain(gpu, wl):
     for k in pb:
         assert np.array_equal(pa[k], pb[k]), k
     sr.close()
+
+
+def test_ellipses_across_a_cut(gpu, wl):
+    """Elliptical particles (their zone, support-function repulsion and gradient refill normal use
+    global coordinates too) straddling and crossing the cut of two slabs: bit-identical."""
+    from paper_2308_16597_b200 import slabs
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=4,
+             max_links_per_particle=wl.max_links_for_diameter(26.0))
+    parts = dict(x=np.array([50.2, 110.0, 160.5, 90.0]), y=np.array([121.0, 128.3, 112.0, 170.0]),
+                 diam=np.array([26.0, 20.0, 18.0, 14.0]), minor=np.array([13.0, 12.0, 18.0, 14.0]),
+                 theta=np.array([0.4, -1.1, 0.0, 0.0]), rho_ratio=np.full(4, 1.5), T_w=np.full(4, 1.0),
+                 ux=np.zeros(4), uy=np.array([-0.04, -0.02, 0.05, -0.06]),
+                 omega=np.array([2e-3, -1e-3, 0.0, 1e-3]))
+    w = wl.Workload("ellipse_slabs", 220, 240, p, 1, 1, particles=parts)
+    grp = slabs.SlabGroup(w, 2)                       # cut at row 120
+    dom = gpu.Simulation.from_workload(w)
+    for nst in (1, 60, 300):
+        grp.step(nst)
+        dom.step(nst)
+        assert_group_equals_domain(grp, dom)
+    grp.close()
