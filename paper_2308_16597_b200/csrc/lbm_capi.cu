@@ -708,7 +708,9 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     // the particle chain holds register space the band kernel's large CTAs need (measured: the band
     // part takes 115 us beside the bounce-back kernel alone, 190 us beside the chain): the chain
     // starts after the band's part and still has the whole one-step kernel to hide under
-    if (fork) {
+    // (a short, unthrottled chain -- few particles -- does not starve it and is itself the
+    // critical path: no hold)
+    if (fork && h->chain_ctas > 0) {
       cudaEventRecord(h->ev_p2, S0);
       cudaStreamWaitEvent(S1, h->ev_p2, 0);
     }
