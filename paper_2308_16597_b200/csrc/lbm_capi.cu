@@ -255,11 +255,13 @@ int check_status(lbm* h) {
 
 // CTAs of a particle-chain kernel while it runs under the lattice kernel (DESIGN.md "Step
 // schedule").  Measured on B200: the lattice kernel keeps its speed when other work holds up to
-// two of its nine CTA slots per SM and loses 7 % at three; a chain CTA under a saturated memory
-// system needs about 30 us per d = 20 particle for its three zone kernels (about 70 us at d = 40).
-// Pick the fewest CTAs per SM (at least 2) with which the chain still ends within 70 % of the
-// lattice kernel's expected duration (224 B per node at 6 TB/s); LBM_CHAIN_CTAS_PER_SM overrides
-// (0 = one CTA per particle).
+// two of its nine 128-thread CTA slots per SM and loses 7 % at three; a 64-thread chain CTA under a
+// saturated memory system needs about 45 us per d = 20 particle for its three zone kernels (75 us
+// at d = 40).  Pick the fewest CTAs per SM (at least 2) with which the chain still ends within
+// 50 % of the time the lattice kernel needs for the WHOLE lattice (224 B per node at 6 TB/s) --
+// with a two-step band below the suspension the kernel covers about two thirds of it.
+// Configs 3 and 4: 5 and 6 per SM, the paper's d = 40 workload: 9.  LBM_CHAIN_CTAS_PER_SM
+// overrides (0 = one CTA per particle).
 void size_chain(lbm* h) {
   if (const char* e = getenv("LBM_CHAIN_CTAS_PER_SM")) {
     h->chain_ctas = atoi(e) * h->sm_count;
@@ -267,9 +269,9 @@ void size_chain(lbm* h) {
   }
   if (h->np == 0) { h->chain_ctas = 0; return; }
   const double sc_us = (double)h->nx * h->ny * 224.0 / 6.0e6;
-  const double tau_us = 30.0 * std::max(1.0, std::pow(h->d_max / 20.0, 1.3));
-  double per_sm = std::ceil(h->np * tau_us / (h->sm_count * 0.7 * sc_us));
-  per_sm = std::min(std::max(per_sm, 2.0), 16.0);
+  const double tau_us = 45.0 * std::max(1.0, std::pow(h->d_max / 20.0, 0.75));
+  double per_sm = std::ceil(h->np * tau_us / (h->sm_count * 0.5 * sc_us));
+  per_sm = std::min(std::max(per_sm, 2.0), 24.0);
   h->chain_ctas = (int)per_sm * h->sm_count;
 }
 
@@ -708,9 +710,7 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     // the particle chain holds register space the band kernel's large CTAs need (measured: the band
     // part takes 115 us beside the bounce-back kernel alone, 190 us beside the chain): the chain
     // starts after the band's part and still has the whole one-step kernel to hide under
-    // (a short, unthrottled chain -- few particles -- does not starve it and is itself the
-    // critical path: no hold)
-    if (fork && h->chain_ctas > 0) {
+    if (fork) {
       cudaEventRecord(h->ev_p2, S0);
       cudaStreamWaitEvent(S1, h->ev_p2, 0);
     }

@@ -23,7 +23,14 @@ namespace {
 __constant__ int p_ex[9] = {0, 1, 0, -1, 0, 1, -1, -1, 1};
 __constant__ int p_ey[9] = {0, 0, 1, 0, -1, 1, 1, -1, -1};
 
-constexpr int PT = 128;   // threads per particle CTA
+// Threads per particle CTA: PT_MAX when a kernel has the GPU to itself (one CTA per particle: the
+// single particle's latency counts), PT_THROTTLED for the few persistent CTAs per SM that run
+// under the lattice kernel: a chain kernel is bound by the latency of its dependent loads, not by
+// threads, and 64-thread CTAs put twice as many particles in flight per register taken from the
+// lattice kernel (r28, r33: config 3 538 -> 533 us, config 5 535 -> 520 us; alone, or on the small
+// configs, 64 threads are slower: config 2 50.7 -> 54.4 us).
+constexpr int PT_MAX = 128;
+constexpr int PT_THROTTLED = 64;
 
 __device__ __forceinline__ bool inside_disc(double xi, double yj, double xc, double yc, double r) {
   const double dx = xi - xc, dy = yj - yc;
@@ -159,16 +166,15 @@ __device__ __forceinline__ double support_shape(const Shape& S, double nx, doubl
 //      shuffle), emission in row-major order (neighbouring links -> neighbouring nodes for the
 //      bounce-back kernel) into shared memory;
 //   5. q and the ladder rung per link, one link per thread, both flag bytes requested together.
-constexpr int LB_WARPS = 4;
-constexpr int LB_T = LB_WARPS * 32;
 constexpr int LB_CPT = 4;
-template <bool ELL>
-__global__ void __launch_bounds__(LB_T)
+template <bool ELL, int LB_WARPS>
+__global__ void __launch_bounds__(LB_WARPS * 32)
 k_build_links(ParticleArrays pa, int buf, const unsigned char* __restrict__ flag,
               const int* __restrict__ owner, LinkArrays la, int np, int max_rows,
               int* __restrict__ status, int early, const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();
+  constexpr int LB_T = LB_WARPS * 32;
   extern __shared__ int s_node[];                           // la.cap packed nodes, la.cap dir bytes,
   unsigned char* s_dir = (unsigned char*)(s_node + la.cap); // then the row tables
   int* s_off = s_node + la.cap + (la.cap + 3) / 4;          // max_rows + 1: candidates before row t
@@ -590,7 +596,7 @@ __device__ __forceinline__ void integrate_particle(const ParticleArrays& pa, int
 template <typename F>
 __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const LbmConst& c, F f) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int j = j0 + warp; j <= j1; j += PT / 32) {
+  for (int j = j0 + warp; j <= j1; j += (int)(blockDim.x >> 5)) {
     if (!row_here(c, j)) continue;
     for (int i = i0 + lane; i <= i1; i += 32)
       if (i >= 0 && i < c.nx) f(i, j);
@@ -608,7 +614,7 @@ __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const L
 // new positions) and appends to the newborn counter of this step (zeroed by the previous step's
 // k_refill_commit).
 template <bool ELL>
-__global__ void __launch_bounds__(PT)
+__global__ void __launch_bounds__(PT_MAX)
 k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
        const int* __restrict__ cell_count_cur, const int* __restrict__ cell_items_cur,
        int* __restrict__ cell_count_nxt, int ncells,
@@ -619,7 +625,7 @@ k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
   __shared__ double s_cfx[32], s_cfy[32];
   if (early) pdl_launch_dependents();
   pdl_wait();
-  for (int k = blockIdx.x * PT + threadIdx.x; k < ncells; k += gridDim.x * PT) cell_count_nxt[k] = 0;
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < ncells; k += gridDim.x * blockDim.x) cell_count_nxt[k] = 0;
   const int nxt = cur ^ 1;
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   if (threadIdx.x < 32)
@@ -661,7 +667,7 @@ k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
 // Thread 0 also enters the particle into the repulsion grid of the step that will use this
 // position (the grid of buffer `buf`; k_move has zeroed its counts).
 template <bool ELL>
-__global__ void __launch_bounds__(PT)
+__global__ void __launch_bounds__(PT_MAX)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
         int* __restrict__ cell_items, int* __restrict__ status, const int* __restrict__ bandp,
@@ -777,10 +783,17 @@ static int chain_grid(const lbm* h, int items, cudaStream_t st) {
   return items;
 }
 
-// Programmatic dependent launch along the chain: a kernel that is NOT throttled (few particles,
-// the launch-latency-bound case) lets its successor's CTAs come up at once -- they wait in
-// griddepcontrol.wait -- so that only the kernel bodies remain on the critical path.  A throttled
-// chain (large lattices) does not: waiting CTAs would hold SM slots the lattice kernel needs.
+// threads of a chain CTA: see PT_MAX / PT_THROTTLED
+static int chain_threads(const lbm* h, int items, cudaStream_t st) {
+  return (st == h->chain_own && h->chain_ctas > 0 && items > h->chain_ctas) ? PT_THROTTLED : PT_MAX;
+}
+
+// Programmatic dependent launch along the chain: every chain kernel waits for its predecessor in
+// griddepcontrol.wait; whether it also lets its successor's CTAs come up at once
+// (launch_dependents at its start).  On the library's chain stream it does not: the waiting CTAs
+// of the queued kernels hold SM slots the lattice kernel -- or, with few particles, the running
+// chain kernel itself -- needs (measured: config 2 50.7 -> 61.6 us with it).  Only set-up launches
+// on the caller's stream and the sequential schedule pass 1 (harmless without the launch attribute).
 static int chain_early(const lbm* h, cudaStream_t st) {
   return (st == h->chain_own && h->chain_ctas > 0) ? 0 : 1;
 }
@@ -796,8 +809,10 @@ void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
   const int max_rows = link_rows(h);
-  launch_k(h->n_ell ? k_build_links<true> : k_build_links<false>, dim3(chain_grid(h, h->np, st)), dim3(LB_T),
-           link_smem(h), st, pdl, h->pa, which_buffer, (const unsigned char*)h->flag, (const int*)h->owner,
+  const int threads = chain_threads(h, h->np, st);
+  auto kernel = threads == PT_MAX ? (h->n_ell ? k_build_links<true, PT_MAX / 32> : k_build_links<false, PT_MAX / 32>)
+                                  : (h->n_ell ? k_build_links<true, PT_THROTTLED / 32> : k_build_links<false, PT_THROTTLED / 32>);
+  launch_k(kernel, dim3(chain_grid(h, h->np, st)), dim3(threads), link_smem(h), st, pdl, h->pa, which_buffer, (const unsigned char*)h->flag, (const int*)h->owner,
            h->la, h->np, max_rows, h->status_dev, chain_early(h, st), h->C);
 }
 
@@ -809,8 +824,10 @@ int particles_configure(lbm* h) {
   const size_t smem = link_smem(h);
   const int dev = (h->device >= 0 && h->device < 64) ? h->device : 0;
   if (smem <= 48 * 1024 || smem <= raised[dev]) return 0;
-  if (cudaFuncSetAttribute(k_build_links<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_build_links<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+  if (cudaFuncSetAttribute(k_build_links<false, PT_MAX / 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_build_links<true, PT_MAX / 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_build_links<false, PT_THROTTLED / 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_build_links<true, PT_THROTTLED / 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
     cudaGetLastError();
     return -1;
   }
@@ -823,7 +840,7 @@ void launch_move(lbm* h, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
   const int c = h->cur;
-  launch_k(h->n_ell ? k_move<true> : k_move<false>, dim3(chain_grid(h, h->np, st)), dim3(PT), 0, st, pdl,
+  launch_k(h->n_ell ? k_move<true> : k_move<false>, dim3(chain_grid(h, h->np, st)), dim3(chain_threads(h, h->np, st)), 0, st, pdl,
            h->pa, c, h->np, h->cell, h->ncx, h->ncy, (const int*)h->cell_count[c],
            (const int*)h->cell_items[c], h->cell_count[c ^ 1], h->ncx * h->ncy, h->flag, h->owner,
            h->newborn_node, h->newborn_pid, h->newborn_count + c, h->newborn_cap, h->status_dev,
@@ -835,7 +852,7 @@ void launch_move(lbm* h, cudaStream_t st, bool pdl) {
 void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   if (h->np == 0) return;
   h->launches++;
-  launch_k(h->n_ell ? k_cover<true> : k_cover<false>, dim3(chain_grid(h, h->np, st)), dim3(PT), 0, st, pdl,
+  launch_k(h->n_ell ? k_cover<true> : k_cover<false>, dim3(chain_grid(h, h->np, st)), dim3(chain_threads(h, h->np, st)), 0, st, pdl,
            h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell, h->ncx, h->ncy,
            h->cell_count[which_buffer], h->cell_items[which_buffer], h->status_dev,
            (const int*)(h->band_live ? h->band : h->band + 1), chain_early(h, st), h->C);
