@@ -270,6 +270,7 @@ def test_coupling_closed_forms_on_the_gpu(gpu, ob, wl):
         assert dom == pytest.approx(Tz / (0.25 * M * (a * a + b * b)), rel=1e-10)
     # (c), (d): the pins themselves, run with the CUDA path standing in for the oracle
     pins.test_repulsion_from_each_of_the_four_walls_in_closed_form(AsGpu(gpu), wl)
+    pins.test_pair_repulsion_of_unequal_discs_uses_the_mean_force_scale(AsGpu(gpu), wl)
     pins.test_ellipse_pair_gap_is_taken_through_the_support_functions(AsGpu(gpu), wl)
     pins.test_upright_ellipse_is_repelled_by_the_bottom_wall_at_its_vertex(AsGpu(gpu), wl)
     # Eq. (14) with a moving wall on a fixed disc (the pin's brute-force case): parity of F, T_z

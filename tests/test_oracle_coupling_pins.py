@@ -238,6 +238,34 @@ def test_repulsion_from_each_of_the_four_walls_in_closed_form(ob, wl):
     assert np.abs(s2.particles()["ux"]).max() < 1e-15
 
 
+def test_pair_repulsion_of_unequal_discs_uses_the_mean_force_scale(ob, wl):
+    """Eq. (15) between two particles (reading 7: the paper defines the force scale
+    C = pi r^2 (rho_p - rho_f) g for a wall only; for a pair the mean of the two is taken, so that
+    the forces are equal and opposite).  Two discs of different radius AND density at surface gap
+    1.2 on a horizontal line, first step from rest (F_hydro = 0): both receive
+    (C_a + C_b) / 2 / eps_w * (s - delta) / s along the line of centres, away from each other, so
+    their momenta change by equal and opposite amounts; gravity acts on y only."""
+    g, s_rep, eps = 1.6e-4, 2.0, 1e-3
+    ra, rb, qa, qb, gap = 5.0, 3.25, 1.5, 1.2, 1.2
+    p = base_params(wl, 2, 2 * ra, g=g, rep_s=s_rep, rep_eps=eps, rep_power=1)
+    o = ob.OracleSim(120, 90, p)
+    xa = 50.0
+    xb = xa + ra + rb + gap
+    o.add_particles(x=[xa, xb], y=[45.0, 45.0], diam=[2 * ra, 2 * rb], rho_ratio=[qa, qb], T_w=[0.0, 0.0])
+    o.step(1)
+    P = o.particles()
+    Aa, Ab = math.pi * ra * ra, math.pi * rb * rb
+    Ca, Cb = Aa * (qa - 1.0) * g, Ab * (qb - 1.0) * g
+    Ma, Mb = qa * Aa, qb * Ab
+    F = 0.5 * (Ca + Cb) / eps * (s_rep - gap) / s_rep
+    assert abs(Ca - Cb) > 0.3 * max(Ca, Cb)             # the two scales differ: own-C readings fail
+    assert P["ux"][0] == pytest.approx(-F / Ma, rel=1e-11)
+    assert P["ux"][1] == pytest.approx(+F / Mb, rel=1e-11)
+    assert Ma * P["ux"][0] + Mb * P["ux"][1] == pytest.approx(0.0, abs=1e-14 * F)
+    assert P["uy"][0] == pytest.approx(-(qa - 1.0) / qa * g, rel=1e-11)
+    assert P["uy"][1] == pytest.approx(-(qb - 1.0) / qb * g, rel=1e-11)
+
+
 # ------------------------------------------------------------------ (d) ellipse gaps
 
 def ellipse_pair(ob, wl, theta_a, theta_b, dist, a=8.0, b=4.0, ratio=1.5, g=1.6e-4, vertical=False):
