@@ -16,9 +16,10 @@ hot particles (seeded synthetic placement, paper_2308_16597_b200/workloads.py).
   roofline      fused stream-collide kernel: algorithmic bytes / its mean CUDA-event duration
   cpu_baseline  the CPU oracle as it stands, timed on this host on a bounded sample
 
-N > 1 (torchrun): the path does not shard in this build:
-every rank runs an independent replica of the workload, no data-path collective; value = all
-ranks' lattice updates / max-over-ranks time ("weak").
+N > 1 (torchrun): north_star keeps the measured path on one GPU: every rank
+runs an independent replica of the workload, no data-path collective; value = all ranks' lattice
+updates / max-over-ranks time ("weak").  --slabs cuts ONE lattice into a y-slab per rank instead
+(include/lbm.h "y-slabs"; "strong").
 
 --impl reference: times the oracle (single thread, host cores) on a bounded sample of the same
 workload; the ratio against it is not a headline (it is a deliberately slow checker).

@@ -1,4 +1,4 @@
-"""Rank plumbing of the "replicas only" multi-GPU mode.
+"""Rank plumbing of the multi-GPU modes (replicas for the headline, y-slabs).
 
 The path does not shard in this build (north_star: no sharding or collectives across GPUs):
 under torchrun every rank runs an independent replica of the workload on its own GPU.  The only

@@ -423,6 +423,36 @@ def test_refilled_node_beside_a_moving_ellipse_is_extrapolated_along_the_surface
     assert checked >= 3, checked
 
 
+def test_newborn_node_carries_the_equilibrium_temperature_of_the_moving_wall(ob, wl):
+    """Eq. (17): g_alpha(x_new) = g_alpha^eq(T_w, u_w) with the wall velocity.
+    A hot disc (T_w = 0.8) moves and spins through cold fluid; on every node it uncovers the
+    pre-collision temperature populations must sum to T_w and carry the heat flux
+    sum e_alpha g_alpha = u_w T_w of that equilibrium, u_w = U + Omega x (x_new - x_c) at t+1."""
+    r, Tw = 7.3, 0.8
+    p = base_params(wl, 1, 2 * r, g=0.0, gbeta=0.0, nu=0.05)
+    parts = dict(x=np.array([30.4]), y=np.array([33.7]), diam=np.array([2 * r]),
+                 rho_ratio=np.array([1e9]), T_w=np.array([Tw]), ux=np.array([0.11]),
+                 uy=np.array([-0.07]), omega=np.array([0.01]))
+    o = ob.OracleSim.from_workload(wl.Workload("refill_T", 72, 64, p, 1, 1, particles=parts))
+    checked = 0
+    for _ in range(10):
+        before = o.fields()
+        o.step(1)
+        after = o.fields()
+        P = o.particles()
+        _, g_new = o.precollision()
+        for j, i in np.argwhere((before["flag"] == 1) & (after["flag"] == 0)):
+            uwx = P["ux"][0] - P["omega"][0] * (j - P["y"][0])
+            uwy = P["uy"][0] + P["omega"][0] * (i - P["x"][0])
+            gq = g_new[:, j, i]
+            assert gq.sum() == pytest.approx(Tw, rel=1e-13)
+            assert gq[1] - gq[3] == pytest.approx(uwx * Tw, rel=1e-11)
+            assert gq[2] - gq[4] == pytest.approx(uwy * Tw, rel=1e-11)
+            assert abs(uwx * Tw) + abs(uwy * Tw) > 0.03               # u_w = 0 would be far off
+            checked += 1
+    assert checked >= 10, checked
+
+
 def best_direction(nx_, ny_):
     """The lattice direction alpha in 1..8 maximising n . e_alpha / |e_alpha| (reading 9)."""
     best, bs = 1, -1e300

@@ -135,6 +135,36 @@ def test_collision_relaxes_stress_with_s_nu_and_matches_bgk_limit(ob, wl):
     assert mo[7] == pytest.approx(-(1 - snu) * 2e-3, abs=1e-16)
 
 
+def test_forced_collision_equals_textbook_bgk_with_guo_forcing_when_all_rates_coincide(ob, wl):
+    """Pins the whole forcing vector of Eq. (5) (reading 2; the paper defers it to its
+    references).  s_q = 8(2 - s)/(8 - s) equals s at s = 8 - sqrt(48), i.e. nu = (1/s - 1/2)/3 =
+    0.14434; every non-conserved moment then relaxes at the same rate and the MRT collision must
+    equal single-relaxation-time BGK with Guo's forcing, written out here in velocity space:
+      f+ = f - s (f - f_eq(rho, u)) + (1 - s/2) w_i [3 (e_i - u) + 9 (e_i . u) e_i] . F,
+      u = (sum e_i f_i + F/2) / rho,  F = rho (a_x, a_y + g beta (T - T0))."""
+    s = 8.0 - math.sqrt(48.0)
+    nu = (1.0 / s - 0.5) / 3.0
+    P = base_params(wl, nu=nu, gbeta=3e-3, body_ax=2e-3, body_ay=-1e-3, T0=0.2)
+    rng = np.random.default_rng(7)
+    W = np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)
+    ex = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1], dtype=float)
+    ey = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1], dtype=float)
+    for _ in range(5):
+        f = ob.feq(1.0 + 0.05 * rng.standard_normal(), 0.06 * rng.standard_normal(),
+                   0.06 * rng.standard_normal()) + 1e-3 * rng.standard_normal(9)
+        T = 0.7 + 0.1 * rng.standard_normal()
+        g = ob.geq(T, 0.0, 0.0, P["kappa"])
+        fo, _ = ob.collide_node(P, f, g)
+        rho = f.sum()
+        Fx, Fy = rho * P["body_ax"], rho * (P["body_ay"] + P["gbeta"] * (T - P["T0"]))
+        ux, uy = ((ex * f).sum() + 0.5 * Fx) / rho, ((ey * f).sum() + 0.5 * Fy) / rho
+        eu = ex * ux + ey * uy
+        feq = W * rho * (1.0 + 3.0 * eu + 4.5 * eu * eu - 1.5 * (ux * ux + uy * uy))
+        guo = W * ((3.0 * (ex - ux) + 9.0 * eu * ex) * Fx + (3.0 * (ey - uy) + 9.0 * eu * ey) * Fy)
+        expect = f - s * (f - feq) + (1.0 - 0.5 * s) * guo
+        assert np.abs(fo - expect).max() < 1e-15
+
+
 # ---------------- links ----------------
 def test_link_q_closed_forms(ob):
     assert ob.link_q(-11.0, 0.0, 1, 0.0, 0.0, 10.0) == 1.0     # SURVEY 8(c) pin (iv)
