@@ -112,6 +112,12 @@ int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const do
  * the state is then undefined), LBM_E_CUDA. */
 int lbm_step(lbm_t* h, int nsteps);
 
+/* Environment variables read by lbm_create / lbm_add_particles (defaults in brackets):
+ *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_PDL [1] (programmatic dependent launch along
+ *   the kernels of a stream), LBM_CHAIN_CTAS_PER_SM [chosen from the sizes],
+ *   LBM_DEBUG_SYNC [0] (debugging: synchronise after every direct launch, abort naming the first
+ *   kernel that fails). */
+
 /* on = 1 (default): the particle update chain of a step (integrator, flag update, refill, link
  * build for the next step) runs on the library's own high-priority stream concurrently with the
  * lattice kernel on the handle's stream, as a few persistent CTAs per SM (chosen from the lattice

@@ -223,6 +223,8 @@ struct Timed {
     }
   }
   ~Timed() {
+    // debugging aid (LBM_DEBUG_SYNC=1, with LBM_GRAPH=0): synchronise after every launch and name
+    // the first kernel that fails, instead of a sticky error at the end of the call
     static const int dbg = getenv("LBM_DEBUG_SYNC") ? atoi(getenv("LBM_DEBUG_SYNC")) : 0;
     if (dbg) {
       cudaError_t e = cudaDeviceSynchronize();
@@ -857,7 +859,7 @@ int lbm_step(lbm_t* h, int nsteps) {
   // The banded schedule needs the particle-free two-step kernel, runs in periods of four steps and
   // is worth one extra synchronisation per call only for calls of some length: the band is planned
   // once here, on the caller's stream, so that the host can size the grids -- the one-step kernel
-  // gets one CTA row per lattice row above (the planned band less a margin, in steps of 32 rows),
+  // gets one CTA row per lattice row above (the planned band less a margin, in steps of 64 rows),
   // the band kernel's grid covers (the planned band plus a margin, in steps of 16 rows); each pair
   // of values is its own graph.  The per-period plans on the device stay below the cap; a band that shrinks faster than
   // the margin is caught by the one-step kernel's row loop.
@@ -871,9 +873,7 @@ int lbm_step(lbm_t* h, int nsteps) {
     // a band of less than 2^18 nodes costs more in launches than it saves in traffic (config 0)
     if (q0 <= 0 || (h->band_on < 2 && (long long)q0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
     else {
-      const char* eh = getenv("LBM_HINT_SLACK");
-      const int hs = eh ? atoi(eh) : 96, hq = hs >= 64 ? 64 : 32;
-      h->band_hint = std::max(0, ((q0 - hs) / hq) * hq);
+      h->band_hint = std::max(0, ((q0 - 96) / 64) * 64);   // (32 / 96 / 160 rows of margin: the same step time)
       h->band_cap = std::min(h->ny, ((q0 + 8 + 15) / 16) * 16);
     }
   }
