@@ -201,6 +201,15 @@ int lbm_slab_halo_doubles(const lbm_t* h, long long* doubles);
 int lbm_slab_pack(lbm_t* h, int side, double* dev_buf);           /* side 0: lowest own rows, 1: highest */
 int lbm_slab_unpack(lbm_t* h, int side, const double* dev_buf);   /* side 0: ghost rows below, 1: above */
 int lbm_slab_exchange_halos(lbm_t** slabs, int n);                /* ascending row ranges, one process */
+/* Fused halo exchange for slabs of one process (ascending row ranges): after lbm_slab_link_peers
+ * the lattice kernel and the refill commit of lbm_slab_advance also write the rows next to a cut
+ * straight into the neighbour slab's ghost rows (peer memory: the same GPU, or another GPU of the
+ * node with peer access over NVLink) -- the exchange becomes the epilogue of the kernel that
+ * produces the data.  lbm_slab_fence (instead of lbm_slab_exchange_halos) then ends a step: all
+ * slabs' streams are synchronised, so every push has landed before the next step reads it.
+ * Every slab must be advanced once per step.  Same bits as the copy-based exchange. */
+int lbm_slab_link_peers(lbm_t** slabs, int n);
+int lbm_slab_fence(lbm_t** slabs, int n);
 int lbm_slab_combine_forces(lbm_t** slabs, int n);                /* same, one device */
 
 /* Readout.  Any pointer may be NULL = not wanted.

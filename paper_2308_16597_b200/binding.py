@@ -91,6 +91,8 @@ def load_library():
     L.lbm_slab_unpack.argtypes = [vp, C.c_int, vp]
     L.lbm_slab_exchange_halos.argtypes = [C.POINTER(vp), C.c_int]
     L.lbm_slab_combine_forces.argtypes = [C.POINTER(vp), C.c_int]
+    L.lbm_slab_link_peers.argtypes = [C.POINTER(vp), C.c_int]
+    L.lbm_slab_fence.argtypes = [C.POINTER(vp), C.c_int]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
     L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
@@ -110,7 +112,7 @@ def load_library():
                  "lbm_set_two_step", "lbm_set_graph", "lbm_set_band", "lbm_get_band", "lbm_create_slab",
                  "lbm_slab_forces", "lbm_slab_force_buffer", "lbm_slab_advance", "lbm_slab_check",
                  "lbm_slab_halo_doubles", "lbm_slab_pack", "lbm_slab_unpack", "lbm_slab_exchange_halos",
-                 "lbm_slab_combine_forces"):
+                 "lbm_slab_combine_forces", "lbm_slab_link_peers", "lbm_slab_fence"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L

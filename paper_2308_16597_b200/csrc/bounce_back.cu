@@ -290,7 +290,7 @@ k_refill(const double* __restrict__ A, double* __restrict__ stash,
 __global__ void k_refill_commit(double* __restrict__ B, const double* __restrict__ stash,
                                 unsigned char* __restrict__ flag, const int* __restrict__ nb_node,
                                 const int* __restrict__ nb_count, int* __restrict__ nb_count_next,
-                                int nb_cap, int early, const LbmConst c) {
+                                int nb_cap, int early, const HaloPush hp, const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();
   if (blockIdx.x == 0 && threadIdx.x == 0) *nb_count_next = 0;
@@ -301,9 +301,21 @@ __global__ void k_refill_commit(double* __restrict__ B, const double* __restrict
     const int e = (int)(t >> 4), k = (int)(t & 15);
     const int x = nb_node[e];
     if (x < 0) continue;
-    if (k < 9) B[f_at(k, x, c.ps)] = stash[(long long)e * 14 + k];
-    else if (k < 14) B[g_at(k - 9, x, c.ps)] = stash[(long long)e * 14 + k];
-    else if (k == 15) flag[x] = 0;
+    if (k < 14) {
+      const double v = stash[(long long)e * 14 + k];
+      if (k < 9) B[f_at(k, x, c.ps)] = v;
+      else B[g_at(k - 9, x, c.ps)] = v;
+      // y-slabs: a newborn node in a row next to a cut also goes to the neighbour's ghost row
+      const int j = x / c.px;
+      if (hp.lo && j >= hp.lo_start && j < hp.lo_end) {
+        const long long xp = x + (long long)hp.lo_shift * c.px;
+        if (k < 9) hp.lo[f_at(k, xp, hp.lo_ps)] = v; else hp.lo[g_at(k - 9, xp, hp.lo_ps)] = v;
+      }
+      if (hp.hi && j >= hp.hi_start && j < hp.hi_end) {
+        const long long xp = x + (long long)hp.hi_shift * c.px;
+        if (k < 9) hp.hi[f_at(k, xp, hp.hi_ps)] = v; else hp.hi[g_at(k - 9, xp, hp.hi_ps)] = v;
+      }
+    } else if (k == 15) flag[x] = 0;
   }
 }
 
@@ -327,12 +339,13 @@ void launch_refill(lbm* h, cudaStream_t st) {
                                         h->newborn_count + h->cur, h->newborn_cap, h->pa, h->cur ^ 1, h->C);
 }
 
-void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl) {
+void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl, const HaloPush* hp) {
   if (h->np == 0) return;
   int blocks = (h->np * 16 + 255) / 256;
   if (blocks > 1184) blocks = 1184;
   h->launches++;
   launch_k(k_refill_commit, dim3(blocks), dim3(256), 0, st, pdl, h->B, (const double*)h->stash, h->flag,
            (const int*)h->newborn_node, (const int*)(h->newborn_count + step_parity),
-           h->newborn_count + (step_parity ^ 1), h->newborn_cap, h->chain_ctas > 0 ? 0 : 1, h->C);
+           h->newborn_count + (step_parity ^ 1), h->newborn_cap, h->chain_ctas > 0 ? 0 : 1,
+           hp ? *hp : HaloPush{nullptr, 0, 0, 0, 0, nullptr, 0, 0, 0, 0}, h->C);
 }

@@ -983,6 +983,29 @@ int lbm_slab_force_buffer(lbm_t* h, double** dev_buf, int* count) {
   return LBM_OK;
 }
 
+// Where the rows next to this slab's cuts go in the neighbours' copies of the state being written.
+// All slabs of a decomposition step in lockstep and swap their A / B in every advance: a neighbour
+// that has already advanced this step holds the new state in its A, one that has not will write it
+// to its B.
+static HaloPush halo_push(const lbm* h) {
+  HaloPush hp = {nullptr, 0, 0, 0, 0, nullptr, 0, 0, 0, 0};
+  if (const lbm* p = h->peer_lo) {
+    hp.lo = p->steps_done > h->steps_done ? p->A : p->B;
+    hp.lo_ps = p->ps;
+    hp.lo_shift = h->yoff - p->yoff;            // (global row) - p->yoff = local row + this
+    hp.lo_start = h->row0;
+    hp.lo_end = h->row0 + h->halo;
+  }
+  if (const lbm* p = h->peer_hi) {
+    hp.hi = p->steps_done > h->steps_done ? p->A : p->B;
+    hp.hi_ps = p->ps;
+    hp.hi_shift = h->yoff - p->yoff;
+    hp.hi_start = h->row1 - h->halo;
+    hp.hi_end = h->row1;
+  }
+  return hp;
+}
+
 int lbm_slab_advance(lbm_t* h) {
   if (!h) return LBM_E_ARG;
   if (!h->is_slab) return fail(h, LBM_E_STATE, "lbm_slab_advance: not a slab handle");
@@ -999,10 +1022,50 @@ int lbm_slab_advance(lbm_t* h) {
     launch_build_links(h, sp ^ 1, S, false);
     h->cur ^= 1;
   }
-  launch_stream_collide(h, 0, nullptr);          // the slab's own rows only (h->row0, h->row1)
-  if (h->np > 0) launch_refill_commit(h, sp, S, false);
+  // the slab's own rows; with linked peers (lbm_slab_link_peers) the rows next to the cuts are
+  // written into the neighbours' ghost rows by the same kernel, and so are the refilled nodes
+  const HaloPush hp = halo_push(h);
+  launch_stream_collide_slab(h, hp);
+  if (h->np > 0) launch_refill_commit(h, sp, S, false, &hp);
   std::swap(h->A, h->B);
   h->steps_done++;
+  return LBM_OK;
+}
+
+// Slabs of ONE process, ascending row ranges: from now on lbm_slab_advance pushes the halo rows
+// straight into the neighbours' ghost rows (peer access is enabled between devices), and
+// lbm_slab_fence replaces lbm_slab_exchange_halos.  Every slab must be advanced in every step.
+int lbm_slab_link_peers(lbm_t** hs, int n) {
+  if (!hs || n < 1) return LBM_E_ARG;
+  for (int s = 0; s < n; ++s) {
+    if (!hs[s] || !hs[s]->is_slab) return LBM_E_ARG;
+    if (s + 1 < n && (hs[s]->own1 != hs[s + 1]->own0 || hs[s]->halo != hs[s + 1]->halo || hs[s]->px != hs[s + 1]->px))
+      return fail(hs[s], LBM_E_ARG, "lbm_slab_link_peers: slabs %d and %d do not adjoin", s, s + 1);
+  }
+  for (int s = 0; s < n; ++s) {
+    hs[s]->peer_lo = s > 0 ? hs[s - 1] : nullptr;
+    hs[s]->peer_hi = s + 1 < n ? hs[s + 1] : nullptr;
+    for (lbm* p : {hs[s]->peer_lo, hs[s]->peer_hi})
+      if (p && p->device != hs[s]->device) {
+        DeviceGuard dg(hs[s]);
+        cudaError_t e = cudaDeviceEnablePeerAccess(p->device, 0);
+        if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled)
+          return fail(hs[s], LBM_E_CUDA, "lbm_slab_link_peers: no peer access from device %d to %d", hs[s]->device, p->device);
+        cudaGetLastError();
+      }
+  }
+  return LBM_OK;
+}
+
+// end of a step with linked peers: every slab's kernels (and with them the pushes into its
+// neighbours) have completed before anyone starts the next step
+int lbm_slab_fence(lbm_t** hs, int n) {
+  if (!hs || n < 1) return LBM_E_ARG;
+  for (int s = 0; s < n; ++s) {
+    if (!hs[s]) return LBM_E_ARG;
+    DeviceGuard dg(hs[s]);
+    CUDA_OK(hs[s], cudaStreamSynchronize(hs[s]->stream));
+  }
   return LBM_OK;
 }
 

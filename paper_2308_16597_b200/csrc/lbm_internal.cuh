@@ -70,6 +70,19 @@ struct LbmConst {
   int rep_power;
 };
 
+// y-slabs: where the rows next to a cut also go -- the ghost rows of the neighbour slab's copy of
+// the state being written (peer memory of the same process).  lo: my local rows
+// [lo_start, lo_end) = the lowest `halo` own rows land in the lower neighbour at its local row
+// (j + lo_shift); hi: the highest own rows [hi_start, hi_end) in the upper neighbour.
+struct HaloPush {
+  double* lo;
+  long long lo_ps;
+  int lo_shift, lo_start, lo_end;
+  double* hi;
+  long long hi_ps;
+  int hi_shift, hi_start, hi_end;
+};
+
 struct ParticleArrays {      // SoA in the workspace, each max_particles long
   double *x[2], *y[2], *theta[2], *ux[2], *uy[2], *omega[2];   // double-buffered state
   double *r, *rho_ratio, *Tw;   // r: radius of a circle, largest semi-axis of an ellipse
@@ -96,6 +109,7 @@ struct lbm {
   // the own rows [own0, own1) (global) are updated, `halo` ghost rows on each interior side.
   // row0, row1: the own rows as LOCAL indices.  A single domain: 0, ny, 0, ny, halo 0.
   int is_slab, yoff, NY, own0, own1, halo, row0, row1;
+  lbm *peer_lo, *peer_hi;    // neighbour slabs in the same process (lbm_slab_link_peers): the halo push targets
   long long ps;
   lbm_params P;
   LbmConst C;
@@ -208,6 +222,7 @@ inline void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
 // ---- kernel launchers (each in its own translation unit) ----
 // stream_collide.cu
 void launch_stream_collide(lbm* h, int band, const double* low);   // on h->stream, h->A -> h->B
+void launch_stream_collide_slab(lbm* h, const HaloPush& hp);       // on h->stream; own rows, with the halo push
 void launch_stream_collide_2step(lbm* h);  // on h->stream; particle-free lattices only
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part);   // on h->stream; rows [0, *h->band)
@@ -231,4 +246,4 @@ void launch_add_buffer(double* dst, const double* src, int n, cudaStream_t st); 
 // bounce_back.cu
 void launch_bounce_back(lbm* h, cudaStream_t st, bool pdl);
 void launch_refill(lbm* h, cudaStream_t st); // reads A, writes the stash; called before cur is flipped
-void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl);  // stash -> B, newborn flags cleared
+void launch_refill_commit(lbm* h, int step_parity, cudaStream_t st, bool pdl, const HaloPush* hp = nullptr);  // stash -> B (and the neighbours' ghost rows), newborn flags cleared

@@ -116,17 +116,20 @@ __device__ __forceinline__ void pull_node(const double* __restrict__ A, const Lb
   }
 }
 
-// the same nine accesses as stores
-__device__ __forceinline__ void store_node(double* __restrict__ B, const LbmConst& c, int i, int j,
-                                           const double (&f)[9], const double (&g)[5]) {
-  const long long x = (long long)j * c.px + i;   // j: the row of the copy the node is stored in
-  const long long ps = c.ps;
+// the same nine accesses as stores (ps, px: plane stride and row pitch of the copy written to)
+__device__ __forceinline__ void store_node_at(double* __restrict__ B, long long ps, int px, int i, int j,
+                                              const double (&f)[9], const double (&g)[5]) {
+  const long long x = (long long)j * px + i;   // j: the row of the copy the node is stored in
   double* __restrict__ O = B + 2 * x;
 #pragma unroll
   for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * ps) = make_double2(f[k], g[k]);
   double* __restrict__ Q = B + 10 * ps + x;
 #pragma unroll
   for (int k = 0; k < 4; ++k) Q[k * ps] = f[5 + k];
+}
+__device__ __forceinline__ void store_node(double* __restrict__ B, const LbmConst& c, int i, int j,
+                                           const double (&f)[9], const double (&g)[5]) {
+  store_node_at(B, c.ps, c.px, i, j, f, g);
 }
 
 // one lattice update of node (i, j): pull, collide, store
@@ -206,6 +209,45 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
 #pragma unroll
       for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
     }
+  }
+}
+
+// y-slabs: the lattice kernel of a slab updates its own rows [row0, row1) and, fused into the same
+// pass, PUSHES the rows next to a cut into the neighbour slab's ghost rows (HaloPush: peer copies
+// in the same process -- the same GPU in the tests, another GPU over NVLink with peer access): the
+// halo exchange is the epilogue of the kernel that produces the data, not a separate copy.
+__global__ void __launch_bounds__(SC_THREADS)
+k_stream_collide_slab(const double* __restrict__ A, double* __restrict__ B,
+                      const unsigned char* __restrict__ flag, int row0, int row1, const HaloPush hp,
+                      const LbmConst c) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int i = blockIdx.x * SC_THREADS + threadIdx.x;
+  const int j = blockIdx.y + row0;
+  if (j >= row1) return;
+  const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
+  const unsigned m = __ballot_sync(0xffffffffu, fluid);
+  if (fluid) {
+    double f[9], g[5];
+    pull_node(A, c, i, j, f, g);
+    mrt_collide(f, g, c);
+    store_node(B, c, i, j, f, g);
+    if (hp.lo && j < hp.lo_end) store_node_at(hp.lo, hp.lo_ps, c.px, i, j + hp.lo_shift, f, g);
+    if (hp.hi && j >= hp.hi_start) store_node_at(hp.hi, hp.hi_ps, c.px, i, j + hp.hi_shift, f, g);
+    return;
+  }
+  const unsigned lane = threadIdx.x & 31u;
+  if (i >= c.px) return;
+  const long long x = (long long)j * c.px + i;
+  if ((m >> (lane & ~(unsigned)(SC_FILL_PAIR - 1))) & ((1u << SC_FILL_PAIR) - 1u)) {
+    double* __restrict__ O = B + 2 * x;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) *reinterpret_cast<double2*>(O + 2 * k * c.ps) = make_double2(0.0, 0.0);
+  }
+  if ((m >> (lane & ~(unsigned)(SC_FILL_DIAG - 1))) & ((1u << SC_FILL_DIAG) - 1u)) {
+    double* __restrict__ Q4 = B + 10 * c.ps + x;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) Q4[k * c.ps] = 0.0;
   }
 }
 
@@ -417,6 +459,12 @@ void launch_stream_collide(lbm* h, int band, const double* low) {
   launch_k(k_stream_collide, grid_rows(h->px, rows, SC_THREADS), dim3(SC_THREADS), 0, h->stream, h->use_pdl != 0,
            (const double*)h->A, h->B, (const unsigned char*)h->flag, band == 1 ? low : (const double*)nullptr,
            (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->row0, h->row1, h->C);
+}
+
+void launch_stream_collide_slab(lbm* h, const HaloPush& hp) {
+  h->launches++;
+  launch_k(k_stream_collide_slab, grid_rows(h->px, h->row1 - h->row0, SC_THREADS), dim3(SC_THREADS), 0, h->stream,
+           h->use_pdl != 0, (const double*)h->A, h->B, (const unsigned char*)h->flag, h->row0, h->row1, hp, h->C);
 }
 
 int stream_collide_configure() {

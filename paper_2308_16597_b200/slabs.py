@@ -63,7 +63,9 @@ def _slice_rows(T, rows):
 class SlabGroup:
     """A cavity cut into y-slabs that all live in this process."""
 
-    def __init__(self, w, n_slabs, halo=None, devices=None):
+    def __init__(self, w, n_slabs, halo=None, devices=None, fused_halo=True):
+        """fused_halo: the lattice kernel pushes the rows next to a cut into the neighbour's ghost
+        rows itself (lbm_slab_link_peers); False: copy-based lbm_slab_exchange_halos after the step."""
         from . import binding
         self.w = w
         d_max = float(np.max(w.particles["diam"])) if w.particles is not None else 0.0
@@ -82,6 +84,9 @@ class SlabGroup:
         import ctypes as C
         self._arr = (C.c_void_p * n_slabs)(*[s._h for s in self.slabs])
         self._n = n_slabs
+        self.fused_halo = bool(fused_halo)
+        if self.fused_halo:
+            self._chk(self._L.lbm_slab_link_peers(self._arr, self._n))
 
     def _chk(self, rc, who=0):
         self.slabs[who]._chk(rc)
@@ -93,7 +98,10 @@ class SlabGroup:
             self._chk(self._L.lbm_slab_combine_forces(self._arr, self._n))
             for s in self.slabs:
                 s.slab_advance()
-            self._chk(self._L.lbm_slab_exchange_halos(self._arr, self._n))
+            if self.fused_halo:
+                self._chk(self._L.lbm_slab_fence(self._arr, self._n))
+            else:
+                self._chk(self._L.lbm_slab_exchange_halos(self._arr, self._n))
         for s in self.slabs:
             s.slab_check()
 

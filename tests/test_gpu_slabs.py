@@ -37,11 +37,13 @@ def assert_group_equals_domain(grp, dom):
         assert np.array_equal(pa[k], pb[k]), k
 
 
-@pytest.mark.parametrize("n_slabs", [2, 3])
-def test_slabs_on_one_device_equal_the_single_domain_bitwise(gpu, wl, n_slabs):
+@pytest.mark.parametrize("n_slabs,fused", [(2, True), (3, True), (2, False), (3, False)])
+def test_slabs_on_one_device_equal_the_single_domain_bitwise(gpu, wl, n_slabs, fused):
     """14 particles of mixed sizes fall through the cuts of a 300 x 390 cavity (some start on a
     cut, one is thrown upwards across it): ownership changes hands, discs straddle two slabs,
-    newborn nodes appear in ghost rows."""
+    newborn nodes appear in ghost rows.  fused: the lattice kernel and the refill commit push the
+    rows next to a cut into the neighbour's ghost rows themselves (lbm_slab_link_peers); otherwise
+    the rows are copied after the step (lbm_slab_exchange_halos)."""
     from paper_2308_16597_b200 import slabs
     w = wl.sedimentation(300, 390, 14, seed=17, y_frac_lo=0.25, d_lo=12.0, d_hi=22.0, name="slabs")
     n = w.n_particles
@@ -51,7 +53,7 @@ def test_slabs_on_one_device_equal_the_single_domain_bitwise(gpu, wl, n_slabs):
     uy = np.full(n, -0.03)
     uy[k] = +0.06 if y[k] < cut else -0.08               # crosses the cut early on
     w.particles.update(ux=np.zeros(n), uy=uy, omega=1e-3 * np.ones(n))
-    grp = slabs.SlabGroup(w, n_slabs)
+    grp = slabs.SlabGroup(w, n_slabs, fused_halo=fused)
     dom = gpu.Simulation.from_workload(w)
     assert grp.halo == 19
     owners0 = slabs.owner_of(dom.particles()["y"], grp.ranges)
