@@ -210,7 +210,7 @@ int lbm_slab_exchange_halos(lbm_t** slabs, int n);                /* ascending r
  * Every slab must be advanced once per step.  Same bits as the copy-based exchange. */
 int lbm_slab_link_peers(lbm_t** slabs, int n);
 int lbm_slab_fence(lbm_t** slabs, int n);
-int lbm_slab_combine_forces(lbm_t** slabs, int n);                /* same, one device */
+int lbm_slab_combine_forces(lbm_t** slabs, int n);                /* same (peer access between devices) */
 
 /* Readout.  Any pointer may be NULL = not wanted.
  * rho, ux, uy, T: nx*ny doubles each; on fluid nodes rho = sum f, T = sum g,

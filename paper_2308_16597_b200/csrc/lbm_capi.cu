@@ -1127,15 +1127,32 @@ int lbm_slab_combine_forces(lbm_t** hs, int n) {
   const int cnt = 3 * hs[0]->np;
   if (cnt == 0) return LBM_OK;
   for (int s = 0; s < n; ++s) {
-    if (!hs[s] || !hs[s]->is_slab || hs[s]->np != hs[0]->np || hs[s]->device != hs[0]->device)
-      return LBM_E_ARG;
+    if (!hs[s] || !hs[s]->is_slab || hs[s]->np != hs[0]->np) return LBM_E_ARG;
+    DeviceGuard dg(hs[s]);
     CUDA_OK(hs[s], cudaStreamSynchronize(hs[s]->stream));
   }
+  // summed on the first slab's device, in ascending slab order; buffers on other devices are read
+  // and written through peer access
+  DeviceGuard dg(hs[0]);
   cudaStream_t S = hs[0]->stream;
-  for (int s = 1; s < n; ++s) launch_add_buffer(hs[0]->force_buf, hs[s]->force_buf, cnt, S);
-  for (int s = 1; s < n; ++s)
-    CUDA_OK(hs[0], cudaMemcpyAsync(hs[s]->force_buf, hs[0]->force_buf, cnt * sizeof(double),
-                                   cudaMemcpyDeviceToDevice, S));
+  for (int s = 1; s < n; ++s) {
+    if (hs[s]->device != hs[0]->device) {
+      cudaError_t e = cudaDeviceEnablePeerAccess(hs[s]->device, 0);
+      if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled)
+        return fail(hs[0], LBM_E_CUDA, "lbm_slab_combine_forces: no peer access from device %d to %d",
+                    hs[0]->device, hs[s]->device);
+      cudaGetLastError();
+    }
+    launch_add_buffer(hs[0]->force_buf, hs[s]->force_buf, cnt, S);
+  }
+  for (int s = 1; s < n; ++s) {
+    if (hs[s]->device != hs[0]->device)
+      CUDA_OK(hs[0], cudaMemcpyPeerAsync(hs[s]->force_buf, hs[s]->device, hs[0]->force_buf, hs[0]->device,
+                                         cnt * sizeof(double), S));
+    else
+      CUDA_OK(hs[0], cudaMemcpyAsync(hs[s]->force_buf, hs[0]->force_buf, cnt * sizeof(double),
+                                     cudaMemcpyDeviceToDevice, S));
+  }
   CUDA_OK(hs[0], cudaStreamSynchronize(S));
   return LBM_OK;
 }
