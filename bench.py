@@ -287,20 +287,23 @@ def main():
     # 14 doubles read + 14 written per fluid node + 1 flag byte per node.
     # With a two-step band the one-step kernel covers the rows from Q up (and row Q-1 in every
     # other step); the band's kernel advances Q*nx nodes by one step per launch on average
+    band_rows = band_q if band_q > 0 else (w.ny + band_q if band_q < 0 else 0)   # (< 0: a band under the lid)
     if two_step:
         alg_bytes = 2 * BYTES_PER_LU * n_fluid
-    elif band_q > 0:
-        fluid_top = int((flag[band_q:] == 0).sum()) + 0.5 * w.nx
-        alg_bytes = BYTES_PER_LU * fluid_top + FLAG_BYTES * (w.ny - band_q + 0.5) * w.nx
+    elif band_rows > 0:
+        outside = flag[band_q:] if band_q > 0 else flag[:-band_q]
+        fluid_top = int((outside == 0).sum()) + 0.5 * w.nx
+        alg_bytes = BYTES_PER_LU * fluid_top + FLAG_BYTES * (w.ny - band_rows + 0.5) * w.nx
     else:
         alg_bytes = BYTES_PER_LU * n_fluid + FLAG_BYTES * n
     band = None
-    if band_q > 0 and not two_step:
+    if band_rows > 0 and not two_step:
         b_s = ovl["stream_collide_2step"] * 1e-3
-        band = {"rows": band_q, "kernel": "k_stream_collide_2step", "launches_per_step": 1,
-                "lattice_updates_per_launch": band_q * w.nx, "avg_launch_ms": b_s * 1e3,
+        band = {"rows": band_rows, "where": "below the suspension" if band_q > 0 else "above the suspension",
+                "kernel": "k_stream_collide_2step", "launches_per_step": 1,
+                "lattice_updates_per_launch": band_rows * w.nx, "avg_launch_ms": b_s * 1e3,
                 "avg_launch_ms_alone": seq["stream_collide_2step"],
-                "algorithmic_gbs_at_224_B_per_update": BYTES_PER_LU * band_q * w.nx / b_s / 1e9 if b_s > 0 else None}
+                "algorithmic_gbs_at_224_B_per_update": BYTES_PER_LU * band_rows * w.nx / b_s / 1e9 if b_s > 0 else None}
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"

@@ -156,7 +156,10 @@ int lbm_set_two_step(lbm_t* h, int on);
  * arithmetic per node and step is unchanged: results are identical bit for bit to on = 0.
  * on = 1 uses a band only if it holds at least 2^18 nodes (below that its extra launches cost more
  * than the traffic it saves); on = 2 uses every band of at least 28 rows (the tests).
- * lbm_get_band: *rows = Q of the last banded period completed by lbm_step (0: none). */
+ * A settled bed leaves the rows under the lid free instead: the plan at the start of a call picks
+ * the larger of the two bands (rows [0, Q) under the lowest particle, rows [Q, ny) above the
+ * highest) and the call keeps that orientation.
+ * lbm_get_band: *rows = Q of the last plan (0: none; > 0: the band is [0, Q); < 0: [-Q, ny)). */
 int lbm_set_band(lbm_t* h, int on);
 int lbm_get_band(lbm_t* h, int* rows);
 

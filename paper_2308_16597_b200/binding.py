@@ -240,7 +240,8 @@ class Simulation:
         self._chk(self._L.lbm_set_band(self._h, int(on)))
 
     def band_rows(self):
-        """Rows [0, Q) the last banded period advanced two steps per pass (0: none)."""
+        """Q of the last band plan: > 0: rows [0, Q) advance two steps per pass; < 0: rows [-Q, ny)
+        (a band above the suspension); 0: none."""
         q = C.c_int(0)
         self._chk(self._L.lbm_get_band(self._h, C.byref(q)))
         return q.value

@@ -779,7 +779,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
     lbm::StepGraph& g = h->graphs[k];
     if (g.A == h->A && g.cur == h->cur && g.steps == steps && g.overlap == h->overlap &&
         g.chain_ctas == h->chain_ctas && g.banded == banded &&
-        (!banded || (g.band_hint == h->band_hint && g.band_cap == h->band_cap)))
+        (!banded || (g.band_hint == h->band_hint && g.band_cap == h->band_cap && g.band_orient == h->band_orient)))
       return &g;
   }
   if (h->n_graphs == LBM_MAX_GRAPHS) drop_graphs(h);
@@ -841,6 +841,7 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   g.banded = banded;
   g.band_hint = h->band_hint;
   g.band_cap = h->band_cap;
+  g.band_orient = h->band_orient;
   g.launches = per;
   return &g;
 }
@@ -866,15 +867,19 @@ int lbm_step(lbm_t* h, int nsteps) {
   bool band_ok = h->np > 0 && h->band_on && h->two_step_ok && nsteps >= LBM_BAND_MIN_STEPS;
   if (band_ok) {
     h->band_cap = h->ny;
+    h->band_orient = 0;                // under or above the suspension: whichever band is larger
     launch_band_plan(h, h->stream);
     CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaStreamSynchronize(h->stream));
-    const int q0 = h->status_host[1];
+    const int q0 = h->status_host[1];                         // > 0: rows [0, q0); < 0: rows [-q0, ny)
+    const int rows0 = q0 > 0 ? q0 : (q0 < 0 ? h->ny + q0 : 0);  // rows of the band
     // a band of less than 2^18 nodes costs more in launches than it saves in traffic (config 0)
-    if (q0 <= 0 || (h->band_on < 2 && (long long)q0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
+    if (rows0 <= 0 || (h->band_on < 2 && (long long)rows0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
     else {
-      h->band_hint = std::max(0, ((q0 - 96) / 64) * 64);   // (32 / 96 / 160 rows of margin: the same step time)
-      h->band_cap = std::min(h->ny, ((q0 + 8 + 15) / 16) * 16);
+      h->band_orient = q0 > 0 ? 1 : -1;                       // fixed for this call: the grids are sized for it
+      h->band_hint = std::max(0, ((rows0 - 96) / 64) * 64);   // (32 / 96 / 160 rows of margin: the same step time)
+      h->band_l1_rows = h->ny - h->band_hint;                 // the rows outside the band, with that margin
+      h->band_cap = std::min(h->ny, ((rows0 + 8 + 15) / 16) * 16);
     }
   }
   // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
@@ -928,7 +933,7 @@ int lbm_set_band(lbm_t* h, int on) {
 
 int lbm_get_band(lbm_t* h, int* rows) {
   if (!h || !rows) return LBM_E_ARG;
-  *rows = (h->np > 0 && h->band_on && h->two_step_ok) ? h->status_host[1] : 0;
+  *rows = (h->np > 0 && h->band_on && h->two_step_ok) ? h->status_host[1] : 0;   // signed, see lbm.h
   return LBM_OK;
 }
 

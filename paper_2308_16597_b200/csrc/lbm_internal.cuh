@@ -149,7 +149,9 @@ struct lbm {
   // [0, Q) are advanced two steps per pass; band[1] = 0 (what the plain schedule's kernels read)
   int* band;
   double* force_buf;         // y-slabs: 3 * max_particles doubles (Fx, Fy, Tz), the slab's share of the force combine
-  int band_hint;             // rows certainly inside the band as the host last saw it (sizes the one-step grid; 0 = unknown)
+  int band_hint;             // rows certainly inside the band as the host last saw it (part of the graph key)
+  int band_l1_rows;          // CTA rows of the one-step kernel in banded steps (the rows outside that, + a margin)
+  int band_orient;           // 0: the call-start plan chooses; +1 band under the suspension, -1 above it
   int band_live;             // the step being enqueued belongs to a banded period (k_cover checks the margin)
   int band_cap;              // most rows the band may have in this call (sizes the band kernel's grid)
   int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
@@ -172,7 +174,7 @@ struct lbm {
   struct StepGraph {
     cudaGraphExec_t exec;
     const double* A;         // phase the graph was captured in
-    int cur, steps, overlap, chain_ctas, banded, band_hint, band_cap;
+    int cur, steps, overlap, chain_ctas, banded, band_hint, band_cap, band_orient;
     long long launches;      // kernels per replay
   } graphs[LBM_MAX_GRAPHS];
   int n_graphs;

@@ -674,7 +674,7 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
         int early, const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();
-  const int Q = *bandp;
+  const int Q = *bandp;   // > 0: band [0, Q); < 0: band [-Q, ny)
   for (int p = blockIdx.x; p < np; p += gridDim.x) {   // grid-size agnostic
   const Shape Sn = load_shape<ELL>(pa, buf, p);
   const double xn = Sn.x, yn = Sn.y;
@@ -682,6 +682,7 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
     // safety net of the two-step band: no solid node within 4 rows of it (k_band_plan's margins
     // make this unreachable for any |U|, dU the method is stable at)
     if (Q > 0 && (int)floor(yn - Sn.r) < Q + 4) atomicOr(status, ST_BAND_REACHED);
+    if (Q < 0 && (int)ceil(yn + Sn.r) > -Q - 5) atomicOr(status, ST_BAND_REACHED);
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
     ci = min(max(ci, 0), ncx - 1);
     cj = min(max(cj, 0), ncy - 1);
@@ -719,26 +720,47 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
 // A band of fewer than BAND_MIN rows is not worth its seam: Q = 0 (no band).  One CTA.
 constexpr int BAND_PERIOD = 8;
 constexpr int BAND_MIN = 28;
+// orient: +1 only a band under the suspension (rows [0, Q), band[0] = Q), -1 only a band above
+// it (rows [Q, ny), band[0] = -Q: a settled bed leaves the rows under the lid free), 0 whichever is
+// larger (the plan at the start of a call; the orientation then stays fixed for the call, because
+// the grids are sized for it).  qcap: most rows the band may have (the band kernel's grid).
 __global__ void __launch_bounds__(1024)
-k_band_plan(ParticleArrays pa, int cur, int np, int ny, int qcap, int* __restrict__ band) {
-  __shared__ double s_min[32];
-  double low = 1.0e300;
+k_band_plan(ParticleArrays pa, int cur, int np, int ny, int orient, int qcap, int* __restrict__ band) {
+  __shared__ double s_min[32], s_max[32];
+  double low = 1.0e300, high = -1.0e300;
   for (int p = threadIdx.x; p < np; p += blockDim.x) {
-    const double fall = pa.fixed[p] ? 0.0 : fmax(-pa.uy[cur][p], 0.0);
-    low = fmin(low, pa.y[cur][p] - pa.r[p] - (double)BAND_PERIOD * fall);
+    const double uy = pa.fixed[p] ? 0.0 : pa.uy[cur][p];
+    low = fmin(low, pa.y[cur][p] - pa.r[p] - (double)BAND_PERIOD * fmax(-uy, 0.0));
+    high = fmax(high, pa.y[cur][p] + pa.r[p] + (double)BAND_PERIOD * fmax(uy, 0.0));
   }
 #pragma unroll
-  for (int d = 16; d >= 1; d >>= 1) low = fmin(low, __shfl_xor_sync(0xffffffffu, low, d));
-  if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = low;
+  for (int d = 16; d >= 1; d >>= 1) {
+    low = fmin(low, __shfl_xor_sync(0xffffffffu, low, d));
+    high = fmax(high, __shfl_xor_sync(0xffffffffu, high, d));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    s_min[threadIdx.x >> 5] = low;
+    s_max[threadIdx.x >> 5] = high;
+  }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) low = fmin(low, s_min[w]);
-    int Q = 0;
-    if (low == low && low < 1.0e9 && low > -1.0e9) Q = (int)floor(low) - 7;
-    if (Q > ny - 8) Q = ny - 8;
-    if (Q > qcap) Q = qcap;        // the band kernel's grid was sized for at most this many rows
-    if (Q < BAND_MIN) Q = 0;
-    band[0] = Q;
+    for (int w = 1; w < (int)(blockDim.x >> 5); ++w) {
+      low = fmin(low, s_min[w]);
+      high = fmax(high, s_max[w]);
+    }
+    int below = 0, above = 0;   // rows of the two candidate bands
+    int Qb = 0, Qt = ny;
+    if (low == low && low < 1.0e9 && low > -1.0e9) {
+      Qb = min((int)floor(low) - 7, ny - 8);
+      below = Qb >= BAND_MIN ? min(Qb, qcap) : 0;
+    }
+    if (high == high && high < 1.0e9 && high > -1.0e9) {
+      Qt = max((int)ceil(high) + 7, 8);
+      above = ny - Qt >= BAND_MIN ? min(ny - Qt, qcap) : 0;
+    }
+    if (orient > 0) above = 0;
+    if (orient < 0) below = 0;
+    band[0] = (below == 0 && above == 0) ? 0 : (below >= above ? below : -(ny - above));
   }
 }
 
@@ -862,7 +884,7 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
 // buffer h->cur); a plain launch: it starts after everything before it in `st` has completed
 void launch_band_plan(lbm* h, cudaStream_t st) {
   h->launches++;
-  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_cap, h->band);
+  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_orient, h->band_cap, h->band);
 }
 
 void launch_slab_forces_out(lbm* h) {

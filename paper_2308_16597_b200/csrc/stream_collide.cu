@@ -37,14 +37,16 @@ struct RowsPlain {
   __device__ __forceinline__ long long row0(int sj) const { return (long long)sj * px; }
 };
 struct RowsSeam {
-  const double* top;   // rows >= Q
-  const double* low;   // rows < Q
+  const double* top;   // rows outside the band
+  const double* low;   // rows of the band: [0, Q), or [Q, ny) for a band under the lid (upper)
   int Q;
-  int low_row;         // >= 0: every row < Q is stored as this row of `low` (the spare row)
+  int low_row;         // >= 0: every band row is stored as this row of `low` (the spare row)
   int px;
-  __device__ __forceinline__ const double* base(int sj) const { return sj < Q ? low : top; }
+  bool upper;
+  __device__ __forceinline__ bool inband(int sj) const { return upper ? sj >= Q : sj < Q; }
+  __device__ __forceinline__ const double* base(int sj) const { return inband(sj) ? low : top; }
   __device__ __forceinline__ long long row0(int sj) const {
-    return (long long)((sj < Q && low_row >= 0) ? low_row : sj) * px;
+    return (long long)((inband(sj) && low_row >= 0) ? low_row : sj) * px;
   }
 };
 
@@ -172,21 +174,31 @@ k_stream_collide(const double* __restrict__ A, double* __restrict__ B,
   // come up as this grid's last wave drains; every kernel waits here for its predecessor's data
   pdl_launch_dependents();
   pdl_wait();
-  const int Q = *bandp;
+  // band[0] > 0: rows [0, Q) are the band; < 0: rows [Q, ny) with Q = -band[0] (a band under the
+  // lid, above a settled bed: the same scheme mirrored -- this kernel then covers the rows BELOW
+  // Q, and in the first step of a pair also row Q, into the spare row); 0: none
+  const int Qs = *bandp;
+  const bool upper = Qs < 0;
+  const int Q = upper ? -Qs : Qs;
   const int i = blockIdx.x * SC_THREADS + threadIdx.x;
+  int jfirst = row0, jend = row1;
+  if (Q > 0) {
+    if (upper) jend = min(row1, Q - delta);
+    else jfirst = max(row0, Q + delta);
+  }
   // The grid has one CTA row per lattice row the host EXPECTS this launch to cover (it knows the
   // band height of the previous lbm_step call); the loop takes care of a band that has shrunk
   // since (normally it runs once).
   // [row0, row1): the rows this launch may update at all (the whole lattice; a y-slab: its own rows)
-  for (int j = blockIdx.y + max(row0, Q > 0 ? Q + delta : 0); j < row1; j += gridDim.y) {
+  for (int j = blockIdx.y + jfirst; j < jend; j += gridDim.y) {
     const bool fluid = i < c.nx && flag[(long long)j * c.px + i] == 0;
-    if (j <= Q && Q > 0) {                       // the two rows along the seam (all fluid)
+    if (Q > 0 && (upper ? j >= Q - 1 : j <= Q)) {   // the two rows along the seam (all fluid)
       if (fluid) {
         double f[9], g[5];
-        const RowsSeam R{A, Alow ? Alow : A, Q, Alow ? -1 : c.ny, c.px};
+        const RowsSeam R{A, Alow ? Alow : A, Q, Alow ? -1 : c.ny, c.px, upper};
         pull_boundary(R, c, i, j, f, g);
         mrt_collide(f, g, c);
-        store_node(B, c, i, j < Q ? c.ny : j, f, g);
+        store_node(B, c, i, R.inband(j) ? c.ny : j, f, g);
       }
       continue;
     }
@@ -278,23 +290,27 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
   extern __shared__ double s_pop[];   // [14][TB_H][TB_W]
   pdl_launch_dependents();
   pdl_wait();
-  const int Q = bandp ? min(*bandp, c.ny) : c.ny;
+  const int Qs = bandp ? *bandp : c.ny;
+  const bool upper = Qs < 0;                       // the band is [Q, ny) instead of [0, Q)
+  const int Q = upper ? -Qs : min(Qs, c.ny);
   // part p owns the p-th contiguous share of the band's tile rows (neighbouring tile rows of one
   // launch share their halo rows through L2)
-  const int per_part = ((Q + TB_Y - 1) / TB_Y + nparts - 1) / nparts;
+  const int tr0 = upper ? Q / TB_Y : 0;            // first tile row that holds band rows
+  const int ntr = (upper ? (c.ny + TB_Y - 1) / TB_Y : (Q + TB_Y - 1) / TB_Y) - tr0;
+  const int per_part = (ntr + nparts - 1) / nparts;
   if ((int)blockIdx.y >= per_part) return;
-  const int tile_j0 = (part * per_part + blockIdx.y) * TB_Y;
-  if (tile_j0 >= Q) return;
+  const int tile_j0 = (tr0 + part * per_part + blockIdx.y) * TB_Y;
+  if (upper ? tile_j0 >= c.ny : tile_j0 >= Q) return;
   const int tx = threadIdx.x % TB_W, ty = threadIdx.x / TB_W;
   const int i = blockIdx.x * TB_X - 1 + tx, j = tile_j0 - 1 + ty;
   // phase 1: node (i, j) of the halo'd tile, wrapped in x when periodic
   int iw = i;
   if (c.periodic_x) iw = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i);
-  const bool exists = iw >= 0 && iw < c.nx && j >= 0 && j < c.ny && j <= Q;
+  const bool exists = iw >= 0 && iw < c.nx && j >= 0 && j < c.ny && (upper ? j >= Q - 1 : j <= Q);
   double f[9], g[5];
   if (exists) {
-    if (j + 1 < Q || Q == c.ny) pull_node(Aband, c, iw, j, f, g);
-    else pull_boundary(RowsSeam{Atop, Aband, Q, -1, c.px}, c, iw, j, f, g);   // rows Q-1, Q (warp-uniform)
+    if (upper ? j - 1 >= Q : (j + 1 < Q || Q == c.ny)) pull_node(Aband, c, iw, j, f, g);
+    else pull_boundary(RowsSeam{Atop, Aband, Q, -1, c.px, upper}, c, iw, j, f, g);   // rows Q-1, Q (warp-uniform)
     mrt_collide(f, g, c);
 #pragma unroll
     for (int k = 0; k < 9; ++k) s_pop[k * TB_THREADS + threadIdx.x] = f[k];
@@ -303,7 +319,7 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
   }
   __syncthreads();
   // phase 2: the tile's own nodes
-  if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= Q) return;
+  if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= c.ny || (upper ? j < Q : j >= Q)) return;
   if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
     // interior: every upstream neighbour is a node of the tile's halo'd image
     const double* __restrict__ S = s_pop + threadIdx.x;
@@ -455,7 +471,7 @@ void launch_stream_collide(lbm* h, int band, const double* low) {
   h->launches++;
   // banded steps: one CTA row per lattice row above the band as the host last saw it
   // (h->band_hint, 0 = unknown); the kernel's row loop covers whatever the band has lost since
-  const int rows = band ? h->ny - h->band_hint : h->row1 - h->row0;
+  const int rows = band ? h->band_l1_rows : h->row1 - h->row0;
   launch_k(k_stream_collide, grid_rows(h->px, rows, SC_THREADS), dim3(SC_THREADS), 0, h->stream, h->use_pdl != 0,
            (const double*)h->A, h->B, (const unsigned char*)h->flag, band == 1 ? low : (const double*)nullptr,
            (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->row0, h->row1, h->C);
@@ -486,7 +502,8 @@ void launch_stream_collide_band(lbm* h, const double* src_band, const double* sr
   h->launches++;
   // CTAs of this kernel are expensive to launch even when they exit at once (512 threads, 57 KB):
   // the grid covers the band as the host last saw it plus a margin (k_band_plan keeps Q below it)
-  const int tile_rows = (std::min(h->band_cap, h->ny) + TB_Y - 1) / TB_Y;
+  // h->band_cap: the most rows the band may have in this call (k_band_plan clamps to it)
+  const int tile_rows = (std::min(h->band_cap, h->ny) + TB_Y - 1) / TB_Y + 1;
   const dim3 grid((h->nx + TB_X - 1) / TB_X, (tile_rows + nparts - 1) / nparts);
   launch_k(k_stream_collide_2step, grid, dim3(TB_THREADS), TB_SMEM, h->stream, h->use_pdl != 0, src_band, src_top,
            dst_band, (const int*)h->band, nparts, part, h->C);

@@ -545,12 +545,14 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
     assert live == sorted(live, reverse=True) and len(set(live)) > 2   # ... that shrinks
     # a particle that starts just above the smallest band worth having and falls: the band is
     # given up (Q = 0) within a few periods and the plain schedule carries on
+    # (a second, fixed disc under the lid keeps the rows above free of a band of their own)
     p = wl.default_params()
-    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=1,
+    p.update(g=1.6e-4, gbeta=1e-5, wall_T_type=[1, 1, 1, 1], max_particles=2,
              max_links_per_particle=wl.max_links_for_diameter(14.0))
-    parts = dict(x=np.array([60.4]), y=np.array([47.0]), diam=np.array([14.0]),
-                 rho_ratio=np.array([1.5]), T_w=np.array([1.0]), ux=np.array([0.0]),
-                 uy=np.array([-0.05]), omega=np.array([0.0]))
+    parts = dict(x=np.array([60.4, 30.0]), y=np.array([47.0, 139.0]), diam=np.array([14.0, 14.0]),
+                 rho_ratio=np.array([1.5, 1.5]), T_w=np.array([1.0, 0.0]), ux=np.array([0.0, 0.0]),
+                 uy=np.array([-0.05, 0.0]), omega=np.array([0.0, 0.0]),
+                 fixed=np.array([0, 1], dtype=np.uint8))
     w2 = wl.Workload("band_vanishes", 120, 150, p, 1, 1, particles=parts)
     a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
     a.set_band(2)
@@ -562,6 +564,64 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
         assert_same_bits(a, b)
         qs.append(a.band_rows())
     assert qs[0] >= 28 and qs[-1] == 0, qs
+
+
+def test_two_step_band_above_a_settled_suspension_equals_plain_schedule_bitwise(gpu, ob, wl):
+    """The mirrored band: particles low in the cavity leave the rows under the lid free; the plan
+    at the start of a call picks the larger band (here the upper one: band_rows() < 0).  Bitwise
+    equality with the plain schedule (graphs / direct launches / one stream) while one particle is
+    thrown upwards into the free rows (the band shrinks from the other side), a heated lid and a
+    periodic case against the oracle."""
+    w = wl.sedimentation(300, 400, 14, seed=8, y_frac_lo=0.0, d_lo=12.0, d_hi=20.0, name="band_up")
+    n = w.n_particles
+    w.particles["y"] = 0.45 * w.particles["y"] + 8.0          # squeeze into the lower half (x unchanged: no overlap)
+    w.particles["y"] = np.maximum(w.particles["y"], 0.5 * w.particles["diam"] + 3.0)
+    # re-space vertically so that no two discs overlap after the squeeze
+    order = np.argsort(w.particles["y"])
+    ys = w.particles["y"].copy()
+    uy = np.zeros(n)
+    k = int(np.argmax(ys))
+    uy[k] = +0.10                                             # thrown upwards into the free rows
+    keep = []
+    for a in range(n):                                        # drop discs that would overlap another one
+        ok = all(np.hypot(w.particles["x"][a] - w.particles["x"][b], ys[a] - ys[b])
+                 >= 0.5 * (w.particles["diam"][a] + w.particles["diam"][b]) + 2.0 for b in keep)
+        if ok:
+            keep.append(a)
+    keep = np.array(keep)
+    assert len(keep) >= 6 and k in keep
+    parts = {key: np.asarray(v)[keep] for key, v in w.particles.items()}
+    parts["y"] = ys[keep]
+    parts.update(ux=np.zeros(len(keep)), uy=uy[keep], omega=np.zeros(len(keep)))
+    w.params["max_particles"] = len(keep)
+    w = wl.Workload("band_up", w.nx, w.ny, w.params, 1, 1, particles=parts)
+    ref = gpu.Simulation.from_workload(w)
+    ref.set_band(False)
+    ref.set_graph(False)
+    sims = [gpu.Simulation.from_workload(w) for _ in range(3)]
+    for s_ in sims:
+        s_.set_band(2)
+    sims[1].set_graph(False)
+    sims[2].set_overlap(False)
+    q_seen = []
+    for nst in (16, 29, 64, 402, 7, 900):
+        ref.step(nst)
+        for s_ in sims:
+            s_.step(nst)
+            assert_same_bits(s_, ref)
+        q_seen.append(sims[0].band_rows())
+    assert all(q < 0 for q in q_seen) and 400 + min(q_seen) > 120, q_seen   # a band under the lid: rows [-Q, ny)
+    assert len(set(q_seen)) > 1                               # ... that the thrown particle pushes back
+    # against the oracle, with a heated lid and periodic sides
+    p = wl.default_params()
+    p.update(g=1.6e-4, gbeta=1e-5, body_ax=1e-6, periodic_x=1, wall_T_type=[0, 0, 1, 1],
+             wall_T=[0.0, 0.0, 0.1, 0.8], max_particles=2,
+             max_links_per_particle=wl.max_links_for_diameter(16.0))
+    parts = dict(x=np.array([40.3, 77.0]), y=np.array([30.2, 41.0]), diam=np.array([16.0, 12.5]),
+                 rho_ratio=np.array([1.5, 1.3]), T_w=np.array([1.0, 0.4]))
+    w2 = wl.Workload("band_up_walls", 131, 181, p, 60, 60, particles=parts)
+    g, o, _ = run_and_compare(gpu, ob, w2, [60], r_min=6.0)
+    assert g.band_rows() < 0 and 181 + g.band_rows() > 100     # rows [55, 181) or so
 
 
 def test_two_step_band_periodic_and_wall_types(gpu, ob, wl):
