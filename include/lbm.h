@@ -226,6 +226,22 @@ int lbm_slab_combine_forces(lbm_t** slabs, int n);                /* same (peer 
 int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T,
                    double* f, double* g, unsigned char* flag);
 
+/* The macroscopic read-out for callers that cannot allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc) and want the workspace left untouched:
+ * the same kernel as lbm_get_fields, but its dense outputs are staged in a file-scope
+ * `static __device__` array of the library instead of the dead copy of the populations, then
+ * copied to the caller's HOST buffers (each nx*ny doubles; any may be NULL).  Calls no cudaMalloc,
+ * cudaFree or allocating library routine.
+ * Limit: nx*ny <= LBM_STATIC_MAX_NODES (2^20 nodes: 4 fields x 8 MiB = 32 MiB of device memory,
+ * held by every GPU that loads the library until the process exits); larger lattices (and slab
+ * handles) are rejected with LBM_E_CAPACITY resp. LBM_E_STATE and a text in lbm_last_error.
+ * Every call on a device shares that array, which keeps the last call's contents (every node of
+ * the requested outputs is rewritten, so nothing stale is ever returned); calls that overlap on
+ * the GPU -- two handles on different streams -- race on it: serialise them.
+ * Results are bit-identical to lbm_get_fields(h, rho, ux, uy, T, NULL, NULL, NULL). */
+#define LBM_STATIC_MAX_NODES (1 << 20)
+int lbm_get_macroscopic_static(lbm_t* h, double* rho, double* ux, double* uy, double* T);
+
 /* Particle state (r, U, theta, Omega_z; F, T_z of the last completed step).
  * *n receives the particle count; arrays (each may be NULL) need that many entries. */
 int lbm_get_particles(lbm_t* h, int* n, double* x, double* y, double* theta,

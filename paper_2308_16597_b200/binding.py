@@ -94,6 +94,7 @@ def load_library():
     L.lbm_slab_link_peers.argtypes = [C.POINTER(vp), C.c_int]
     L.lbm_slab_fence.argtypes = [C.POINTER(vp), C.c_int]
     L.lbm_get_fields.argtypes = [vp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
+    L.lbm_get_macroscopic_static.argtypes = [vp, _dp, _dp, _dp, _dp]
     L.lbm_get_particles.argtypes = [vp, _ip] + [_dp] * 9
     L.lbm_get_links.argtypes = [vp, C.POINTER(ll), _ip, _ip, _ip, _ip, _dp]
     L.lbm_profile_enable.argtypes = [vp, C.c_int]
@@ -112,7 +113,8 @@ def load_library():
                  "lbm_set_two_step", "lbm_set_graph", "lbm_set_band", "lbm_get_band", "lbm_create_slab",
                  "lbm_slab_forces", "lbm_slab_force_buffer", "lbm_slab_advance", "lbm_slab_check",
                  "lbm_slab_halo_doubles", "lbm_slab_pack", "lbm_slab_unpack", "lbm_slab_exchange_halos",
-                 "lbm_slab_combine_forces", "lbm_slab_link_peers", "lbm_slab_fence"):
+                 "lbm_slab_combine_forces", "lbm_slab_link_peers", "lbm_slab_fence",
+                 "lbm_get_macroscopic_static"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -299,6 +301,14 @@ class Simulation:
             res["f"] = f.reshape(9, self.ny, self.nx)
             res["g"] = g.reshape(5, self.ny, self.nx)
         return res
+
+    def macroscopic_static(self):
+        """rho, ux, uy, T through lbm_get_macroscopic_static (no allocation on the device, workspace
+        untouched; lattices of at most 2^20 nodes)."""
+        out = {k: np.empty(self.n, dtype=np.float64) for k in ("rho", "ux", "uy", "T")}
+        self._chk(self._L.lbm_get_macroscopic_static(self._h, _d(out["rho"]), _d(out["ux"]),
+                                                     _d(out["uy"]), _d(out["T"])))
+        return {k: v.reshape(self.ny, self.nx) for k, v in out.items()}
 
     def particles(self):
         n = C.c_int()

@@ -1232,6 +1232,25 @@ int lbm_get_fields(lbm_t* h, double* rho, double* ux, double* uy, double* T, dou
   return LBM_OK;
 }
 
+int lbm_get_macroscopic_static(lbm_t* h, double* rho, double* ux, double* uy, double* T) {
+  if (!h) return LBM_E_ARG;
+  if (h->is_slab) return fail(h, LBM_E_STATE, "lbm_get_macroscopic_static: not for slab handles");
+  DeviceGuard dg(h);
+  double* s[4] = {nullptr, nullptr, nullptr, nullptr};
+  const int rc = launch_macroscopic_static(h, s);
+  if (rc == -1)
+    return fail(h, LBM_E_CAPACITY, "lbm_get_macroscopic_static: %d x %d nodes exceed the static scratch array (LBM_STATIC_MAX_NODES = %d)",
+                h->nx, h->ny, (int)LBM_STATIC_MAX_NODES);
+  if (rc != 0) return fail(h, LBM_E_CUDA, "lbm_get_macroscopic_static: cudaGetSymbolAddress failed");
+  const size_t bytes = (size_t)h->nx * h->ny * sizeof(double);
+  double* out[4] = {rho, ux, uy, T};
+  for (int k = 0; k < 4; ++k)
+    if (out[k]) CUDA_OK(h, cudaMemcpyAsync(out[k], s[k], bytes, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_OK(h, cudaStreamSynchronize(h->stream));
+  CUDA_OK(h, cudaGetLastError());
+  return LBM_OK;
+}
+
 int lbm_get_particles(lbm_t* h, int* n, double* x, double* y, double* theta, double* ux,
                       double* uy, double* omega, double* Fx, double* Fy, double* Tz) {
   if (!h || !n) return h ? fail(h, LBM_E_ARG, "get_particles: n is NULL") : LBM_E_ARG;

@@ -234,6 +234,7 @@ void launch_set_temperature(lbm* h, const double* T_dev_dense);
 void launch_set_equilibrium(lbm* h);
 void launch_export(lbm* h, double* f_dense, double* g_dense);    // dense f[9][n], g[5][n], device
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T);  // dense nx*ny, device
+int launch_macroscopic_static(lbm* h, double** fields4);   // into the library's static scratch array; 0 / -1 too large / -2
 // particles.cu (compiled with -fmad=false)
 // `pdl`: launch with the programmatic-serialisation attribute (the kernel then waits for its
 // predecessor in `st` itself, see pdl_wait)

@@ -530,6 +530,42 @@ void launch_export(lbm* h, double* f_dense, double* g_dense) {
                                                                 f_dense, g_dense, h->C);
 }
 
+// ---- read-out that allocates nothing and touches none of the caller's workspace ----
+// lbm_get_fields stages its dense outputs in the dead copy B of the workspace.  For callers that
+// must not allocate and want the workspace left alone (include/lbm.h lbm_get_macroscopic_static)
+// the same kernel writes into this file-scope array instead: 4 fields x LBM_STATIC_MAX_NODES
+// doubles = 32 MiB, held by every GPU that loads the library until the process exits.  Every call
+// shares it and it keeps the last call's contents; k_macroscopic writes every node of the
+// nx x ny outputs it is asked for, so nothing has to start at zero.  Calls that overlap on the
+// GPU (two handles on different streams) race on it.
+static __device__ __align__(256) double g_static_fields[4 * (size_t)LBM_STATIC_MAX_NODES];
+
+// The array's name is a host-side stand-in here, not a device address: the address is looked up
+// once per device, with that device current (the caller's DeviceGuard), and handed to the kernel.
+// 0 = ok, -1 = lattice too large, -2 = cudaGetSymbolAddress failed.
+int launch_macroscopic_static(lbm* h, double** fields4) {
+  static double* addr[64] = {nullptr};
+  if ((long long)h->nx * h->ny > (long long)LBM_STATIC_MAX_NODES) return -1;
+  const int dev = (h->device >= 0 && h->device < 64) ? h->device : 0;
+  if (!addr[dev]) {
+    double* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_static_fields) != cudaSuccess || !p) {
+      cudaGetLastError();
+      return -2;
+    }
+    addr[dev] = p;
+  }
+  double* base = addr[dev];
+  const size_t n = (size_t)LBM_STATIC_MAX_NODES;
+  const int c = h->cur;
+  h->launches++;
+  k_macroscopic<<<grid_rows(h->nx, h->ny, 128), 128, 0, h->stream>>>(
+      h->A, h->flag, h->owner, h->pa.x[c], h->pa.y[c], h->pa.ux[c], h->pa.uy[c], h->pa.omega[c],
+      h->pa.Tw, h->primed, base, base + n, base + 2 * n, base + 3 * n, h->C);
+  for (int k = 0; k < 4; ++k) fields4[k] = base + k * n;
+  return 0;
+}
+
 void launch_macroscopic(lbm* h, double* rho, double* ux, double* uy, double* T) {
   const int c = h->cur;
   h->launches++;
