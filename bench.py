@@ -279,8 +279,11 @@ def main():
     # a particle-free lattice advances two steps per launch (k_stream_collide_2step): the launch
     # then carries two lattice updates per node (2 x 224 B algorithmic) while moving ~137 B per
     # update, so its fraction of the 224 B/LU roofline may exceed 1
-    two_step = ovl.get("stream_collide_2step", 0.0) > 0.0 and ovl.get("stream_collide", 0.0) == 0.0
-    kname = "stream_collide_2step" if two_step else "stream_collide"
+    # (three per launch with k_stream_collide_3step: 3 x 224 B algorithmic, ~105 B per update moved)
+    three_step = ovl.get("stream_collide_3step", 0.0) > 0.0 and w.particles is None
+    two_step = three_step or (ovl.get("stream_collide_2step", 0.0) > 0.0 and ovl.get("stream_collide", 0.0) == 0.0)
+    kname = "stream_collide_3step" if three_step else ("stream_collide_2step" if two_step else "stream_collide")
+    per_launch = 3 if three_step else (2 if two_step else 1)
     far_s = seq[kname] * 1e-3
     far_ovl_s = ovl[kname] * 1e-3
     step_ms_seq = sum(seq.values())
@@ -289,7 +292,7 @@ def main():
     # other step); the band's kernel advances Q*nx nodes by one step per launch on average
     band_rows = band_q if band_q > 0 else (w.ny + band_q if band_q < 0 else 0)   # (< 0: a band under the lid)
     if two_step:
-        alg_bytes = 2 * BYTES_PER_LU * n_fluid
+        alg_bytes = per_launch * BYTES_PER_LU * n_fluid
     elif band_rows > 0:
         outside = flag[band_q:] if band_q > 0 else flag[:-band_q]
         fluid_top = int((outside == 0).sum()) + 0.5 * w.nx
@@ -312,7 +315,7 @@ def main():
     # `achieved` is taken in the schedule the timed region runs (the particle chain sharing the
     # GPU with the lattice kernel); the kernel alone on the GPU is reported beside it
     achieved = alg_bytes / far_ovl_s / 1e9 if far_ovl_s > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_" + kname, "lattice_updates_per_launch": 2 if two_step else 1,
+    roofline = {"bound": "hbm", "kernel": "k_" + kname, "lattice_updates_per_launch": per_launch,
                 "achieved": achieved,
                 "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": read_traffic() if args.config == 3 else None,

@@ -139,10 +139,15 @@ int lbm_set_overlap(lbm_t* h, int on);
  * direct launches. */
 int lbm_set_graph(lbm_t* h, int on);
 
-/* on = 1 (default): while no particle has been added, lbm_step advances the lattice two time steps
- * per pass over the populations (shared-memory tile with a one-node halo; about 137 B instead of
- * 224 B of HBM traffic per lattice update), an odd last step through the one-step kernel.  The
- * arithmetic per step is the same, so results are identical bit for bit to on = 0. */
+/* Particle-free lattices (no particle added): time steps per pass over the populations.
+ * on = 0: one (the fused one-step kernel, 224 B of HBM traffic per lattice update);
+ * on = 1 or 2: two (shared-memory tile of 30 x 14 nodes with a one-node halo, about 137 B requested
+ *   and 111 B of DRAM traffic per update);
+ * on = 3 (default; the environment variable LBM_STEPS_PER_PASS = 1 / 2 / 3 sets the default): three
+ *   (tile of 28 x 12 nodes with a two-node halo, the intermediate levels written back in place in
+ *   shared memory; about 105 B requested per update), the last one or two steps of a call through
+ *   the two-step and one-step kernels.
+ * The arithmetic per node and step is the same in all three, so results are identical bit for bit. */
 int lbm_set_two_step(lbm_t* h, int on);
 
 /* on = 1 (default; the environment variable LBM_BAND = 0 / 1 / 2 sets the default): lattices WITH particles also use the

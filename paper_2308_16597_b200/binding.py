@@ -249,7 +249,9 @@ class Simulation:
         return q.value
 
     def set_two_step(self, on=True):
-        self._chk(self._L.lbm_set_two_step(self._h, 1 if on else 0))
+        """Particle-free lattices: time steps per pass over the populations.  False / 0: one;
+        True / 1 / 2: two; 3: three (lbm_set_two_step)."""
+        self._chk(self._L.lbm_set_two_step(self._h, int(on)))
 
     # ---- y-slabs: the two halves of a step and the exchanges' end points (slabs.py drives them) ----
     def slab_forces(self):

@@ -21,7 +21,8 @@ char g_create_error[512] = "";
 
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "integrate_uncover",
-    "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step", "band_plan"};
+    "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step", "band_plan",
+    "stream_collide_3step"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -343,7 +344,11 @@ static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, 
   fill_const(h);
   cudaGetDevice(&h->device);
   h->two_step_ok = stream_collide_configure() == 0 ? 1 : 0;
-  h->two_step = h->two_step_ok;
+  h->two_step = h->two_step_ok ? 2 : 0;   // 0: one step per pass, 1: two, 2: three (then two, then one)
+  if (h->two_step_ok) {
+    const char* e3 = getenv("LBM_STEPS_PER_PASS");
+    if (e3) h->two_step = atoi(e3) >= 3 ? 2 : (atoi(e3) == 2 ? 1 : 0);
+  }
   if (particles_configure(h) != 0) {
     delete h;
     return fail(nullptr, LBM_E_CUDA, "lbm_create: max_links_per_particle needs more shared memory than the device has");
@@ -902,6 +907,14 @@ int lbm_step(lbm_t* h, int nsteps) {
   const bool direct = s < nsteps;
   int direct_periods = 0;   // a band plan serves two periods
   while (s < nsteps) {
+    if (h->np == 0 && h->two_step >= 2 && nsteps - s >= 3) {
+      // particle-free lattice: three time steps per pass
+      { Timed tm(h, K_STREAM_COLLIDE_3STEP, h->stream); launch_stream_collide_3step(h); }
+      std::swap(h->A, h->B);
+      h->steps_done += 3;
+      s += 3;
+      continue;
+    }
     if (h->np == 0 && h->two_step && nsteps - s >= 2) {
       // particle-free lattice: two time steps per pass over the populations (A -> B)
       { Timed tm(h, K_STREAM_COLLIDE_2STEP, h->stream); launch_stream_collide_2step(h); }
@@ -1170,7 +1183,7 @@ int lbm_set_graph(lbm_t* h, int on) {
 
 int lbm_set_two_step(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
-  h->two_step = (on && h->two_step_ok) ? 1 : 0;
+  h->two_step = (on && h->two_step_ok) ? (on >= 3 ? 2 : 1) : 0;   // on: steps per pass (1 = 2: two)
   return LBM_OK;
 }
 

@@ -32,7 +32,7 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_MOVE, K_COVER, K_REFILL,
-  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_BAND_PLAN, K_COUNT
+  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_BAND_PLAN, K_STREAM_COLLIDE_3STEP, K_COUNT
 };
 
 // link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along
@@ -226,6 +226,7 @@ inline void launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sme
 void launch_stream_collide(lbm* h, int band, const double* low);   // on h->stream, h->A -> h->B
 void launch_stream_collide_slab(lbm* h, const HaloPush& hp);       // on h->stream; own rows, with the halo push
 void launch_stream_collide_2step(lbm* h);  // on h->stream; particle-free lattices only
+void launch_stream_collide_3step(lbm* h);  // on h->stream; particle-free lattices only
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part);   // on h->stream; rows [0, *h->band)
 int stream_collide_configure();            // kernel attributes (0 = ok)

@@ -74,7 +74,9 @@ def test_two_steps_per_pass_equals_one_step_per_pass_bitwise(gpu, wl):
     """Particle-free lattices advance two time steps per pass (shared-memory tile).
     Same arithmetic per step, so every population must equal the one-step kernel's bit for bit:
     ragged sizes (tiles of 32 x 14 with partial tiles in both directions), every wall type, a
-    body force, and the periodic wrap; odd step counts leave one step to the one-step kernel."""
+    body force, and the periodic wrap; odd step counts leave one step to the one-step kernel.
+    The same for THREE steps per pass (tiles of 28 x 12 with a two-node halo, levels written back
+    in place), including lattices narrower than one tile and the periodic images two columns out."""
     rng = np.random.default_rng(17)
     cases = []
     p = wl.default_params()
@@ -86,18 +88,26 @@ def test_two_steps_per_pass_equals_one_step_per_pass_bitwise(gpu, wl):
     q.update(periodic_x=1, body_ax=1e-6, nu=0.1, gbeta=1e-4, wall_T_type=[0, 0, 1, 1], wall_T=[0, 0, 1.0, 0.0])
     cases.append((77, 45, q))                            # periodic, nx not a multiple of 32
     cases.append((33, 15, dict(q)))
+    cases.append((5, 9, dict(q)))                        # narrower than the halo is wide
+    cases.append((29, 13, dict(p)))
     for nx, ny, prm in cases:
         T = 0.25 + 0.5 * rng.uniform(-1, 1, size=(ny, nx))
         w = wl.Workload("two_step", nx, ny, prm, 1, 1, T_init=T)
-        a = gpu.Simulation.from_workload(w)
+        a = gpu.Simulation.from_workload(w)          # the library's default
+        a2 = gpu.Simulation.from_workload(w)
+        a2.set_two_step(2)                           # two steps per pass
+        a3 = gpu.Simulation.from_workload(w)
+        a3.set_two_step(3)                           # three steps per pass (then two, then one)
         b = gpu.Simulation.from_workload(w)
         b.set_two_step(False)
-        for n in (1, 2, 7, 40):
-            a.step(n)
+        for n in (1, 2, 3, 5, 7, 40):
             b.step(n)
-            fa, fb = a.fields(populations=True), b.fields(populations=True)
-            for k in ("f", "g", "rho", "ux", "uy", "T"):
-                assert np.array_equal(fa[k], fb[k]), (nx, ny, n, k)
+            fb = b.fields(populations=True)
+            for s_ in (a, a2, a3):
+                s_.step(n)
+                fa = s_.fields(populations=True)
+                for k in ("f", "g", "rho", "ux", "uy", "T"):
+                    assert np.array_equal(fa[k], fb[k]), (nx, ny, n, k)
 
 
 def test_periodic_poiseuille(gpu, ob, wl):
