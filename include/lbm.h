@@ -113,7 +113,7 @@ int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const do
 int lbm_step(lbm_t* h, int nsteps);
 
 /* Environment variables read by lbm_create / lbm_add_particles (defaults in brackets):
- *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_PDL [1] (programmatic dependent launch along
+ *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_PDL [1] (programmatic dependent launch along
  *   the kernels of a stream), LBM_CHAIN_CTAS_PER_SM [chosen from the sizes],
  *   LBM_DEBUG_SYNC [0] (debugging: synchronise after every direct launch, abort naming the first
  *   kernel that fails). */

@@ -1373,6 +1373,9 @@ long long lbm_kernel_launches(const lbm_t* h) { return h ? h->launches : -1; }
 int lbm_destroy(lbm_t* h) {
   if (!h) return LBM_OK;
   DeviceGuard dg(h);
+  // a linked neighbour slab must not push into (or read the step counter of) a handle that is gone
+  if (h->peer_lo && h->peer_lo->peer_hi == h) h->peer_lo->peer_hi = nullptr;
+  if (h->peer_hi && h->peer_hi->peer_lo == h) h->peer_hi->peer_lo = nullptr;
   cudaStreamSynchronize(h->stream);
   drop_graphs(h);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
