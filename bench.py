@@ -242,6 +242,9 @@ def main():
     # to its idle clocks (120 MHz), and the ramp back up then lands inside the timed steps
     # (measured: one run in four 15-55 us per step slower)
     sim.step(W)
+    # one-time plan building outside the timed region (lbm_prepare: band plan, capture, instantiation
+    # and upload of the CUDA graphs the timed call replays; no time step is taken)
+    sim.prepare(K)
     barrier()
     l0 = sim.kernel_launches()
     t0 = time.perf_counter()
@@ -398,7 +401,9 @@ def main():
                            "l2": f"inputs larger than L2: {2 * 14 * 8 * n / 1e6:.0f} MB of "
                                  "populations stream through per step (126 MB L2)"
                                  if 2 * 14 * 8 * n > 126e6 * 2 else "working set fits L2: not an HBM-bound configuration",
-                           "seed": "numpy default_rng(config index)"},
+                           "seed": "numpy default_rng(config index)",
+                           "timed_region": "one lbm_step(K) call after lbm_step(W) and lbm_prepare(K) "
+                                           "(graphs captured and uploaded beforehand)"},
                 "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu,
                 "context": {"paper_single_gpu_mlups": 1750, "paper_hardware": "1x A100, OpenACC "

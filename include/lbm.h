@@ -112,6 +112,15 @@ int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const do
  * the state is then undefined), LBM_E_CUDA. */
 int lbm_step(lbm_t* h, int nsteps);
 
+/* Optional set-up call: does everything a following lbm_step(h, nsteps) would do before its first
+ * time step -- collides the initial state, builds the first links, plans the two-step band and
+ * captures, instantiates and uploads the CUDA graphs that call will replay -- without advancing
+ * time, so that a short timed lbm_step (tens of steps) does not pay for graph instantiation (about
+ * a millisecond per graph; like building an FFT plan before the loop).  The graphs are keyed by
+ * the state's phase and the band plan, both unchanged by this call.  After it the set-up calls
+ * (lbm_set_temperature, lbm_add_particles) return LBM_E_STATE, as after lbm_step. */
+int lbm_prepare(lbm_t* h, int nsteps);
+
 /* Environment variables read by lbm_create / lbm_add_particles (defaults in brackets):
  *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_PDL [1] (programmatic dependent launch along
  *   the kernels of a stream), LBM_CHAIN_CTAS_PER_SM [chosen from the sizes],

@@ -74,6 +74,7 @@ def load_library():
     L.lbm_add_particles.argtypes = [vp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_add_ellipses.argtypes = [vp, C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _bp]
     L.lbm_step.argtypes = [vp, C.c_int]
+    L.lbm_prepare.argtypes = [vp, C.c_int]
     L.lbm_set_overlap.argtypes = [vp, C.c_int]
     L.lbm_set_two_step.argtypes = [vp, C.c_int]
     L.lbm_set_graph.argtypes = [vp, C.c_int]
@@ -114,7 +115,7 @@ def load_library():
                  "lbm_slab_forces", "lbm_slab_force_buffer", "lbm_slab_advance", "lbm_slab_check",
                  "lbm_slab_halo_doubles", "lbm_slab_pack", "lbm_slab_unpack", "lbm_slab_exchange_halos",
                  "lbm_slab_combine_forces", "lbm_slab_link_peers", "lbm_slab_fence",
-                 "lbm_get_macroscopic_static"):
+                 "lbm_get_macroscopic_static", "lbm_prepare"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -230,6 +231,10 @@ class Simulation:
     # ---- the hot path ----
     def step(self, nsteps=1):
         self._chk(self._L.lbm_step(self._h, int(nsteps)))
+
+    def prepare(self, nsteps):
+        """lbm_prepare: plans, captures and uploads what step(nsteps) will replay, without stepping."""
+        self._chk(self._L.lbm_prepare(self._h, int(nsteps)))
 
     def set_overlap(self, on=True):
         self._chk(self._L.lbm_set_overlap(self._h, 1 if on else 0))

@@ -851,24 +851,14 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   return &g;
 }
 
-int lbm_step(lbm_t* h, int nsteps) {
-  if (!h) return LBM_E_ARG;
-  if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
-  if (h->is_slab && nsteps > 0)
-    return fail(h, LBM_E_STATE, "lbm_step on a slab: use lbm_slab_forces / lbm_slab_advance and the exchanges between them");
-  DeviceGuard dg(h);
-  if (nsteps > 0) {
-    prime(h);
-    ensure_links(h);
-  }
-  int s = 0;
-  // The banded schedule needs the particle-free two-step kernel, runs in periods of four steps and
-  // is worth one extra synchronisation per call only for calls of some length: the band is planned
-  // once here, on the caller's stream, so that the host can size the grids -- the one-step kernel
-  // gets one CTA row per lattice row above (the planned band less a margin, in steps of 64 rows),
-  // the band kernel's grid covers (the planned band plus a margin, in steps of 16 rows); each pair
-  // of values is its own graph.  The per-period plans on the device stay below the cap; a band that shrinks faster than
-  // the margin is caught by the one-step kernel's row loop.
+// The banded schedule needs the particle-free two-step kernel, runs in periods of four steps and
+// is worth one extra synchronisation per call only for calls of some length: the band is planned
+// once at the start of a call, on the caller's stream, so that the host can size the grids -- the
+// one-step kernel gets one CTA row per lattice row above (the planned band less a margin, in steps
+// of 64 rows), the band kernel's grid covers (the planned band plus a margin, in steps of 16 rows);
+// each pair of values is its own graph.  The per-period plans on the device stay below the cap; a
+// band that shrinks faster than the margin is caught by the one-step kernel's row loop.
+static int plan_call(lbm* h, int nsteps, bool* band_ok_out) {
   bool band_ok = h->np > 0 && h->band_on && h->two_step_ok && nsteps >= LBM_BAND_MIN_STEPS;
   if (band_ok) {
     h->band_cap = h->ny;
@@ -887,14 +877,64 @@ int lbm_step(lbm_t* h, int nsteps) {
       h->band_cap = std::min(h->ny, ((rows0 + 8 + 15) / 16) * 16);
     }
   }
+  *band_ok_out = band_ok;
+  return LBM_OK;
+}
+
+// how many steps the next graph launch of a call with `left` steps to go covers, and in which schedule
+static int graph_unit(int left, bool band_ok, int* banded) {
+  *banded = (band_ok && left >= 4) ? 1 : 0;
+  return left >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : (*banded ? 4 : 2);
+}
+
+int lbm_prepare(lbm_t* h, int nsteps) {
+  if (!h) return LBM_E_ARG;
+  if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_prepare: negative step count");
+  if (h->is_slab) return fail(h, LBM_E_STATE, "lbm_prepare: not for slab handles");
+  DeviceGuard dg(h);
+  if (nsteps == 0) return LBM_OK;
+  prime(h);
+  ensure_links(h);
+  bool band_ok = false;
+  int rc = plan_call(h, nsteps, &band_ok);
+  if (rc) return rc;
+  if (h->np > 0 && h->use_graph && !h->prof_on) {
+    // every unit of a call is an even number of steps, so all of them start in the current phase
+    for (int s = 0; nsteps - s >= 2;) {
+      int banded = 0;
+      const int unit = graph_unit(nsteps - s, band_ok, &banded);
+      lbm::StepGraph* g = step_graph(h, unit, banded);
+      if (!g) break;
+      cudaGraphUpload(g->exec, h->stream);
+      s += unit;
+    }
+  }
+  return check_status(h);
+}
+
+int lbm_step(lbm_t* h, int nsteps) {
+  if (!h) return LBM_E_ARG;
+  if (nsteps < 0) return fail(h, LBM_E_ARG, "lbm_step: negative step count");
+  if (h->is_slab && nsteps > 0)
+    return fail(h, LBM_E_STATE, "lbm_step on a slab: use lbm_slab_forces / lbm_slab_advance and the exchanges between them");
+  DeviceGuard dg(h);
+  if (nsteps > 0) {
+    prime(h);
+    ensure_links(h);
+  }
+  int s = 0;
+  bool band_ok = false;
+  {
+    const int rc = plan_call(h, nsteps, &band_ok);
+    if (rc) return rc;
+  }
   // lattices with particles: whole periods of the schedule as CUDA graph replays (8 steps per
   // launch while that many remain, then 4 if banded, then 2), the odd last step directly; event
   // profiling needs the direct launches
   if (h->np > 0 && h->use_graph && !h->prof_on) {
     while (nsteps - s >= 2) {
-      const int left = nsteps - s;
-      const int banded = (band_ok && left >= 4) ? 1 : 0;
-      const int unit = left >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : (banded ? 4 : 2);
+      int banded = 0;
+      const int unit = graph_unit(nsteps - s, band_ok, &banded);
       lbm::StepGraph* g = step_graph(h, unit, banded);
       if (!g) break;
       CUDA_OK(h, cudaGraphLaunch(g->exec, h->stream));

@@ -675,6 +675,32 @@ def test_results_do_not_depend_on_what_the_workspace_held_before(gpu, wl, monkey
     assert sims[0].band_rows() > 50
 
 
+def test_prepare_builds_the_graphs_without_stepping(gpu, wl):
+    """lbm_prepare(n) plans the band and captures the graphs lbm_step(n) replays, takes no time
+    step, and changes no result; set-up calls are closed afterwards."""
+    w = wl.sedimentation(300, 260, 14, seed=9, y_frac_lo=0.2, d_lo=12.0, d_hi=24.0, name="prep")
+    a, b = gpu.Simulation.from_workload(w), gpu.Simulation.from_workload(w)
+    p0 = a.particles()
+    a.prepare(20)
+    p1 = a.particles()
+    for k in ("x", "y", "ux", "uy", "omega", "theta"):
+        assert np.array_equal(p0[k], p1[k]), k
+    with pytest.raises(gpu.LbmError) as e:
+        a.set_temperature(np.zeros((w.ny, w.nx)))
+    assert e.value.code == gpu.LBM_E_STATE
+    for n in (20, 5, 20, 33):
+        a.prepare(n)
+        l0 = a.kernel_launches()
+        a.step(n)
+        b.step(n)
+        assert a.kernel_launches() - l0 > 0
+        assert_same_bits(a, b)
+    a.prepare(0)
+    c = gpu.Simulation.from_workload(wl.config(1))       # particle-free: nothing to capture
+    c.prepare(12)
+    c.step(12)
+
+
 def dense_pack(wl, n_side=10, d=12.0, gap=1.95, big=True):
     """A hexagonal pack of d = 12 discs at surface gap 1.95 (every disc has six neighbours just
     inside the repulsion range s = 2) next to one d = 30 disc, which makes the repulsion cells 32
