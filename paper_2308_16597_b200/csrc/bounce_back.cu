@@ -178,7 +178,7 @@ k_bounce_back(double* __restrict__ A, LinkArrays la, ParticleArrays pa, int cur,
 // of t+1, so it runs in the particle chain UNDER the lattice kernel, whose zero fill of non-fluid
 // lanes may still touch the node's slots in B; k_refill_commit copies the record into B after it.
 constexpr int RW = 8;   // warps (newborn nodes) per CTA
-__global__ void __launch_bounds__(RW * 32)
+__global__ void __launch_bounds__(RW * 32, 4)
 k_refill(const double* __restrict__ A, double* __restrict__ stash,
          const unsigned char* __restrict__ flag, int* __restrict__ nb_node,
          const int* __restrict__ nb_pid, const int* __restrict__ nb_count, int nb_cap,

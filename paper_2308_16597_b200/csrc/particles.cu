@@ -614,7 +614,7 @@ __device__ __forceinline__ void for_zone(int i0, int i1, int j0, int j1, const L
 // new positions) and appends to the newborn counter of this step (zeroed by the previous step's
 // k_refill_commit).
 template <bool ELL>
-__global__ void __launch_bounds__(PT_MAX)
+__global__ void __launch_bounds__(PT_MAX, 12)
 k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
        const int* __restrict__ cell_count_cur, const int* __restrict__ cell_items_cur,
        int* __restrict__ cell_count_nxt, int ncells,
@@ -667,7 +667,7 @@ k_move(ParticleArrays pa, int cur, int np, double cell, int ncx, int ncy,
 // Thread 0 also enters the particle into the repulsion grid of the step that will use this
 // position (the grid of buffer `buf`; k_move has zeroed its counts).
 template <bool ELL>
-__global__ void __launch_bounds__(PT_MAX)
+__global__ void __launch_bounds__(PT_MAX, 12)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
         int* __restrict__ cell_items, int* __restrict__ status, const int* __restrict__ bandp,
