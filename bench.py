@@ -352,17 +352,35 @@ def main():
         h2d = T_host.numel() * 8
         if w.particles is not None:
             h2d += sum(int(np.asarray(v).nbytes) for v in w.particles.values())
-        barrier()
-        te0 = time.perf_counter()
+        # one untimed rehearsal of the job (3 steps): every kernel of the set-up and read-out path is
+        # loaded, the allocator and the pinned buffers have been used once
         s2 = binding.Simulation(w.nx, w.ny, w.params, device=dev)
         s2.set_temperature(T_host)
         if w.particles is not None:
             s2.add_particles(**w.particles)
+        s2.step(3)
+        s2.fields(out=outs)
+        s2.particles()
+        s2.close()
+        del s2
+        barrier()
+        te0 = time.perf_counter()
+        s2 = binding.Simulation(w.nx, w.ny, w.params, device=dev)
+        tb = [time.perf_counter()]
+        s2.set_temperature(T_host)
+        tb.append(time.perf_counter())
+        if w.particles is not None:
+            s2.add_particles(**w.particles)
+        tb.append(time.perf_counter())
         s2.step(K)
+        tb.append(time.perf_counter())
         res = s2.fields(out=outs)
         pr = s2.particles()
         barrier()
-        te = time.perf_counter() - te0
+        tb.append(time.perf_counter())
+        te = tb[-1] - te0
+        stages = dict(zip(("create", "set_temperature", "add_particles", "step", "read_out"),
+                          (round(1e3 * (b - a), 3) for a, b in zip([te0] + tb[:-1], tb))))
         d2h = 4 * n * 8 + n + sum(int(v.nbytes) for v in pr.values())
         te_max = replicas.max_over_ranks(te, dev)
         assert np.isfinite(res["rho"]).all()
@@ -370,7 +388,7 @@ def main():
                "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                "job": "create + set_temperature(host) + add_particles(host) + step(K) + "
                       "get_fields(rho,ux,uy,T,flag -> pinned host) + get_particles",
-               "job_seconds": te_max}
+               "job_seconds": te_max, "job_stages_ms": stages}
         s2.close()
 
     # ---------------- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)

@@ -22,6 +22,7 @@
 #define MIN_CELL 16.0        // smallest repulsion-grid cell edge (workspace is sized for it)
 #define NEWBORN_PER_PARTICLE 32
 #define LBM_MAX_GRAPHS 8
+#define LBM_TMA_MIN_NODES (1LL << 20)   // three-step passes go through the persistent TMA-fed kernel from this size up
 
 // status bits written by kernels, read once per lbm_step call
 #define ST_NONFINITE 1
@@ -162,6 +163,12 @@ struct lbm {
   long long launches;        // kernels launched (lbm_kernel_launches)
   int device;                // the device the handle was created on (every entry point selects it)
   int two_step_ok;           // the two-step kernel's attributes could be set
+  // k_stream_collide_3step_tma: tensor maps of the two copies ([2*copy] pair planes, [2*copy+1]
+  // diagonal planes; opaque CUtensorMap bytes), the copies' base pointers, and whether they exist
+  unsigned long long tmaps[4][16];
+  const double* tma_base[2];
+  int tma_ok;
+  int use_tma;               // lbm_set_tma / LBM_TMA: three-step passes go through the TMA-fed kernel
   // CUDA graphs: a period of the schedule -- an even number of steps,
   // after which A/B and the particle buffer index are back where they started -- is captured once
   // per (phase, length, schedule) and replayed; the fork/join onto the chain stream is part of
@@ -227,6 +234,8 @@ void launch_stream_collide(lbm* h, int band, const double* low);   // on h->stre
 void launch_stream_collide_slab(lbm* h, const HaloPush& hp);       // on h->stream; own rows, with the halo push
 void launch_stream_collide_2step(lbm* h);  // on h->stream; particle-free lattices only
 void launch_stream_collide_3step(lbm* h);  // on h->stream; particle-free lattices only
+int stream_collide_tma_setup(lbm* h);      // tensor maps for the TMA-fed three-step kernel (0 = ok, sets h->tma_ok)
+void launch_stream_collide_3step_tma(lbm* h);  // on h->stream; particle-free closed cavities, needs h->tma_ok
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part);   // on h->stream; rows [0, *h->band)
 int stream_collide_configure();            // kernel attributes (0 = ok)

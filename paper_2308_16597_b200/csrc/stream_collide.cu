@@ -13,6 +13,9 @@
 // f_k(x,t+1) = f+_kbar(x,t); thermal g_k(x,t+1) = -g+_kbar(x,t) + 2 w_k T_wall (Dirichlet) or
 // g+_kbar(x,t) (adiabatic)  (DESIGN.md readings; the paper only says "no-slip").
 #include <algorithm>
+#include <cstring>
+
+#include <cuda.h>   // CUtensorMap and the encoder's signature; the entry point is looked up at run time
 
 #include "collide.cuh"
 
@@ -447,6 +450,184 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
   store_node(B, c, i, j, f, g);
 }
 
+// THREE time steps per pass, TMA-fed and persistent (the multi-step kernel IS a
+// tile-movement kernel).  One CTA per SM for the whole launch; it walks the tiles b, b + G, b + 2G,
+// ... (G = gridDim.x, x fastest: the ~148 tiles in flight are neighbours in a tile row, so their
+// overlapping halos meet in L2).  A tile's input -- the state at t on the T3_X x T3_Y tile plus a
+// three-node halo, as a TP_IW x TP_IH node image of all 14 populations in the HBM layout (pair
+// planes interleaved) -- is fetched by TWO 3-D tensor copies (cp.async.bulk.tensor: box 72 x 18 x 5
+// doubles of the pair planes, 36 x 18 x 4 of the diagonal planes; four extra columns on the left
+// keep the box 16-byte aligned) into a ring of TP_STAGES images that signal an mbarrier each;
+// rows and columns outside the lattice are zero-filled by the copy engine and never used (walls as
+// in pull_boundary, the node's own slot standing in).  No thread computes a global load address.
+//
+// The 1024 threads are two groups of 512 (named barriers), each of which takes every other tile of
+// the CTA's sequence and runs the three levels of k_stream_collide_3step on its image IN PLACE:
+// pull from the neighbours' slots, barrier, collide, write back to the own slot, barrier -- level 1
+// on the 32 x 16 nodes of the tile dilated by two, level 2 on 30 x 14, level 3 on 28 x 12 and from
+// registers to B.  When a group has pulled level 3 its image is free: the group's warp 0 collects
+// the other warps' arrivals (bar.arrive / bar.sync) and one lane issues the copies for the CTA's
+// tile after next but one into it, which land while both groups compute -- the loads of tile m + 3
+// overlap the arithmetic of tiles m + 1 and m + 2 instead of alternating with it.
+// Same pull, same collision, same order: bit-identical to three passes of the one-step kernel.
+constexpr int TP_IW = T3_W + 4, TP_IH = T3_H + 2;       // 36 x 18 node image
+constexpr int TP_PLANE = TP_IW * TP_IH;
+constexpr int TP_PAIR_DOUBLES = 5 * 2 * TP_PLANE;       // pair planes: (f_k, g_k) interleaved
+constexpr int TP_IMG_DOUBLES = 14 * TP_PLANE;
+constexpr int TP_IMG_BYTES = TP_IMG_DOUBLES * (int)sizeof(double);   // 72,576 = 567 x 128
+constexpr int TP_STAGES = 3, TP_GROUPS = 2;
+constexpr int TP_THREADS = TP_GROUPS * T3_THREADS;
+constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 128;   // + the mbarriers
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+  const unsigned a = smem_u32(bar);
+  unsigned ok;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, void* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+               ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void group_sync(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(T3_THREADS) : "memory"); }
+__device__ __forceinline__ void group_arrive(int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(T3_THREADS) : "memory"); }
+
+// f_k, g_k of the node in slot s of an image (lattice column i, row j) pulled from its neighbours'
+// slots; cavity walls as in pull_boundary (closed cavity only: the kernel is not used with periodic x)
+__device__ __forceinline__ void pull_img(const double* img, int s, int i, int j, const LbmConst& c,
+                                         double (&f)[9], double (&g)[5]) {
+  if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
+    const double2* __restrict__ P = reinterpret_cast<const double2*>(img) + s;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      const double2 v = P[k * TP_PLANE - ey_of(k) * TP_IW - ex_of(k)];
+      f[k] = v.x;
+      g[k] = v.y;
+    }
+    const double* __restrict__ D = img + TP_PAIR_DOUBLES + s;
+#pragma unroll
+    for (int k = 5; k < 9; ++k) f[k] = D[(k - 5) * TP_PLANE - ey_of(k) * TP_IW - ex_of(k)];
+    return;
+  }
+#pragma unroll
+  for (int k = 0; k < 9; ++k) {
+    const int si = i - ex_of(k), sj = j - ey_of(k);
+    const bool in = sj >= 0 && sj < c.ny && si >= 0 && si < c.nx;
+    const int kk = in ? k : opp_of(k);
+    const int ss = in ? s - ey_of(k) * TP_IW - ex_of(k) : s;
+    f[k] = kk <= 4 ? img[2 * (kk * TP_PLANE + ss)] : img[TP_PAIR_DOUBLES + (kk - 5) * TP_PLANE + ss];
+  }
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const int si = i - ex_of(k), sj = j - ey_of(k);
+    bool in = (sj >= 0 && sj < c.ny);
+    int wall = sj < 0 ? 2 : 3;
+    if (si < 0 || si >= c.nx) { in = false; wall = si < 0 ? 0 : 1; }
+    if (in) g[k] = img[2 * (k * TP_PLANE + s - ey_of(k) * TP_IW - ex_of(k)) + 1];
+    else {
+      const double gb = img[2 * (opp_of(k) * TP_PLANE + s) + 1];
+      g[k] = c.wall_type[wall] == 1 ? (2.0 * c.wT * c.wall_T[wall] - gb) : gb;
+    }
+  }
+}
+__device__ __forceinline__ void put_img(double* img, int s, const double (&f)[9], const double (&g)[5]) {
+  double2* __restrict__ P = reinterpret_cast<double2*>(img) + s;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) P[k * TP_PLANE] = make_double2(f[k], g[k]);
+  double* __restrict__ D = img + TP_PAIR_DOUBLES + s;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) D[k * TP_PLANE] = f[5 + k];
+}
+
+__global__ void __launch_bounds__(TP_THREADS, 1)
+k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __grid_constant__ CUtensorMap tm_diag,
+                           double* __restrict__ B, int ntx, int ntiles, const LbmConst c) {
+  extern __shared__ __align__(128) unsigned char s_raw[];
+  double* const imgs = reinterpret_cast<double*>(s_raw);
+  unsigned long long* const full = reinterpret_cast<unsigned long long*>(s_raw + TP_STAGES * TP_IMG_BYTES);
+  pdl_launch_dependents();
+  const int grp = threadIdx.x / T3_THREADS, tid = threadIdx.x % T3_THREADS;
+  const int tx = tid % T3_W, ty = tid / T3_W;
+  const int s = (ty + 1) * TP_IW + tx + 2;               // the thread's slot in every image
+  // tile m of this CTA's sequence -> stage m % TP_STAGES; one thread arms the stage's mbarrier with
+  // the byte count and issues the two box copies
+  auto fetch = [&](int m) {
+    const int tile = blockIdx.x + m * gridDim.x;
+    if (tile >= ntiles) return;
+    const int st = m % TP_STAGES;
+    const int i0 = (tile % ntx) * T3_X - 4, j0 = (tile / ntx) * T3_Y - 3;
+    double* img = imgs + st * TP_IMG_DOUBLES;
+    mbar_expect_tx(full + st, TP_IMG_BYTES);
+    tma_load_3d(img, &tm_pair, 2 * i0, j0, 0, full + st);
+    tma_load_3d(img + TP_PAIR_DOUBLES, &tm_diag, i0, j0, 0, full + st);
+  };
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int st = 0; st < TP_STAGES; ++st) mbar_init(full + st, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_wait();                                            // the previous pass has written A
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int m = 0; m < TP_STAGES; ++m) fetch(m);
+  }
+  for (int m = grp;; m += TP_GROUPS) {
+    const int tile = blockIdx.x + m * gridDim.x;
+    if (tile >= ntiles) break;
+    const int st = m % TP_STAGES;
+    double* img = imgs + st * TP_IMG_DOUBLES;
+    const int i = (tile % ntx) * T3_X - 2 + tx, j = (tile / ntx) * T3_Y - 2 + ty;
+    const bool ex1 = i >= 0 && i < c.nx && j >= 0 && j < c.ny;
+    const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2;
+    const bool ex3 = ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3;
+    double f[9], g[5];
+    mbar_wait(full + st, (unsigned)(m / TP_STAGES) & 1u);
+    // level 1: t -> t+1
+    if (ex1) pull_img(img, s, i, j, c, f, g);
+    group_sync(1 + grp);
+    if (ex1) {
+      mrt_collide(f, g, c);
+      put_img(img, s, f, g);
+    }
+    group_sync(1 + grp);
+    // level 2: t+1 -> t+2
+    if (ex2) pull_img(img, s, i, j, c, f, g);
+    group_sync(1 + grp);
+    if (ex2) {
+      mrt_collide(f, g, c);
+      put_img(img, s, f, g);
+    }
+    group_sync(1 + grp);
+    // level 3: t+2 -> t+3, to global memory; the image is free once everybody has pulled
+    if (ex3) pull_img(img, s, i, j, c, f, g);
+    if (tid < 32) {
+      group_sync(3 + grp);                               // every warp of the group has pulled
+      if (tid == 0) {
+        // the group's reads and in-place writes of this image (ordered before this point by the
+        // barrier) come before the copy engine's writes into it
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fetch(m + TP_STAGES);
+      }
+    } else {
+      group_arrive(3 + grp);
+    }
+    if (ex3) {
+      mrt_collide(f, g, c);
+      store_node(B, c, i, j, f, g);
+    }
+  }
+}
+
 // first step only: A holds the PRE-collision initial state f(x,0); collide it (in place when
 // priming, into the scratch copy when the populations are read out before the first step)
 __global__ void __launch_bounds__(SC_THREADS)
@@ -582,6 +763,85 @@ int stream_collide_configure() {
                                TB_SMEM) == cudaSuccess &&
           cudaFuncSetAttribute(k_stream_collide_3step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                T3_SMEM) == cudaSuccess) ? 0 : -1;
+}
+
+// Tensor maps of the two copies of the populations for k_stream_collide_3step_tma: per copy one
+// 3-D map of the five pair planes (2*px x ny x 5 doubles; rows and planes strided) and one of the
+// four diagonal planes (px x ny x 4).  The spare row ny is outside the maps.  cuTensorMapEncodeTiled
+// is a driver entry point; it is looked up through the runtime, so the library does not link libcuda.
+// 0 = ok (h->tma_ok set), -1 = not available (the plain three-step kernel is used instead).
+int stream_collide_tma_setup(lbm* h) {
+  h->tma_ok = 0;
+  if (h->C.periodic_x || h->is_slab) return -1;
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn encode = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess) {
+      cudaGetLastError();
+      p = nullptr;
+    }
+    return (encode_fn)p;
+  }();
+  if (!encode) return -1;
+  if (cudaFuncSetAttribute(k_stream_collide_3step_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM) !=
+      cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
+  double* base[2] = {h->A, h->B};
+  for (int cpy = 0; cpy < 2; ++cpy) {
+    CUtensorMap tm;
+    const cuuint32_t ones[3] = {1, 1, 1};
+    {
+      const cuuint64_t dims[3] = {(cuuint64_t)2 * h->px, (cuuint64_t)h->ny, 5};
+      const cuuint64_t strides[2] = {(cuuint64_t)h->px * 16, (cuuint64_t)h->ps * 16};
+      const cuuint32_t box[3] = {2 * TP_IW, TP_IH, 5};
+      if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base[cpy], dims, strides, box, ones,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return -1;
+      static_assert(sizeof(tm) == sizeof(h->tmaps[0]), "CUtensorMap is 128 bytes");
+      std::memcpy(h->tmaps[2 * cpy], &tm, sizeof(tm));
+    }
+    {
+      const cuuint64_t dims[3] = {(cuuint64_t)h->px, (cuuint64_t)h->ny, 4};
+      const cuuint64_t strides[2] = {(cuuint64_t)h->px * 8, (cuuint64_t)h->ps * 8};
+      const cuuint32_t box[3] = {TP_IW, TP_IH, 4};
+      if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, base[cpy] + 10 * h->ps, dims, strides, box, ones,
+                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                 CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return -1;
+      std::memcpy(h->tmaps[2 * cpy + 1], &tm, sizeof(tm));
+    }
+    h->tma_base[cpy] = base[cpy];
+  }
+  h->tma_ok = 1;
+  return 0;
+}
+
+// particle-free closed cavity: every row, A -> B, three time steps, persistent TMA-fed kernel
+void launch_stream_collide_3step_tma(lbm* h) {
+  h->launches++;
+  const int cpy = h->A == h->tma_base[0] ? 0 : 1;
+  alignas(64) CUtensorMap tp, td;
+  std::memcpy(&tp, h->tmaps[2 * cpy], sizeof(tp));
+  std::memcpy(&td, h->tmaps[2 * cpy + 1], sizeof(td));
+  const int ntx = (h->nx + T3_X - 1) / T3_X, nty = (h->ny + T3_Y - 1) / T3_Y;
+  const int ntiles = ntx * nty;
+  // One CTA per SM -- but not a grid that shares a factor with the tiles per row: a CTA would then
+  // keep returning to the same few tile columns, and a launch in which every CTA stays in ONE
+  // column takes 20 % longer (4096^2, 147 tiles per row: 1103 us with 147 CTAs against 898 us with
+  // 148; 2048^2, 74 per row: 286 us with 148 against 234 us with 147; 1024^2, 37 per row: 80
+  // against 68 us).  The largest grid coprime to ntx costs a few SMs at most.
+  int grid = std::min(ntiles, h->sm_count > 0 ? h->sm_count : 148);
+  auto gcd = [](int a, int b) { while (b) { const int t = a % b; a = b; b = t; } return a; };
+  while (grid > 1 && ntx > 1 && gcd(grid, ntx) != 1) --grid;
+  launch_k(k_stream_collide_3step_tma, dim3(grid), dim3(TP_THREADS), TP_SMEM, h->stream, h->use_pdl != 0, tp, td,
+           h->B, ntx, ntiles, h->C);
 }
 
 // particle-free lattice: every row, A -> B, three time steps

@@ -98,16 +98,57 @@ def test_two_steps_per_pass_equals_one_step_per_pass_bitwise(gpu, wl):
         a2.set_two_step(2)                           # two steps per pass
         a3 = gpu.Simulation.from_workload(w)
         a3.set_two_step(3)                           # three steps per pass (then two, then one)
+        a3p = gpu.Simulation.from_workload(w)
+        a3p.set_two_step(3)
+        if not prm.get("periodic_x"):
+            a3p.set_tma(False)                       # the plain three-step kernel (a3: the TMA-fed one)
         b = gpu.Simulation.from_workload(w)
         b.set_two_step(False)
         for n in (1, 2, 3, 5, 7, 40):
             b.step(n)
             fb = b.fields(populations=True)
-            for s_ in (a, a2, a3):
+            for s_ in (a, a2, a3, a3p):
                 s_.step(n)
                 fa = s_.fields(populations=True)
                 for k in ("f", "g", "rho", "ux", "uy", "T"):
                     assert np.array_equal(fa[k], fb[k]), (nx, ny, n, k)
+
+
+def test_tma_fed_three_step_kernel_equals_one_step_kernel_bitwise(gpu, wl):
+    """k_stream_collide_3step_tma (persistent CTAs, tile images by cp.async.bulk.tensor into a
+    three-deep ring, two thread groups per CTA) against the one-step kernel, bit for bit, on
+    lattices large enough that every CTA walks many tiles (the ring wraps, both groups and all
+    three stages are reused: 1591, 550 and 150 tiles on 148 SMs), with a ragged last tile column
+    and row, every wall type and a body force; and that periodic lattices refuse it."""
+    rng = np.random.default_rng(23)
+    p = wl.default_params()
+    p.update(wall_T_type=[1, 0, 1, 1], wall_T=[0.3, 0.0, 1.0, -0.2], gbeta=2e-4, T0=0.25,
+             body_ax=1e-5, body_ay=-2e-5, nu=0.05, kappa=0.03)
+    for nx, ny, steps in ((1024, 512, (3, 30)), (601, 299, (6, 9)), (4200, 12, (3,)), (27, 1790, (9,))):
+        T = 0.25 + 0.5 * rng.uniform(-1, 1, size=(ny, nx))
+        w = wl.Workload("tma", nx, ny, p, 1, 1, T_init=T)
+        sims = []
+        for mode in (1,):
+            a = gpu.Simulation.from_workload(w)
+            a.set_two_step(3)
+            a.set_tma(mode)
+            sims.append(a)
+        b = gpu.Simulation.from_workload(w)
+        b.set_two_step(False)
+        for n in steps:
+            b.step(n)
+            fb = b.fields(populations=True)
+            for mode, a in enumerate(sims, 1):
+                a.step(n)
+                fa = a.fields(populations=True)
+                for k in ("f", "g", "rho", "ux", "uy", "T"):
+                    assert np.array_equal(fa[k], fb[k]), (nx, ny, n, k, mode)
+    q = wl.default_params()
+    q.update(periodic_x=1, body_ax=1e-6)
+    s_ = gpu.Simulation.from_workload(wl.Workload("tma_periodic", 64, 32, q, 1, 1))
+    with pytest.raises(Exception):
+        s_.set_tma(True)
+    s_.set_tma(False)
 
 
 def test_periodic_poiseuille(gpu, ob, wl):
