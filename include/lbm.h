@@ -122,7 +122,7 @@ int lbm_step(lbm_t* h, int nsteps);
 int lbm_prepare(lbm_t* h, int nsteps);
 
 /* Environment variables read by lbm_create / lbm_add_particles (defaults in brackets):
- *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_TMA [1], LBM_PDL [1] (programmatic dependent launch along
+ *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_TMA [2] (0 / 1 / 2), LBM_PDL [1] (programmatic dependent launch along
  *   the kernels of a stream), LBM_CHAIN_CTAS_PER_SM [chosen from the sizes],
  *   LBM_DEBUG_SYNC [0] (debugging: synchronise after every direct launch, abort naming the first
  *   kernel that fails). */
@@ -160,15 +160,18 @@ int lbm_set_graph(lbm_t* h, int on);
 int lbm_set_two_step(lbm_t* h, int on);
 
 /* Which kernel takes the three-steps-per-pass passes of a particle-free lattice.
- * on = 1 (default where available; the environment variable LBM_TMA = 0 / 1 sets the default): the
- *   persistent TMA-fed kernel k_stream_collide_3step_tma -- one CTA per SM walks the tiles, each
- *   tile's input image (tile + three-node halo, all 14 populations) arrives by two
- *   cp.async.bulk.tensor box copies into a three-deep shared-memory ring with an mbarrier per stage,
- *   two groups of 512 threads collide alternate tiles in place while the next ones load.
+ * on = 2 (default on closed cavities of at least 2^20 nodes; the environment variable LBM_TMA =
+ *   0 / 1 / 2 sets the default): the persistent TMA-fed kernel k_stream_collide_3step_tma -- one CTA
+ *   per SM walks the tiles, each tile's input image (tile + three-node halo, all 14 populations)
+ *   arrives by two cp.async.bulk.tensor box copies into a three-deep shared-memory ring with an
+ *   mbarrier per stage, two groups of 512 threads collide alternate tiles in place while the next
+ *   ones load; inside a group each warp owns a tile row and hands over to its two neighbour rows
+ *   through per-row mbarriers instead of group-wide barriers.
  *   Closed cavities only (periodic_x = 0), not for slab handles; needs cuTensorMapEncodeTiled.
+ * on = 1: the same kernel with group-wide named barriers between the levels.
  * on = 0: k_stream_collide_3step (one CTA per tile, plain loads).
  * Same arithmetic per node and step: identical results bit for bit.
- * Errors: LBM_E_STATE if on = 1 and the handle has no tensor maps. */
+ * Errors: LBM_E_STATE if on != 0 and the handle has no tensor maps. */
 int lbm_set_tma(lbm_t* h, int on);
 
 /* on = 1 (default; the environment variable LBM_BAND = 0 / 1 / 2 sets the default): lattices WITH particles also use the

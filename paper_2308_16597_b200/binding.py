@@ -260,8 +260,9 @@ class Simulation:
         self._chk(self._L.lbm_set_two_step(self._h, int(on)))
 
     def set_tma(self, on=True):
-        """Three-step passes of a particle-free closed cavity through the persistent TMA-fed kernel
-        (True, the default where available) or the plain three-step kernel (False) (lbm_set_tma)."""
+        """Three-step passes of a particle-free closed cavity: 0 / False the plain three-step kernel,
+        1 / True the persistent TMA-fed kernel with group barriers, 2 the same with the row-wise
+        hand-over (the default from 2^20 nodes) (lbm_set_tma)."""
         self._chk(self._L.lbm_set_tma(self._h, int(on)))
 
     # ---- y-slabs: the two halves of a step and the exchanges' end points (slabs.py drives them) ----

@@ -354,9 +354,10 @@ static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, 
   h->use_tma = 0;
   if (h->two_step_ok && stream_collide_tma_setup(h) == 0) {
     const char* et = getenv("LBM_TMA");
-    // default: from 2^20 nodes up (measured per pass against the plain three-step kernel, CUDA
-    // events over 402 steps: 1024^2 66.6 / 68.1 us, 2048^2 229 / 236 us, 4096^2 886 / 916 us)
-    h->use_tma = et ? (atoi(et) != 0) : ((long long)nx * ny >= LBM_TMA_MIN_NODES ? 1 : 0);
+    // default: from 2^20 nodes up, with the row-wise hand-over (2).  Measured per pass against the
+    // plain three-step kernel (CUDA events, 402 steps): 1024^2 64.0 / 68.1 us, 2048^2 217 / 236 us,
+    // 4096^2 855 / 903 us; with group barriers (1): 66.7 / 229 / 886 us
+    h->use_tma = et ? std::min(std::max(atoi(et), 0), 2) : ((long long)nx * ny >= LBM_TMA_MIN_NODES ? 2 : 0);
   }
   if (particles_configure(h) != 0) {
     delete h;
@@ -1243,7 +1244,7 @@ int lbm_set_two_step(lbm_t* h, int on) {
 int lbm_set_tma(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
   if (on && !h->tma_ok) return fail(h, LBM_E_STATE, "lbm_set_tma: no tensor maps for this handle (periodic x, a slab, or the driver lacks cuTensorMapEncodeTiled)");
-  h->use_tma = on ? 1 : 0;
+  h->use_tma = on ? (on >= 2 ? 2 : 1) : 0;
   return LBM_OK;
 }
 

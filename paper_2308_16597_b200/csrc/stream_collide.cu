@@ -477,7 +477,7 @@ constexpr int TP_IMG_DOUBLES = 14 * TP_PLANE;
 constexpr int TP_IMG_BYTES = TP_IMG_DOUBLES * (int)sizeof(double);   // 72,576 = 567 x 128
 constexpr int TP_STAGES = 3, TP_GROUPS = 2;
 constexpr int TP_THREADS = TP_GROUPS * T3_THREADS;
-constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 128;   // + the mbarriers
+constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 64 + TP_GROUPS * 2 * T3_H * 8;   // + the stage and the row mbarriers
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
@@ -548,6 +548,30 @@ __device__ __forceinline__ void put_img(double* img, int s, const double (&f)[9]
   for (int k = 0; k < 4; ++k) D[k * TP_PLANE] = f[5 + k];
 }
 
+// Row-wise hand-over inside a group (ROWSYNC): warp w of a group owns row w of the dilated tile,
+// and a level's pull of row r reads only rows r-1, r, r+1 of the level below, so instead of four
+// group-wide barriers per tile each warp publishes how far it has come (a counter per row in
+// shared memory, st.release / ld.acquire at CTA scope) and waits for its two neighbours only:
+// before writing its row back in place, that they have pulled; before pulling the next level,
+// that they have written.  Neighbouring rows stay within one phase of each other, the sixteen
+// warps of a group spread over the phases, and shared-memory phases of some warps run under the
+// fp64 phases of others.
+// rb: the group's row barriers [T3_H][2] (mbarriers, one arrival each): phases 1 and 3 of a tile
+// complete [row][0], phases 2 and 4 [row][1], so that two completions of one barrier are always
+// separated by the neighbours' observation of the first (a row cannot publish phase p + 2 before
+// both neighbours have published p + 1, i.e. have seen p) and the parity wait stays unambiguous
+__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0)
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))) : "memory");
+}
+__device__ __forceinline__ void row_wait(unsigned long long* rb, int row, int phase) {
+  const unsigned parity = (unsigned)((phase - 1) >> 1) & 1u;   // two completions per barrier and tile
+  if (row > 0) mbar_wait(rb + 2 * (row - 1) + ((phase - 1) & 1), parity);
+  if (row < T3_H - 1) mbar_wait(rb + 2 * (row + 1) + ((phase - 1) & 1), parity);
+}
+
+template <bool ROWSYNC>
 __global__ void __launch_bounds__(TP_THREADS, 1)
 k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __grid_constant__ CUtensorMap tm_diag,
                            double* __restrict__ B, int ntx, int ntiles, const LbmConst c) {
@@ -570,9 +594,15 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     tma_load_3d(img, &tm_pair, 2 * i0, j0, 0, full + st);
     tma_load_3d(img + TP_PAIR_DOUBLES, &tm_diag, i0, j0, 0, full + st);
   };
+  unsigned long long* const empty = full + 4;                   // ROWSYNC: image handed back (16 warps)
+  unsigned long long* const rb = full + 8 + grp * (2 * T3_H);   // the group's row barriers [row][2]
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int st = 0; st < TP_STAGES; ++st) mbar_init(full + st, 1);
+    if (ROWSYNC) {
+      for (int st = 0; st < TP_STAGES; ++st) mbar_init(empty + st, T3_THREADS / 32);
+      for (int k = 0; k < TP_GROUPS * 2 * T3_H; ++k) mbar_init(full + 8 + k, 1);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -592,25 +622,59 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     const bool ex3 = ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3;
     double f[9], g[5];
     mbar_wait(full + st, (unsigned)(m / TP_STAGES) & 1u);
-    // level 1: t -> t+1
-    if (ex1) pull_img(img, s, i, j, c, f, g);
-    group_sync(1 + grp);
-    if (ex1) {
-      mrt_collide(f, g, c);
-      put_img(img, s, f, g);
+    if (ROWSYNC) {
+      // level 1: t -> t+1
+      if (ex1) pull_img(img, s, i, j, c, f, g);
+      row_publish(rb, ty, 1);
+      if (ex1) mrt_collide(f, g, c);
+      row_wait(rb, ty, 1);                                 // the neighbour rows have pulled
+      if (ex1) put_img(img, s, f, g);
+      row_publish(rb, ty, 2);
+      // level 2: t+1 -> t+2
+      row_wait(rb, ty, 2);                                 // ... have written level 1
+      if (ex2) pull_img(img, s, i, j, c, f, g);
+      row_publish(rb, ty, 3);
+      if (ex2) mrt_collide(f, g, c);
+      row_wait(rb, ty, 3);
+      if (ex2) put_img(img, s, f, g);
+      row_publish(rb, ty, 4);
+      // level 3: t+2 -> t+3
+      row_wait(rb, ty, 4);
+      if (ex3) pull_img(img, s, i, j, c, f, g);
+    } else {
+      // level 1: t -> t+1
+      if (ex1) pull_img(img, s, i, j, c, f, g);
+      group_sync(1 + grp);
+      if (ex1) {
+        mrt_collide(f, g, c);
+        put_img(img, s, f, g);
+      }
+      group_sync(1 + grp);
+      // level 2: t+1 -> t+2
+      if (ex2) pull_img(img, s, i, j, c, f, g);
+      group_sync(1 + grp);
+      if (ex2) {
+        mrt_collide(f, g, c);
+        put_img(img, s, f, g);
+      }
+      group_sync(1 + grp);
+      // level 3: t+2 -> t+3
+      if (ex3) pull_img(img, s, i, j, c, f, g);
     }
-    group_sync(1 + grp);
-    // level 2: t+1 -> t+2
-    if (ex2) pull_img(img, s, i, j, c, f, g);
-    group_sync(1 + grp);
-    if (ex2) {
-      mrt_collide(f, g, c);
-      put_img(img, s, f, g);
-    }
-    group_sync(1 + grp);
-    // level 3: t+2 -> t+3, to global memory; the image is free once everybody has pulled
-    if (ex3) pull_img(img, s, i, j, c, f, g);
-    if (tid < 32) {
+    // ... to global memory; the image is free once everybody has pulled
+    if (ROWSYNC) {
+      // the warps of a group may be tiles apart here, so the image is handed back through an
+      // mbarrier of its own (one arrival per warp; a named barrier would count a fast warp twice)
+      __syncwarp();
+      if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + st)) : "memory");
+      if (tid < 32) {
+        mbar_wait(empty + st, (unsigned)(m / TP_STAGES) & 1u);
+        if (tid == 0) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          fetch(m + TP_STAGES);
+        }
+      }
+    } else if (tid < 32) {
       group_sync(3 + grp);                               // every warp of the group has pulled
       if (tid == 0) {
         // the group's reads and in-place writes of this image (ordered before this point by the
@@ -787,8 +851,10 @@ int stream_collide_tma_setup(lbm* h) {
     return (encode_fn)p;
   }();
   if (!encode) return -1;
-  if (cudaFuncSetAttribute(k_stream_collide_3step_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM) !=
-      cudaSuccess) {
+  if (cudaFuncSetAttribute(k_stream_collide_3step_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM) !=
+          cudaSuccess ||
+      cudaFuncSetAttribute(k_stream_collide_3step_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM) !=
+          cudaSuccess) {
     cudaGetLastError();
     return -1;
   }
@@ -840,8 +906,12 @@ void launch_stream_collide_3step_tma(lbm* h) {
   int grid = std::min(ntiles, h->sm_count > 0 ? h->sm_count : 148);
   auto gcd = [](int a, int b) { while (b) { const int t = a % b; a = b; b = t; } return a; };
   while (grid > 1 && ntx > 1 && gcd(grid, ntx) != 1) --grid;
-  launch_k(k_stream_collide_3step_tma, dim3(grid), dim3(TP_THREADS), TP_SMEM, h->stream, h->use_pdl != 0, tp, td,
-           h->B, ntx, ntiles, h->C);
+  if (h->use_tma >= 2)
+    launch_k(k_stream_collide_3step_tma<true>, dim3(grid), dim3(TP_THREADS), TP_SMEM, h->stream, h->use_pdl != 0, tp,
+             td, h->B, ntx, ntiles, h->C);
+  else
+    launch_k(k_stream_collide_3step_tma<false>, dim3(grid), dim3(TP_THREADS), TP_SMEM, h->stream, h->use_pdl != 0, tp,
+             td, h->B, ntx, ntiles, h->C);
 }
 
 // particle-free lattice: every row, A -> B, three time steps
