@@ -283,9 +283,12 @@ def main():
     # then carries two lattice updates per node (2 x 224 B algorithmic) while moving ~137 B per
     # update, so its fraction of the 224 B/LU roofline may exceed 1
     # (three per launch with k_stream_collide_3step: 3 x 224 B algorithmic, ~105 B per update moved)
-    three_step = ovl.get("stream_collide_3step", 0.0) > 0.0 and w.particles is None
+    # (k_stream_collide_3step_tma: the persistent TMA-fed variant, the default from 2^20 nodes)
+    three_tma = ovl.get("stream_collide_3step_tma", 0.0) > 0.0 and w.particles is None
+    three_step = three_tma or (ovl.get("stream_collide_3step", 0.0) > 0.0 and w.particles is None)
     two_step = three_step or (ovl.get("stream_collide_2step", 0.0) > 0.0 and ovl.get("stream_collide", 0.0) == 0.0)
-    kname = "stream_collide_3step" if three_step else ("stream_collide_2step" if two_step else "stream_collide")
+    kname = ("stream_collide_3step_tma" if three_tma else "stream_collide_3step") if three_step else \
+        ("stream_collide_2step" if two_step else "stream_collide")
     per_launch = 3 if three_step else (2 if two_step else 1)
     far_s = seq[kname] * 1e-3
     far_ovl_s = ovl[kname] * 1e-3

@@ -22,7 +22,7 @@ char g_create_error[512] = "";
 const char* const kKernelNames[K_COUNT] = {
     "stream_collide", "build_links", "bounce_back_force", "integrate_uncover",
     "flags_cover", "refill", "init_collide", "refill_commit", "stream_collide_2step", "band_plan",
-    "stream_collide_3step"};
+    "stream_collide_3step", "stream_collide_3step_tma"};
 
 int fail(lbm* h, int code, const char* fmt, ...) {
   va_list ap;
@@ -959,10 +959,12 @@ int lbm_step(lbm_t* h, int nsteps) {
   while (s < nsteps) {
     if (h->np == 0 && h->two_step >= 2 && nsteps - s >= 3) {
       // particle-free lattice: three time steps per pass
-      {
+      if (h->use_tma && h->tma_ok) {
+        Timed tm(h, K_STREAM_COLLIDE_3STEP_TMA, h->stream);
+        launch_stream_collide_3step_tma(h);
+      } else {
         Timed tm(h, K_STREAM_COLLIDE_3STEP, h->stream);
-        if (h->use_tma && h->tma_ok) launch_stream_collide_3step_tma(h);
-        else launch_stream_collide_3step(h);
+        launch_stream_collide_3step(h);
       }
       std::swap(h->A, h->B);
       h->steps_done += 3;

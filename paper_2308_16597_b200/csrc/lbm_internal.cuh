@@ -33,7 +33,8 @@
 
 enum {
   K_STREAM_COLLIDE = 0, K_BUILD_LINKS, K_BOUNCE_BACK, K_MOVE, K_COVER, K_REFILL,
-  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_BAND_PLAN, K_STREAM_COLLIDE_3STEP, K_COUNT
+  K_INIT, K_REFILL_COMMIT, K_STREAM_COLLIDE_2STEP, K_BAND_PLAN, K_STREAM_COLLIDE_3STEP,
+  K_STREAM_COLLIDE_3STEP_TMA, K_COUNT
 };
 
 // link_dir byte: bits 0-3 = alpha (1..8), bits 4-5 = number of fluid nodes behind x_f along

@@ -266,6 +266,26 @@ k_stream_collide_slab(const double* __restrict__ A, double* __restrict__ B,
   }
 }
 
+// ---- mbarrier helpers (shared memory, CTA scope)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+  const unsigned a = smem_u32(bar);
+  unsigned ok;
+  do {
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive(void* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
 // TWO time steps per pass over particle-free rows (traffic below 224 B per
 // update).  A CTA owns a TB_X x TB_Y tile of output nodes.  Phase 1: its TB_W x TB_H threads
 // update the tile plus a one-node halo from the state at t (the same pull + collide as the
@@ -284,14 +304,17 @@ k_stream_collide_slab(const double* __restrict__ A, double* __restrict__ B,
 constexpr int TB_X = 30, TB_Y = 14;   // TB_W = 32: one warp per tile row
 constexpr int TB_W = TB_X + 2, TB_H = TB_Y + 2;
 constexpr int TB_THREADS = TB_W * TB_H;   // 512 = 16 warps
-constexpr int TB_SMEM = 14 * TB_THREADS * (int)sizeof(double);
+constexpr int TB_SMEM = 14 * TB_THREADS * (int)sizeof(double) + TB_H * 8;   // + one mbarrier per tile row
 
 __global__ void __launch_bounds__(TB_THREADS)
 k_stream_collide_2step(const double* __restrict__ Aband, const double* __restrict__ Atop,
                        double* __restrict__ Bband, const int* __restrict__ bandp, int nparts,
                        int part, const LbmConst c) {
-  extern __shared__ double s_pop[];   // [14][TB_H][TB_W]
+  extern __shared__ double s_pop[];   // [14][TB_H][TB_W], then TB_H mbarriers
+  unsigned long long* const rowbar = reinterpret_cast<unsigned long long*>(s_pop + 14 * TB_THREADS);
   pdl_launch_dependents();
+  if (threadIdx.x < TB_H) mbar_init(rowbar + threadIdx.x, 1);
+  __syncthreads();                    // (under the predecessor's tail: nothing of its data is touched yet)
   pdl_wait();
   const int Qs = bandp ? *bandp : c.ny;
   const bool upper = Qs < 0;                       // the band is [Q, ny) instead of [0, Q)
@@ -320,7 +343,14 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
 #pragma unroll
     for (int k = 0; k < 5; ++k) s_pop[(9 + k) * TB_THREADS + threadIdx.x] = g[k];
   }
-  __syncthreads();
+  // A warp is a tile row, and phase 2 of row ty pulls from rows ty - 1, ty, ty + 1 only: instead of
+  // a CTA-wide barrier each row signals its own mbarrier and waits for its two neighbours', so the
+  // sixteen warps drift apart and some rows' loads run under other rows' second collision.
+  __syncwarp();
+  if (tx == 0) mbar_arrive(rowbar + ty);
+  if (ty == 0 || ty == TB_H - 1) return;             // halo rows have no phase 2
+  mbar_wait(rowbar + ty - 1, 0);
+  mbar_wait(rowbar + ty + 1, 0);
   // phase 2: the tile's own nodes
   if (tx < 1 || tx > TB_X || ty < 1 || ty > TB_Y || i >= c.nx || j >= c.ny || (upper ? j < Q : j >= Q)) return;
   if (i >= 1 && i < c.nx - 1 && j >= 1 && j < c.ny - 1) {
@@ -479,21 +509,6 @@ constexpr int TP_STAGES = 3, TP_GROUPS = 2;
 constexpr int TP_THREADS = TP_GROUPS * T3_THREADS;
 constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 64 + TP_GROUPS * 2 * T3_H * 8;   // + the stage and the row mbarriers
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(void* bar, unsigned count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
-  const unsigned a = smem_u32(bar);
-  unsigned ok;
-  do {
-    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                 : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-  } while (!ok);
-}
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, void* bar) {
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
