@@ -286,6 +286,22 @@ __device__ __forceinline__ void mbar_arrive(void* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+// Row-wise hand-over between the warps (= tile rows) of a multi-step kernel.
+// rb: row barriers [rows][2] (mbarriers, one arrival each): phases 1 and 3 of a tile
+// complete [row][0], phases 2 and 4 [row][1], so that two completions of one barrier are always
+// separated by the neighbours' observation of the first (a row cannot publish phase p + 2 before
+// both neighbours have published p + 1, i.e. have seen p) and the parity wait stays unambiguous
+__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0)
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))) : "memory");
+}
+__device__ __forceinline__ void row_wait(unsigned long long* rb, int row, int phase, int rows) {
+  const unsigned parity = (unsigned)((phase - 1) >> 1) & 1u;   // two completions per barrier and tile
+  if (row > 0) mbar_wait(rb + 2 * (row - 1) + ((phase - 1) & 1), parity);
+  if (row < rows - 1) mbar_wait(rb + 2 * (row + 1) + ((phase - 1) & 1), parity);
+}
+
 // TWO time steps per pass over particle-free rows (traffic below 224 B per
 // update).  A CTA owns a TB_X x TB_Y tile of output nodes.  Phase 1: its TB_W x TB_H threads
 // update the tile plus a one-node halo from the state at t (the same pull + collide as the
@@ -399,7 +415,7 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
 constexpr int T3_X = 28, T3_Y = 12;
 constexpr int T3_W = T3_X + 4, T3_H = T3_Y + 4;   // 32 x 16: one warp per row of the halo'd tile
 constexpr int T3_THREADS = T3_W * T3_H;
-constexpr int T3_SMEM = 14 * T3_THREADS * (int)sizeof(double);
+constexpr int T3_SMEM = 14 * T3_THREADS * (int)sizeof(double) + 2 * T3_H * 8;   // + two mbarriers per tile row
 
 // f_k, g_k of the node in slot `tid` (lattice column iw -- wrapped when periodic --, row j) pulled
 // from the slots of its neighbours in the tile image s_pop[14][T3_THREADS]; cavity walls as in
@@ -438,8 +454,11 @@ __device__ __forceinline__ void pull_tile3(const double* s_pop, int tid, int iw,
 
 __global__ void __launch_bounds__(T3_THREADS)
 k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, const LbmConst c) {
-  extern __shared__ double s_pop[];   // [14][T3_H][T3_W]
+  extern __shared__ double s_pop[];   // [14][T3_H][T3_W], then the row barriers [T3_H][2]
+  unsigned long long* const rb = reinterpret_cast<unsigned long long*>(s_pop + 14 * T3_THREADS);
   pdl_launch_dependents();
+  if (threadIdx.x < 2 * T3_H) mbar_init(rb + threadIdx.x, 1);
+  __syncthreads();                    // (under the predecessor's tail)
   pdl_wait();
   const int tid = threadIdx.x;
   const int tx = tid % T3_W, ty = tid / T3_W;
@@ -459,20 +478,25 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
 #pragma unroll
     for (int k = 0; k < 5; ++k) s_pop[(9 + k) * T3_THREADS + tid] = g[k];
   }
-  __syncthreads();
+  // No CTA-wide barriers: a warp is a tile row and hands over to its two neighbour rows only
+  // (phase 1: level 1 written; 2: level 1 pulled; 3: level 2 written)
+  row_publish(rb, ty, 1);
+  row_wait(rb, ty, 1, T3_H);
   // level 2: t+1 -> t+2 on the tile dilated by one node, written back in place
   const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2 &&
                    (!c.periodic_x || (i >= -1 && i <= c.nx));
   if (ex2) pull_tile3(s_pop, tid, iw, j, c, f, g);
-  __syncthreads();                    // every level-1 value has been read
+  row_publish(rb, ty, 2);
+  if (ex2) mrt_collide(f, g, c);
+  row_wait(rb, ty, 2, T3_H);          // the neighbour rows have read this row's level-1 values
   if (ex2) {
-    mrt_collide(f, g, c);
 #pragma unroll
     for (int k = 0; k < 9; ++k) s_pop[k * T3_THREADS + tid] = f[k];
 #pragma unroll
     for (int k = 0; k < 5; ++k) s_pop[(9 + k) * T3_THREADS + tid] = g[k];
   }
-  __syncthreads();
+  row_publish(rb, ty, 3);
+  row_wait(rb, ty, 3, T3_H);
   // level 3: t+2 -> t+3 on the tile's own nodes, to global memory
   if (!(ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3 && i >= 0 && i < c.nx)) return;
   pull_tile3(s_pop, tid, iw, j, c, f, g);
@@ -571,21 +595,6 @@ __device__ __forceinline__ void put_img(double* img, int s, const double (&f)[9]
 // that they have written.  Neighbouring rows stay within one phase of each other, the sixteen
 // warps of a group spread over the phases, and shared-memory phases of some warps run under the
 // fp64 phases of others.
-// rb: the group's row barriers [T3_H][2] (mbarriers, one arrival each): phases 1 and 3 of a tile
-// complete [row][0], phases 2 and 4 [row][1], so that two completions of one barrier are always
-// separated by the neighbours' observation of the first (a row cannot publish phase p + 2 before
-// both neighbours have published p + 1, i.e. have seen p) and the parity wait stays unambiguous
-__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase) {
-  __syncwarp();
-  if ((threadIdx.x & 31) == 0)
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))) : "memory");
-}
-__device__ __forceinline__ void row_wait(unsigned long long* rb, int row, int phase) {
-  const unsigned parity = (unsigned)((phase - 1) >> 1) & 1u;   // two completions per barrier and tile
-  if (row > 0) mbar_wait(rb + 2 * (row - 1) + ((phase - 1) & 1), parity);
-  if (row < T3_H - 1) mbar_wait(rb + 2 * (row + 1) + ((phase - 1) & 1), parity);
-}
-
 template <bool ROWSYNC>
 __global__ void __launch_bounds__(TP_THREADS, 1)
 k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __grid_constant__ CUtensorMap tm_diag,
@@ -642,19 +651,19 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
       if (ex1) pull_img(img, s, i, j, c, f, g);
       row_publish(rb, ty, 1);
       if (ex1) mrt_collide(f, g, c);
-      row_wait(rb, ty, 1);                                 // the neighbour rows have pulled
+      row_wait(rb, ty, 1, T3_H);                                 // the neighbour rows have pulled
       if (ex1) put_img(img, s, f, g);
       row_publish(rb, ty, 2);
       // level 2: t+1 -> t+2
-      row_wait(rb, ty, 2);                                 // ... have written level 1
+      row_wait(rb, ty, 2, T3_H);                                 // ... have written level 1
       if (ex2) pull_img(img, s, i, j, c, f, g);
       row_publish(rb, ty, 3);
       if (ex2) mrt_collide(f, g, c);
-      row_wait(rb, ty, 3);
+      row_wait(rb, ty, 3, T3_H);
       if (ex2) put_img(img, s, f, g);
       row_publish(rb, ty, 4);
       // level 3: t+2 -> t+3
-      row_wait(rb, ty, 4);
+      row_wait(rb, ty, 4, T3_H);
       if (ex3) pull_img(img, s, i, j, c, f, g);
     } else {
       // level 1: t -> t+1
