@@ -8,7 +8,6 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
-#include <map>
 #include <new>
 #include <utility>
 #include <vector>
@@ -564,37 +563,48 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
     SS[n0 + k] = os;
     dmax = std::max(dmax, 2.0 * r);
   }
-  // overlap test through a host cell grid (cell >= largest diameter)
+  // overlap test through a host cell grid (cell >= largest diameter): flat cells filled in particle
+  // order (counting sort), each new particle tested against the earlier ones in its 3 x 3 cells
   {
     const double cell = std::max(dmax, 1.0);
-    std::map<std::pair<int, int>, std::vector<int>> grid;
-    for (int k = 0; k < nt; ++k) {
-      const int ci = (int)std::floor(X[k] / cell), cj = (int)std::floor(Y[k] / cell);
-      if (k >= n0)
-        for (int a = ci - 1; a <= ci + 1; ++a)
-          for (int b = cj - 1; b <= cj + 1; ++b) {
-            auto it = grid.find({a, b});
-            if (it == grid.end()) continue;
-            for (int m : it->second) {
-              const double dx = X[k] - X[m], dy = Y[k] - Y[m];
-              const double dist = std::sqrt(dx * dx + dy * dy);
-              // circles: centre distance against r_a + r_b; with an ellipse: the support
-              // functions along the line of centres (conservative)
-              auto support = [&](int q, double nx, double ny) {
-                if (SA[q] == SB[q]) return R[q];
-                const double mm = nx * SC[q] + ny * SS[q], ww = ny * SC[q] - nx * SS[q];
-                const double am = SA[q] * mm, bw = SB[q] * ww;
-                return std::sqrt(am * am + bw * bw);
-              };
-              bool bad;
-              if (SA[k] == SB[k] && SA[m] == SB[m]) bad = dist < R[k] + R[m];
-              else bad = !(dist > 0.0) || dist < support(k, dx / dist, dy / dist) + support(m, dx / dist, dy / dist);
-              if (bad)
-                return fail(h, LBM_E_ARG, "add_particles: particles %d and %d overlap", m, k);
-            }
-          }
-      grid[{ci, cj}].push_back(k);
+    double xlo = X[0], ylo = Y[0], xhi = X[0], yhi = Y[0];
+    for (int k = 1; k < nt; ++k) {
+      xlo = std::min(xlo, X[k]); xhi = std::max(xhi, X[k]);
+      ylo = std::min(ylo, Y[k]); yhi = std::max(yhi, Y[k]);
     }
+    const int gx = (int)std::floor((xhi - xlo) / cell) + 1, gy = (int)std::floor((yhi - ylo) / cell) + 1;
+    std::vector<int> ci(nt), cj(nt), start((size_t)gx * gy + 1, 0), order(nt);
+    for (int k = 0; k < nt; ++k) {
+      ci[k] = std::min((int)std::floor((X[k] - xlo) / cell), gx - 1);
+      cj[k] = std::min((int)std::floor((Y[k] - ylo) / cell), gy - 1);
+      start[(size_t)cj[k] * gx + ci[k] + 1]++;
+    }
+    for (size_t q = 0; q < (size_t)gx * gy; ++q) start[q + 1] += start[q];
+    {
+      std::vector<int> fill(start.begin(), start.end() - 1);
+      for (int k = 0; k < nt; ++k) order[fill[(size_t)cj[k] * gx + ci[k]]++] = k;   // ascending k inside a cell
+    }
+    // circles: centre distance against r_a + r_b; with an ellipse: the support functions along
+    // the line of centres (conservative)
+    auto support = [&](int q, double nx, double ny) {
+      if (SA[q] == SB[q]) return R[q];
+      const double mm = nx * SC[q] + ny * SS[q], ww = ny * SC[q] - nx * SS[q];
+      const double am = SA[q] * mm, bw = SB[q] * ww;
+      return std::sqrt(am * am + bw * bw);
+    };
+    for (int k = n0; k < nt; ++k)
+      for (int b = std::max(cj[k] - 1, 0); b <= std::min(cj[k] + 1, gy - 1); ++b)
+        for (int a = std::max(ci[k] - 1, 0); a <= std::min(ci[k] + 1, gx - 1); ++a)
+          for (int q = start[(size_t)b * gx + a]; q < start[(size_t)b * gx + a + 1]; ++q) {
+            const int m = order[q];
+            if (m >= k) break;                             // (a new particle is tested against the earlier ones)
+            const double dx = X[k] - X[m], dy = Y[k] - Y[m];
+            const double dist = std::sqrt(dx * dx + dy * dy);
+            bool bad;
+            if (SA[k] == SB[k] && SA[m] == SB[m]) bad = dist < R[k] + R[m];
+            else bad = !(dist > 0.0) || dist < support(k, dx / dist, dy / dist) + support(m, dx / dist, dy / dist);
+            if (bad) return fail(h, LBM_E_ARG, "add_particles: particles %d and %d overlap", m, k);
+          }
   }
   // upload
   const int c = h->cur;
