@@ -301,17 +301,23 @@ def main():
         alg_bytes = per_launch * BYTES_PER_LU * n_fluid
     elif band_rows > 0:
         outside = flag[band_q:] if band_q > 0 else flag[:-band_q]
-        fluid_top = int((outside == 0).sum()) + 0.5 * w.nx
-        alg_bytes = BYTES_PER_LU * fluid_top + FLAG_BYTES * (w.ny - band_rows + 0.5) * w.nx
+        # (two steps per pass: the one-step kernel also updates row Q-1 in every other step)
+        extra = 0.0 if ovl.get("stream_collide_3step", 0.0) > 0.0 else 0.5
+        fluid_top = int((outside == 0).sum()) + extra * w.nx
+        alg_bytes = BYTES_PER_LU * fluid_top + FLAG_BYTES * (w.ny - band_rows + extra) * w.nx
     else:
         alg_bytes = BYTES_PER_LU * n_fluid + FLAG_BYTES * n
     band = None
     if band_rows > 0 and not two_step:
-        b_s = ovl["stream_collide_2step"] * 1e-3
+        # the band's kernel: three steps per pass (k_stream_collide_3step<BAND>, a third of the tile
+        # rows per step) under the suspension by default, else two (k_stream_collide_2step, half)
+        bk = "stream_collide_3step" if ovl.get("stream_collide_3step", 0.0) > 0.0 else "stream_collide_2step"
+        b_s = ovl[bk] * 1e-3
         band = {"rows": band_rows, "where": "below the suspension" if band_q > 0 else "above the suspension",
-                "kernel": "k_stream_collide_2step", "launches_per_step": 1,
+                "kernel": "k_" + bk + ("<BAND>" if bk.endswith("3step") else ""), "launches_per_step": 1,
+                "steps_per_pass": 3 if bk.endswith("3step") else 2,
                 "lattice_updates_per_launch": band_rows * w.nx, "avg_launch_ms": b_s * 1e3,
-                "avg_launch_ms_alone": seq["stream_collide_2step"],
+                "avg_launch_ms_alone": seq[bk],
                 "algorithmic_gbs_at_224_B_per_update": BYTES_PER_LU * band_rows * w.nx / b_s / 1e9 if b_s > 0 else None}
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(peaks_path):

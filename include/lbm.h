@@ -122,7 +122,7 @@ int lbm_step(lbm_t* h, int nsteps);
 int lbm_prepare(lbm_t* h, int nsteps);
 
 /* Environment variables read by lbm_create / lbm_add_particles (defaults in brackets):
- *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_TMA [2] (0 / 1 / 2), LBM_PDL [1] (programmatic dependent launch along
+ *   LBM_GRAPH [1], LBM_BAND [1] (0 / 1 / 2), LBM_BAND_STEPS [3] (2 / 3), LBM_STEPS_PER_PASS [3] (1 / 2 / 3), LBM_TMA [2] (0 / 1 / 2), LBM_PDL [1] (programmatic dependent launch along
  *   the kernels of a stream), LBM_CHAIN_CTAS_PER_SM [chosen from the sizes],
  *   LBM_DEBUG_SYNC [0] (debugging: synchronise after every direct launch, abort naming the first
  *   kernel that fails). */
@@ -158,6 +158,14 @@ int lbm_set_graph(lbm_t* h, int on);
  *   the two-step and one-step kernels.
  * The arithmetic per node and step is the same in all three, so results are identical bit for bit. */
 int lbm_set_two_step(lbm_t* h, int on);
+
+/* Time steps per pass in a band UNDER the suspension (lbm_set_band): 3 (default; the environment
+ * variable LBM_BAND_STEPS = 2 / 3 sets the default): periods of six steps, the band kernel
+ * k_stream_collide_3step<BAND> advances the rows [0, Q) three steps per pass and hands row Q-1 at
+ * the two intermediate times to the rows above through the spare row; 2: periods of four steps
+ * with k_stream_collide_2step.  A band above a settled suspension always takes two steps per pass.
+ * Identical results bit for bit.  Errors: LBM_E_ARG unless steps is 2 or 3. */
+int lbm_set_band_steps(lbm_t* h, int steps);
 
 /* Which kernel takes the three-steps-per-pass passes of a particle-free lattice.
  * on = 2 (default on closed cavities of at least 2^20 nodes; the environment variable LBM_TMA =

@@ -78,6 +78,7 @@ def load_library():
     L.lbm_set_overlap.argtypes = [vp, C.c_int]
     L.lbm_set_two_step.argtypes = [vp, C.c_int]
     L.lbm_set_tma.argtypes = [vp, C.c_int]
+    L.lbm_set_band_steps.argtypes = [vp, C.c_int]
     L.lbm_set_graph.argtypes = [vp, C.c_int]
     L.lbm_set_band.argtypes = [vp, C.c_int]
     L.lbm_get_band.argtypes = [vp, C.POINTER(C.c_int)]
@@ -116,7 +117,7 @@ def load_library():
                  "lbm_slab_forces", "lbm_slab_force_buffer", "lbm_slab_advance", "lbm_slab_check",
                  "lbm_slab_halo_doubles", "lbm_slab_pack", "lbm_slab_unpack", "lbm_slab_exchange_halos",
                  "lbm_slab_combine_forces", "lbm_slab_link_peers", "lbm_slab_fence",
-                 "lbm_get_macroscopic_static", "lbm_prepare", "lbm_set_tma"):
+                 "lbm_get_macroscopic_static", "lbm_prepare", "lbm_set_tma", "lbm_set_band_steps"):
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -258,6 +259,10 @@ class Simulation:
         """Particle-free lattices: time steps per pass over the populations.  False / 0: one;
         True / 1 / 2: two; 3: three (lbm_set_two_step)."""
         self._chk(self._L.lbm_set_two_step(self._h, int(on)))
+
+    def set_band_steps(self, steps):
+        """Time steps per pass in a band under the suspension: 3 (default) or 2 (lbm_set_band_steps)."""
+        self._chk(self._L.lbm_set_band_steps(self._h, int(steps)))
 
     def set_tma(self, on=True):
         """Three-step passes of a particle-free closed cavity: 0 / False the plain three-step kernel,

@@ -348,6 +348,8 @@ static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, 
     const char* e3 = getenv("LBM_STEPS_PER_PASS");
     if (e3) h->two_step = atoi(e3) >= 3 ? 2 : (atoi(e3) == 2 ? 1 : 0);
   }
+  h->band_steps = 3;
+  if (const char* eb = getenv("LBM_BAND_STEPS")) h->band_steps = atoi(eb) >= 3 ? 3 : 2;
   // three steps per pass through the persistent TMA-fed kernel where it can run (closed cavity,
   // tensor maps encodable); LBM_TMA=0 keeps the plain three-step kernel
   h->use_tma = 0;
@@ -717,8 +719,14 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
   const int sp = h->cur;   // step parity: which newborn counter / repulsion grid this step uses
   double* X = (phase & 1) ? h->B : h->A;   // the copies as they were named at the start of the period
   double* Y = (phase & 1) ? h->A : h->B;
-  const double* band_src = phase < 2 ? X : Y;
-  double* band_dst = phase < 2 ? Y : X;
+  // h->band3: periods of SIX steps, the band advancing three steps per pass (phases 0-2: X -> Y,
+  // 3-5: Y -> X); the band and the rows above it are then in the same copy at the start of every
+  // half period, so the band kernel needs no second source and the one-step kernel never computes
+  // a band row: it reads row Q-1 in place in the first step of a half period and from the spare
+  // row, where the band kernel's top tiles put it, in the other two
+  const int half = h->band3 ? 3 : 2;
+  double* band_src = phase < half ? X : Y;
+  double* band_dst = phase < half ? Y : X;
   if (banded && phase == 0 && plan) {   // one plan serves two periods (k_band_plan allows for 8 steps of motion)
     { Timed tm(h, K_BAND_PLAN, S1); launch_band_plan(h, S1); }
     note_chain_node(h, S1);
@@ -733,7 +741,13 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     if (fork) cudaEventRecord(h->ev_bb, S1);
   }
   if (banded) {
-    { Timed tm(h, K_STREAM_COLLIDE_2STEP, S0); launch_stream_collide_band(h, band_src, X, band_dst, 2, phase & 1); }
+    if (h->band3) {
+      Timed tm(h, K_STREAM_COLLIDE_3STEP, S0);
+      launch_stream_collide_band3(h, band_src, band_dst, 3, phase % 3);
+    } else {
+      Timed tm(h, K_STREAM_COLLIDE_2STEP, S0);
+      launch_stream_collide_band(h, band_src, X, band_dst, 2, phase & 1);
+    }
     // the particle chain holds register space the band kernel's large CTAs need (measured: the band
     // part takes 115 us beside the bounce-back kernel alone, 190 us beside the chain): the chain
     // starts after the band's part and still has the whole one-step kernel to hide under
@@ -743,7 +757,7 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     }
   }
   if (h->np > 0 && fork) cudaStreamWaitEvent(S0, h->ev_bb, 0);
-  const int lattice_mode = banded ? ((phase & 1) ? 2 : 1) : 0;
+  const int lattice_mode = !banded ? 0 : (h->band3 ? (phase % 3 == 0 ? 3 : 2) : ((phase & 1) ? 2 : 1));
   if (fork || h->np == 0) {
     Timed tm(h, K_STREAM_COLLIDE, S0);
     launch_stream_collide(h, lattice_mode, band_src);
@@ -821,7 +835,8 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
   if (e == cudaSuccess) {
     if (h->chain != h->stream) h->cap_nodes = &chain_nodes;
     join_in(h);
-    for (int s = 0; s < steps; ++s) enqueue_step(h, banded ? s % 4 : -1, s == 0);
+    h->band3 = banded == 3 ? 1 : 0;   // (the unit's schedule: plan margins, band kernel, cover's safety net)
+    for (int s = 0; s < steps; ++s) enqueue_step(h, banded ? s % (h->band3 ? 6 : 4) : -1, s == 0);
     join_out(h);
     h->cap_nodes = nullptr;
     e = cudaStreamEndCapture(h->cap_stream, &graph);
@@ -880,15 +895,18 @@ static lbm::StepGraph* step_graph(lbm* h, int steps, int banded) {
 // band that shrinks faster than the margin is caught by the one-step kernel's row loop.
 static int plan_call(lbm* h, int nsteps, bool* band_ok_out) {
   bool band_ok = h->np > 0 && h->band_on && h->two_step_ok && nsteps >= LBM_BAND_MIN_STEPS;
+  h->band3 = h->want3 = 0;
   if (band_ok) {
     h->band_cap = h->ny;
     h->band_orient = 0;                // under or above the suspension: whichever band is larger
+    h->band3 = h->want3 = h->band_steps >= 3 ? 1 : 0;   // (planned with the wider margins; dropped below for a band above)
     launch_band_plan(h, h->stream);
     CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaStreamSynchronize(h->stream));
     const int q0 = h->status_host[1];                         // > 0: rows [0, q0); < 0: rows [-q0, ny)
     const int rows0 = q0 > 0 ? q0 : (q0 < 0 ? h->ny + q0 : 0);  // rows of the band
     // a band of less than 2^18 nodes costs more in launches than it saves in traffic (config 0)
+    if (q0 <= 0) h->band3 = h->want3 = 0;   // three steps per pass only in a band under the suspension
     if (rows0 <= 0 || (h->band_on < 2 && (long long)rows0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
     else {
       h->band_orient = q0 > 0 ? 1 : -1;                       // fixed for this call: the grids are sized for it
@@ -897,12 +915,25 @@ static int plan_call(lbm* h, int nsteps, bool* band_ok_out) {
       h->band_cap = std::min(h->ny, ((rows0 + 8 + 15) / 16) * 16);
     }
   }
+  if (!band_ok) h->band3 = h->want3 = 0;
   *band_ok_out = band_ok;
   return LBM_OK;
 }
 
 // how many steps the next graph launch of a call with `left` steps to go covers, and in which schedule
-static int graph_unit(int left, bool band_ok, int* banded) {
+// With the three-step band (h->want3) a period is six steps -- units of 12 and 6, `banded` = 3 --
+// and a remainder of four is a period of the two-step band (`banded` = 1): every even number of
+// steps >= 4 is a sum of sixes and fours, so only a unit that would leave exactly two steps is
+// passed over (20 = 12 + 4 + 4, 14 = 6 + 4 + 4).
+static int graph_unit(const lbm* h, int left, bool band_ok, int* banded) {
+  if (band_ok && h->want3) {
+    const int even = left & ~1;
+    if (even >= 12 && even - 12 != 2) { *banded = 3; return 12; }
+    if (even >= 6 && even - 6 != 2) { *banded = 3; return 6; }
+    if (even >= 4) { *banded = 1; return 4; }
+    *banded = 0;
+    return 2;
+  }
   *banded = (band_ok && left >= 4) ? 1 : 0;
   return left >= LBM_GRAPH_STEPS ? LBM_GRAPH_STEPS : (*banded ? 4 : 2);
 }
@@ -922,7 +953,7 @@ int lbm_prepare(lbm_t* h, int nsteps) {
     // every unit of a call is an even number of steps, so all of them start in the current phase
     for (int s = 0; nsteps - s >= 2;) {
       int banded = 0;
-      const int unit = graph_unit(nsteps - s, band_ok, &banded);
+      const int unit = graph_unit(h, nsteps - s, band_ok, &banded);
       lbm::StepGraph* g = step_graph(h, unit, banded);
       if (!g) break;
       cudaGraphUpload(g->exec, h->stream);
@@ -954,7 +985,7 @@ int lbm_step(lbm_t* h, int nsteps) {
   if (h->np > 0 && h->use_graph && !h->prof_on) {
     while (nsteps - s >= 2) {
       int banded = 0;
-      const int unit = graph_unit(nsteps - s, band_ok, &banded);
+      const int unit = graph_unit(h, nsteps - s, band_ok, &banded);
       lbm::StepGraph* g = step_graph(h, unit, banded);
       if (!g) break;
       CUDA_OK(h, cudaGraphLaunch(g->exec, h->stream));
@@ -965,7 +996,6 @@ int lbm_step(lbm_t* h, int nsteps) {
   }
   if (s < nsteps) join_in(h);
   const bool direct = s < nsteps;
-  int direct_periods = 0;   // a band plan serves two periods
   while (s < nsteps) {
     if (h->np == 0 && h->two_step >= 2 && nsteps - s >= 3) {
       // particle-free lattice: three time steps per pass
@@ -990,11 +1020,16 @@ int lbm_step(lbm_t* h, int nsteps) {
       continue;
     }
     if (band_ok && nsteps - s >= 4) {
-      for (int ph = 0; ph < 4; ++ph) enqueue_step(h, ph, (direct_periods & 1) == 0);
-      ++direct_periods;
-      h->steps_done += 4;
-      s += 4;
-      continue;
+      // direct launches of the unit a graph would replay (same steps, same plans, same kernels)
+      int banded = 0;
+      const int unit = graph_unit(h, nsteps - s, band_ok, &banded);
+      if (banded) {
+        h->band3 = banded == 3 ? 1 : 0;
+        for (int k = 0; k < unit; ++k) enqueue_step(h, k % (h->band3 ? 6 : 4), k == 0);
+        h->steps_done += unit;
+        s += unit;
+        continue;
+      }
     }
     enqueue_step(h, -1);
     h->steps_done++;
@@ -1250,6 +1285,13 @@ int lbm_set_graph(lbm_t* h, int on) {
 int lbm_set_two_step(lbm_t* h, int on) {
   if (!h) return LBM_E_ARG;
   h->two_step = (on && h->two_step_ok) ? (on >= 3 ? 2 : 1) : 0;   // on: steps per pass (1 = 2: two)
+  return LBM_OK;
+}
+
+int lbm_set_band_steps(lbm_t* h, int steps) {
+  if (!h) return LBM_E_ARG;
+  if (steps != 2 && steps != 3) return fail(h, LBM_E_ARG, "lbm_set_band_steps: 2 or 3");
+  h->band_steps = steps;
   return LBM_OK;
 }
 

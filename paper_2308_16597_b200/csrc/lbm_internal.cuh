@@ -157,6 +157,9 @@ struct lbm {
   int band_live;             // the step being enqueued belongs to a banded period (k_cover checks the margin)
   int band_cap;              // most rows the band may have in this call (sizes the band kernel's grid)
   int band_on;               // lbm_set_band / LBM_BAND: use the banded schedule where it applies
+  int band_steps;            // lbm_set_band_steps / LBM_BAND_STEPS: 2 or 3 time steps per pass in a band under the suspension
+  int want3;                 // this call may use periods of six steps (band under the suspension, band_steps == 3)
+  int band3;                 // the unit being enqueued is such a period: the band advances three steps per pass
   cudaEvent_t ev_p2;         // the band kernel's part of a step has been issued (the particle chain follows it)
   cudaEvent_t ev_plan;       // the band plan of a period has been issued (the caller's stream follows it)
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
@@ -239,6 +242,7 @@ int stream_collide_tma_setup(lbm* h);      // tensor maps for the TMA-fed three-
 void launch_stream_collide_3step_tma(lbm* h);  // on h->stream; particle-free closed cavities, needs h->tma_ok
 void launch_stream_collide_band(lbm* h, const double* src_band, const double* src_top, double* dst_band,
                                 int nparts, int part);   // on h->stream; rows [0, *h->band)
+void launch_stream_collide_band3(lbm* h, double* src, double* dst, int nparts, int part);   // on h->stream; rows [0, *h->band), three steps per pass
 int stream_collide_configure();            // kernel attributes (0 = ok)
 void launch_init_collide(lbm* h, double* dst);   // dst = h->A (in place) or scratch
 void launch_set_temperature(lbm* h, const double* T_dev_dense);
@@ -252,7 +256,7 @@ int launch_macroscopic_static(lbm* h, double** fields4);   // into the library's
 void launch_build_links(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
 void launch_move(lbm* h, cudaStream_t st, bool pdl);   // integrator + uncover, buffer cur -> cur ^ 1
 int particles_configure(lbm* h);           // per-handle kernel attributes (0 = ok)
-void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);
+void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl);   // (band margin check: 4 rows, 5 with h->band3)
 void launch_band_plan(lbm* h, cudaStream_t st);
 void launch_slab_forces_out(lbm* h);   // owned particles' F, T_z -> h->force_buf (zeros for the others)
 void launch_slab_forces_in(lbm* h);    // h->force_buf (combined over the slabs) -> F, T_z

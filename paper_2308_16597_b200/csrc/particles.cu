@@ -671,7 +671,7 @@ __global__ void __launch_bounds__(PT_MAX, 12)
 k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__ flag,
         int* __restrict__ owner, double cell, int ncx, int ncy, int* __restrict__ cell_count,
         int* __restrict__ cell_items, int* __restrict__ status, const int* __restrict__ bandp,
-        int early, const LbmConst c) {
+        int guard, int early, const LbmConst c) {
   if (early) pdl_launch_dependents();
   pdl_wait();
   const int Q = *bandp;   // > 0: band [0, Q); < 0: band [-Q, ny)
@@ -681,7 +681,7 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
   if (threadIdx.x == 0) {
     // safety net of the two-step band: no solid node within 4 rows of it (k_band_plan's margins
     // make this unreachable for any |U|, dU the method is stable at)
-    if (Q > 0 && (int)floor(yn - Sn.r) < Q + 4) atomicOr(status, ST_BAND_REACHED);
+    if (Q > 0 && (int)floor(yn - Sn.r) < Q + guard) atomicOr(status, ST_BAND_REACHED);
     if (Q < 0 && (int)ceil(yn + Sn.r) > -Q - 5) atomicOr(status, ST_BAND_REACHED);
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
     ci = min(max(ci, 0), ncx - 1);
@@ -718,6 +718,9 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
 // fall in BAND_PERIOD steps (its speed now, two nodes for its acceleration -- the stiffest
 // repulsion of Eq. 15 gives 32 a = 1.7 -- one in reserve); k_cover checks it every step.
 // A band of fewer than BAND_MIN rows is not worth its seam: Q = 0 (no band).  One CTA.
+// Three steps per pass (h->band3; bands under the suspension only): the band kernel reads one more
+// row above Q and a plan serves two periods of SIX steps: period 12, margin 8 instead of 8 and 7,
+// and k_cover's safety net moves up by one row.
 constexpr int BAND_PERIOD = 8;
 constexpr int BAND_MIN = 28;
 // orient: +1 only a band under the suspension (rows [0, Q), band[0] = Q), -1 only a band above
@@ -725,13 +728,14 @@ constexpr int BAND_MIN = 28;
 // larger (the plan at the start of a call; the orientation then stays fixed for the call, because
 // the grids are sized for it).  qcap: most rows the band may have (the band kernel's grid).
 __global__ void __launch_bounds__(1024)
-k_band_plan(ParticleArrays pa, int cur, int np, int ny, int orient, int qcap, int* __restrict__ band) {
+k_band_plan(ParticleArrays pa, int cur, int np, int ny, int orient, int qcap, int period, int margin,
+            int* __restrict__ band) {
   __shared__ double s_min[32], s_max[32];
   double low = 1.0e300, high = -1.0e300;
   for (int p = threadIdx.x; p < np; p += blockDim.x) {
     const double uy = pa.fixed[p] ? 0.0 : pa.uy[cur][p];
-    low = fmin(low, pa.y[cur][p] - pa.r[p] - (double)BAND_PERIOD * fmax(-uy, 0.0));
-    high = fmax(high, pa.y[cur][p] + pa.r[p] + (double)BAND_PERIOD * fmax(uy, 0.0));
+    low = fmin(low, pa.y[cur][p] - pa.r[p] - (double)period * fmax(-uy, 0.0));
+    high = fmax(high, pa.y[cur][p] + pa.r[p] + (double)period * fmax(uy, 0.0));
   }
 #pragma unroll
   for (int d = 16; d >= 1; d >>= 1) {
@@ -751,11 +755,11 @@ k_band_plan(ParticleArrays pa, int cur, int np, int ny, int orient, int qcap, in
     int below = 0, above = 0;   // rows of the two candidate bands
     int Qb = 0, Qt = ny;
     if (low == low && low < 1.0e9 && low > -1.0e9) {
-      Qb = min((int)floor(low) - 7, ny - 8);
+      Qb = min((int)floor(low) - margin, ny - 8);
       below = Qb >= BAND_MIN ? min(Qb, qcap) : 0;
     }
     if (high == high && high < 1.0e9 && high > -1.0e9) {
-      Qt = max((int)ceil(high) + 7, 8);
+      Qt = max((int)ceil(high) + margin, 8);
       above = ny - Qt >= BAND_MIN ? min(ny - Qt, qcap) : 0;
     }
     if (orient > 0) above = 0;
@@ -877,14 +881,15 @@ void launch_cover(lbm* h, int which_buffer, cudaStream_t st, bool pdl) {
   launch_k(h->n_ell ? k_cover<true> : k_cover<false>, dim3(chain_grid(h, h->np, st)), dim3(chain_threads(h, h->np, st)), 0, st, pdl,
            h->pa, which_buffer, h->np, h->primed ? 0 : 1, h->flag, h->owner, h->cell, h->ncx, h->ncy,
            h->cell_count[which_buffer], h->cell_items[which_buffer], h->status_dev,
-           (const int*)(h->band_live ? h->band : h->band + 1), chain_early(h, st), h->C);
+           (const int*)(h->band_live ? h->band : h->band + 1), h->band3 ? 5 : 4, chain_early(h, st), h->C);
 }
 
 // rows [0, h->band[0]) of the next BAND_PERIOD steps go to the two-step kernel (positions of
 // buffer h->cur); a plain launch: it starts after everything before it in `st` has completed
 void launch_band_plan(lbm* h, cudaStream_t st) {
   h->launches++;
-  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_orient, h->band_cap, h->band);
+  k_band_plan<<<1, 1024, 0, st>>>(h->pa, h->cur, h->np, h->ny, h->band_orient, h->band_cap,
+                                  h->band3 ? 12 : BAND_PERIOD, h->band3 ? 8 : 7, h->band);
 }
 
 void launch_slab_forces_out(lbm* h) {

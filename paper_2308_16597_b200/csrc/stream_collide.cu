@@ -452,8 +452,22 @@ __device__ __forceinline__ void pull_tile3(const double* s_pop, int tid, int iw,
   }
 }
 
-__global__ void __launch_bounds__(T3_THREADS)
-k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, const LbmConst c) {
+//
+// BAND: the kernel advances the rows
+// [0, Q), Q = *bandp, of a lattice WITH particles from the period's state t (every row of A at time
+// t) to t+3 in B.  The rows Q .. Q+2 it needs as halo are ordinary fluid rows of the same copy
+// (three steps per pass keep the band and the rows above it in the same copy at the start of every
+// half period, so there is no seam inside this kernel): level 1 covers the rows up to Q+1, level 2
+// up to Q, level 3 stores the rows below Q.  What the one-step kernel above the band needs at the
+// intermediate times -- row Q-1 at t+1 and at t+2 -- is written by the tile that owns row Q-1 into
+// the spare row ny: level 1's into B's (read by the second step of the half period), level 2's
+// into A's (read by the third).  The tile rows are dealt to the three steps FROM THE TOP (part 0 =
+// the top third): the rows >= Q of A are overwritten by the second step's one-step kernel, which
+// runs after the parts 0 and 1 of the pass (stream order); part 2 only reads rows below Q.
+template <bool BAND>
+__global__ void __launch_bounds__(T3_THREADS, 2)
+k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, double* __restrict__ Aspare,
+                       const int* __restrict__ bandp, int nparts, int part, const LbmConst c) {
   extern __shared__ double s_pop[];   // [14][T3_H][T3_W], then the row barriers [T3_H][2]
   unsigned long long* const rb = reinterpret_cast<unsigned long long*>(s_pop + 14 * T3_THREADS);
   pdl_launch_dependents();
@@ -462,12 +476,25 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
   pdl_wait();
   const int tid = threadIdx.x;
   const int tx = tid % T3_W, ty = tid / T3_W;
-  const int i = blockIdx.x * T3_X - 2 + tx, j = blockIdx.y * T3_Y - 2 + ty;
+  int Q = c.ny, tile_row = blockIdx.y;
+  if (BAND) {
+    const int Qs = *bandp;
+    if (Qs <= 0) return;              // no band (a band above the suspension has its own schedule)
+    Q = min(Qs, c.ny);
+    const int ntr = (Q + T3_Y - 1) / T3_Y;
+    const int per_part = (ntr + nparts - 1) / nparts;
+    if ((int)blockIdx.y >= per_part) return;
+    tile_row = ntr - (part + 1) * per_part + (int)blockIdx.y;
+    if (tile_row < 0) return;
+  }
+  const int i = blockIdx.x * T3_X - 2 + tx, j = tile_row * T3_Y - 2 + ty;
+  // the node of row Q-1 in the tile that owns it hands its levels 1 and 2 to the rows above
+  const bool hand = BAND && j == Q - 1 && ty >= 2 && ty <= T3_H - 3 && tx >= 2 && tx <= T3_W - 3 && i >= 0 && i < c.nx;
   // periodic x: the columns -2, -1 and nx, nx+1 are images of nx-2, nx-1 and 0, 1
   int iw = i;
   if (c.periodic_x) iw = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i);
   const bool col1 = c.periodic_x ? (i >= -2 && i <= c.nx + 1 && iw >= 0 && iw < c.nx) : (i >= 0 && i < c.nx);
-  const bool ex1 = col1 && j >= 0 && j < c.ny;
+  const bool ex1 = col1 && j >= 0 && j < c.ny && (!BAND || j <= Q + 1);
   double f[9], g[5];
   // level 1: t -> t+1, from global memory
   if (ex1) {
@@ -477,6 +504,7 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
     for (int k = 0; k < 9; ++k) s_pop[k * T3_THREADS + tid] = f[k];
 #pragma unroll
     for (int k = 0; k < 5; ++k) s_pop[(9 + k) * T3_THREADS + tid] = g[k];
+    if (hand) store_node_at(B, c.ps, c.px, i, c.ny, f, g);
   }
   // No CTA-wide barriers: a warp is a tile row and hands over to its two neighbour rows only
   // (phase 1: level 1 written; 2: level 1 pulled; 3: level 2 written)
@@ -484,12 +512,13 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
   row_wait(rb, ty, 1, T3_H);
   // level 2: t+1 -> t+2 on the tile dilated by one node, written back in place
   const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2 &&
-                   (!c.periodic_x || (i >= -1 && i <= c.nx));
+                   (!c.periodic_x || (i >= -1 && i <= c.nx)) && (!BAND || j <= Q);
   if (ex2) pull_tile3(s_pop, tid, iw, j, c, f, g);
   row_publish(rb, ty, 2);
   if (ex2) mrt_collide(f, g, c);
   row_wait(rb, ty, 2, T3_H);          // the neighbour rows have read this row's level-1 values
   if (ex2) {
+    if (hand) store_node_at(Aspare, c.ps, c.px, i, c.ny, f, g);
 #pragma unroll
     for (int k = 0; k < 9; ++k) s_pop[k * T3_THREADS + tid] = f[k];
 #pragma unroll
@@ -498,7 +527,7 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, con
   row_publish(rb, ty, 3);
   row_wait(rb, ty, 3, T3_H);
   // level 3: t+2 -> t+3 on the tile's own nodes, to global memory
-  if (!(ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3 && i >= 0 && i < c.nx)) return;
+  if (!(ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3 && i >= 0 && i < c.nx && (!BAND || j < Q))) return;
   pull_tile3(s_pop, tid, iw, j, c, f, g);
   mrt_collide(f, g, c);
   store_node(B, c, i, j, f, g);
@@ -829,14 +858,17 @@ inline dim3 grid_rows(int n, int ny, int threads) { return dim3((n + threads - 1
 
 // band == 0: the plain step (every row).  band == 1 / 2: first / second step of a pair of the
 // banded schedule (lbm_capi.cu): rows from *h->band - 1 resp. *h->band up; low = the band's copy
-// (first step only).
+// (first step only).  band == 3: first step of a half period of the three-step band (rows from
+// *h->band up, the band's rows read in place from low = h->A; the later steps of the half period
+// are band == 2: row Q-1 from the spare row).
 void launch_stream_collide(lbm* h, int band, const double* low) {
   h->launches++;
   // banded steps: one CTA row per lattice row above the band as the host last saw it
   // (h->band_hint, 0 = unknown); the kernel's row loop covers whatever the band has lost since
   const int rows = band ? h->band_l1_rows : h->row1 - h->row0;
   launch_k(k_stream_collide, grid_rows(h->px, rows, SC_THREADS), dim3(SC_THREADS), 0, h->stream, h->use_pdl != 0,
-           (const double*)h->A, h->B, (const unsigned char*)h->flag, band == 1 ? low : (const double*)nullptr,
+           (const double*)h->A, h->B, (const unsigned char*)h->flag,
+           (band == 1 || band == 3) ? low : (const double*)nullptr,
            (const int*)(band ? h->band : h->band + 1), band == 1 ? -1 : 0, h->row0, h->row1, h->C);
 }
 
@@ -849,7 +881,9 @@ void launch_stream_collide_slab(lbm* h, const HaloPush& hp) {
 int stream_collide_configure() {
   return (cudaFuncSetAttribute(k_stream_collide_2step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                TB_SMEM) == cudaSuccess &&
-          cudaFuncSetAttribute(k_stream_collide_3step, cudaFuncAttributeMaxDynamicSharedMemorySize,
+          cudaFuncSetAttribute(k_stream_collide_3step<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               T3_SMEM) == cudaSuccess &&
+          cudaFuncSetAttribute(k_stream_collide_3step<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                T3_SMEM) == cudaSuccess) ? 0 : -1;
 }
 
@@ -942,8 +976,19 @@ void launch_stream_collide_3step_tma(lbm* h) {
 void launch_stream_collide_3step(lbm* h) {
   h->launches++;
   const dim3 grid((h->nx + T3_X - 1) / T3_X, (h->ny + T3_Y - 1) / T3_Y);
-  launch_k(k_stream_collide_3step, grid, dim3(T3_THREADS), T3_SMEM, h->stream, h->use_pdl != 0,
-           (const double*)h->A, h->B, h->C);
+  launch_k(k_stream_collide_3step<false>, grid, dim3(T3_THREADS), T3_SMEM, h->stream, h->use_pdl != 0,
+           (const double*)h->A, h->B, (double*)nullptr, (const int*)nullptr, 1, 0, h->C);
+}
+
+// the band rows [0, *h->band) of a lattice with particles, three steps per pass: the part-th of
+// nparts shares of the tile rows, counted from the top; src: the copy that holds every row at the
+// start of the half period, dst: the other one
+void launch_stream_collide_band3(lbm* h, double* src, double* dst, int nparts, int part) {
+  h->launches++;
+  const int tile_rows = (std::min(h->band_cap, h->ny) + T3_Y - 1) / T3_Y + 1;
+  const dim3 grid((h->nx + T3_X - 1) / T3_X, (tile_rows + nparts - 1) / nparts);
+  launch_k(k_stream_collide_3step<true>, grid, dim3(T3_THREADS), T3_SMEM, h->stream, h->use_pdl != 0,
+           (const double*)src, dst, src, (const int*)h->band, nparts, part, h->C);
 }
 
 // particle-free lattice: every row, A -> B

@@ -579,11 +579,14 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
     ref = gpu.Simulation.from_workload(w)
     ref.set_band(False)
     ref.set_graph(False)
-    sims = [gpu.Simulation.from_workload(w) for _ in range(3)]
+    sims = [gpu.Simulation.from_workload(w) for _ in range(5)]
     for s_ in sims:
         s_.set_band(2)                               # every band, however small the lattice
     sims[1].set_graph(False)                         # direct launches (the profiling path)
     sims[2].set_overlap(False)                       # one stream
+    sims[3].set_band_steps(2)                        # periods of four steps, two steps per pass
+    sims[4].set_band_steps(2)                        # (the default is three: periods of six)
+    sims[4].set_graph(False)
     q_seen = []
     for nst in (1, 4, 8, 3, 29, 64, 402, 7, 1500):
         ref.step(nst)
@@ -607,16 +610,18 @@ def test_two_step_band_equals_plain_schedule_bitwise(gpu, wl):
                  uy=np.array([-0.05, 0.0]), omega=np.array([0.0, 0.0]),
                  fixed=np.array([0, 1], dtype=np.uint8))
     w2 = wl.Workload("band_vanishes", 120, 150, p, 1, 1, particles=parts)
-    a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
-    a.set_band(2)
-    b.set_band(False)
-    qs = []
-    for nst in (16, 16, 24, 40, 200):         # (calls shorter than 16 steps never use the band)
-        a.step(nst)
-        b.step(nst)
-        assert_same_bits(a, b)
-        qs.append(a.band_rows())
-    assert qs[0] >= 28 and qs[-1] == 0, qs
+    for band_steps in (3, 2):
+        a, b = gpu.Simulation.from_workload(w2), gpu.Simulation.from_workload(w2)
+        a.set_band(2)
+        a.set_band_steps(band_steps)
+        b.set_band(False)
+        qs = []
+        for nst in (16, 16, 24, 40, 200):         # (calls shorter than 16 steps never use the band)
+            a.step(nst)
+            b.step(nst)
+            assert_same_bits(a, b)
+            qs.append(a.band_rows())
+        assert qs[0] >= 28 and qs[-1] == 0, (band_steps, qs)
 
 
 def test_two_step_band_above_a_settled_suspension_equals_plain_schedule_bitwise(gpu, ob, wl):
