@@ -406,8 +406,8 @@ k_stream_collide_2step(const double* __restrict__ Aband, const double* __restric
 // of T3_W x T3_H threads owns a T3_X x T3_Y tile of output nodes and its two-node halo.  Level 1:
 // every thread pulls its node of the halo'd tile from A and collides (state t+1) into its slot of
 // ONE shared buffer.  Level 2: the threads of the tile dilated by one node pull from their
-// neighbours' slots, and -- after a barrier, when nobody reads level 1 any more -- write their
-// collided result (t+2) back IN PLACE.  Level 3: the tile's own nodes pull level 2, collide and
+// neighbours' slots, and -- once the neighbour rows have pulled too, so that nobody reads those
+// level-1 values any more -- write their collided result (t+2) back IN PLACE.  Level 3: the tile's own nodes pull level 2, collide and
 // store f+(x, t+3) to B.  Per three updates a node costs (T3_W+2)(T3_H+2)/(T3_X T3_Y) = 1.82 reads
 // and one write of its 112 B: 105 B per update requested (less from DRAM: the halo re-reads hit
 // L2) against 137 B for two steps per pass and 224 B for one, for 1.26 collisions per update
@@ -544,14 +544,18 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
 // rows and columns outside the lattice are zero-filled by the copy engine and never used (walls as
 // in pull_boundary, the node's own slot standing in).  No thread computes a global load address.
 //
-// The 1024 threads are two groups of 512 (named barriers), each of which takes every other tile of
-// the CTA's sequence and runs the three levels of k_stream_collide_3step on its image IN PLACE:
-// pull from the neighbours' slots, barrier, collide, write back to the own slot, barrier -- level 1
-// on the 32 x 16 nodes of the tile dilated by two, level 2 on 30 x 14, level 3 on 28 x 12 and from
-// registers to B.  When a group has pulled level 3 its image is free: the group's warp 0 collects
-// the other warps' arrivals (bar.arrive / bar.sync) and one lane issues the copies for the CTA's
-// tile after next but one into it, which land while both groups compute -- the loads of tile m + 3
-// overlap the arithmetic of tiles m + 1 and m + 2 instead of alternating with it.
+// The 1024 threads are two groups of 512, each of which takes every other tile of the CTA's
+// sequence and runs the three levels of k_stream_collide_3step on its image IN PLACE: pull from
+// the neighbours' slots, (neighbours have pulled) collide, write back to the own slot, (neighbours
+// have written) next level -- level 1 on the 32 x 16 nodes of the tile dilated by two, level 2 on
+// 30 x 14, level 3 on 28 x 12 and from registers to B.  ROWSYNC (the default): the hand-over in
+// brackets is per row -- a warp owns a tile row and waits for its two neighbour rows' mbarriers
+// (row_publish / row_wait above); otherwise it is a named barrier of the whole group.  When a
+// group has pulled level 3 its image is free: the group's warp 0 collects the other warps'
+// arrivals (an mbarrier per stage with ROWSYNC, where the warps of a group may be tiles apart;
+// bar.arrive / bar.sync otherwise) and one lane issues the copies for the CTA's tile after next but
+// one into it, which land while both groups compute -- the loads of tile m + 3 overlap the
+// arithmetic of tiles m + 1 and m + 2 instead of alternating with it.
 // Same pull, same collision, same order: bit-identical to three passes of the one-step kernel.
 constexpr int TP_IW = T3_W + 4, TP_IH = T3_H + 2;       // 36 x 18 node image
 constexpr int TP_PLANE = TP_IW * TP_IH;
@@ -618,10 +622,10 @@ __device__ __forceinline__ void put_img(double* img, int s, const double (&f)[9]
 
 // Row-wise hand-over inside a group (ROWSYNC): warp w of a group owns row w of the dilated tile,
 // and a level's pull of row r reads only rows r-1, r, r+1 of the level below, so instead of four
-// group-wide barriers per tile each warp publishes how far it has come (a counter per row in
-// shared memory, st.release / ld.acquire at CTA scope) and waits for its two neighbours only:
-// before writing its row back in place, that they have pulled; before pulling the next level,
-// that they have written.  Neighbouring rows stay within one phase of each other, the sixteen
+// group-wide barriers per tile each warp publishes how far it has come (two mbarriers per row,
+// row_publish / row_wait; plain counters with st.release / ld.acquire cost a MEMBAR per store
+// and lost) and waits for its two neighbours only: before writing its row back in place, that
+// they have pulled; before pulling the next level, that they have written.  Neighbouring rows stay within one phase of each other, the sixteen
 // warps of a group spread over the phases, and shared-memory phases of some warps run under the
 // fp64 phases of others.
 template <bool ROWSYNC>
