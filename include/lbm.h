@@ -113,7 +113,7 @@ int lbm_add_ellipses(lbm_t* h, int n, const double* x, const double* y, const do
 int lbm_step(lbm_t* h, int nsteps);
 
 /* Optional set-up call: does everything a following lbm_step(h, nsteps) would do before its first
- * time step -- collides the initial state, builds the first links, plans the two-step band and
+ * time step -- collides the initial state, builds the first links, plans the band and
  * captures, instantiates and uploads the CUDA graphs that call will replay -- without advancing
  * time, so that a short timed lbm_step (tens of steps) does not pay for graph instantiation (about
  * a millisecond per graph; like building an FFT plan before the loop).  The graphs are keyed by
@@ -182,14 +182,15 @@ int lbm_set_band_steps(lbm_t* h, int steps);
  * Errors: LBM_E_STATE if on != 0 and the handle has no tensor maps. */
 int lbm_set_tma(lbm_t* h, int on);
 
-/* on = 1 (default; the environment variable LBM_BAND = 0 / 1 / 2 sets the default): lattices WITH particles also use the
- * two-steps-per-pass kernel, on the particle-free rows [0, Q) below the lowest particle (SURVEY
- * 8(f)-4), in lbm_step calls of at least 16
- * steps (such a call plans the band once on entry to size its grids: one more synchronisation).
- * In periods of four time steps a device kernel picks Q from the particle positions and speeds (far enough below the lowest
- * particle that no link or refill stencil reaches the band within the period; fewer than 28 free
- * rows: no band), the band is advanced t -> t+2 -> t+4 by the two-step kernel while the rows
- * above it take four ordinary steps, the two meeting in one row that is computed by both.  The
+/* on = 1 (default; the environment variable LBM_BAND = 0 / 1 / 2 sets the default): lattices WITH
+ * particles also use a multi-step kernel, on the particle-free rows [0, Q) below the lowest
+ * particle (DESIGN.md sections 6a, 6b), in lbm_step calls of at least 16 steps (such
+ * a call plans the band once on entry to size its grids: one more synchronisation).  In periods of
+ * six time steps (four with lbm_set_band_steps(h, 2)) a device kernel picks Q from the particle
+ * positions and speeds (far enough below the lowest particle that no link or refill stencil reaches
+ * the band within the period; fewer than 28 free rows: no band); the band is advanced t -> t+3 ->
+ * t+6 by the three-step kernel (t -> t+2 -> t+4 by the two-step kernel) while the rows above it
+ * take ordinary steps, reading the band's top row at the intermediate times from a spare row.  The
  * arithmetic per node and step is unchanged: results are identical bit for bit to on = 0.
  * on = 1 uses a band only if it holds at least 2^18 nodes (below that its extra launches cost more
  * than the traffic it saves); on = 2 uses every band of at least 28 rows (the tests).
