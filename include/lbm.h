@@ -159,12 +159,12 @@ int lbm_set_graph(lbm_t* h, int on);
  * The arithmetic per node and step is the same in all three, so results are identical bit for bit. */
 int lbm_set_two_step(lbm_t* h, int on);
 
-/* Time steps per pass in a band UNDER the suspension (lbm_set_band): 3 (default; the environment
- * variable LBM_BAND_STEPS = 2 / 3 sets the default): periods of six steps, the band kernel
- * k_stream_collide_3step<BAND> advances the rows [0, Q) three steps per pass and hands row Q-1 at
- * the two intermediate times to the rows above through the spare row; 2: periods of four steps
- * with k_stream_collide_2step.  A band above a settled suspension always takes two steps per pass.
- * Identical results bit for bit.  Errors: LBM_E_ARG unless steps is 2 or 3. */
+/* Time steps per pass in a band (lbm_set_band): 3 (default; the environment variable
+ * LBM_BAND_STEPS = 2 / 3 sets the default): periods of six steps, the band kernel
+ * k_stream_collide_3step<BAND> advances the band's rows three steps per pass and hands its row next
+ * to the seam, at the two intermediate times, to the rows outside through the spare row; 2: periods
+ * of four steps with k_stream_collide_2step.  Identical results bit for bit.
+ * Errors: LBM_E_ARG unless steps is 2 or 3. */
 int lbm_set_band_steps(lbm_t* h, int steps);
 
 /* Which kernel takes the three-steps-per-pass passes of a particle-free lattice.

@@ -899,14 +899,13 @@ static int plan_call(lbm* h, int nsteps, bool* band_ok_out) {
   if (band_ok) {
     h->band_cap = h->ny;
     h->band_orient = 0;                // under or above the suspension: whichever band is larger
-    h->band3 = h->want3 = h->band_steps >= 3 ? 1 : 0;   // (planned with the wider margins; dropped below for a band above)
+    h->band3 = h->want3 = h->band_steps >= 3 ? 1 : 0;   // (the call-start plan then takes the wider margins)
     launch_band_plan(h, h->stream);
     CUDA_OK(h, cudaMemcpyAsync(h->status_host + 1, h->band, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CUDA_OK(h, cudaStreamSynchronize(h->stream));
     const int q0 = h->status_host[1];                         // > 0: rows [0, q0); < 0: rows [-q0, ny)
     const int rows0 = q0 > 0 ? q0 : (q0 < 0 ? h->ny + q0 : 0);  // rows of the band
     // a band of less than 2^18 nodes costs more in launches than it saves in traffic (config 0)
-    if (q0 <= 0) h->band3 = h->want3 = 0;   // three steps per pass only in a band under the suspension
     if (rows0 <= 0 || (h->band_on < 2 && (long long)rows0 * h->nx < LBM_BAND_MIN_NODES)) band_ok = false;
     else {
       h->band_orient = q0 > 0 ? 1 : -1;                       // fixed for this call: the grids are sized for it

@@ -682,7 +682,7 @@ k_cover(ParticleArrays pa, int buf, int np, int all, unsigned char* __restrict__
     // safety net of the two-step band: no solid node within 4 rows of it (k_band_plan's margins
     // make this unreachable for any |U|, dU the method is stable at)
     if (Q > 0 && (int)floor(yn - Sn.r) < Q + guard) atomicOr(status, ST_BAND_REACHED);
-    if (Q < 0 && (int)ceil(yn + Sn.r) > -Q - 5) atomicOr(status, ST_BAND_REACHED);
+    if (Q < 0 && (int)ceil(yn + Sn.r) > -Q - guard - 1) atomicOr(status, ST_BAND_REACHED);
     int ci = (int)floor(xn / cell), cj = (int)floor(yn / cell);
     ci = min(max(ci, 0), ncx - 1);
     cj = min(max(cj, 0), ncy - 1);

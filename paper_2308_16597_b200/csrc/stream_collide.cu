@@ -476,25 +476,37 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
   pdl_wait();
   const int tid = threadIdx.x;
   const int tx = tid % T3_W, ty = tid / T3_W;
+  // A band under the lid (Qs < 0: rows [Q, ny), Q = -Qs, above a settled bed) is the same scheme
+  // mirrored: halo rows Q-3 .. Q-1, row Q handed over, the parts dealt from the bottom.
   int Q = c.ny, tile_row = blockIdx.y;
+  bool upper = false;
   if (BAND) {
     const int Qs = *bandp;
-    if (Qs <= 0) return;              // no band (a band above the suspension has its own schedule)
-    Q = min(Qs, c.ny);
-    const int ntr = (Q + T3_Y - 1) / T3_Y;
+    if (Qs == 0) return;
+    upper = Qs < 0;
+    Q = upper ? -Qs : min(Qs, c.ny);
+    const int tr0 = upper ? Q / T3_Y : 0;            // first tile row that holds band rows
+    const int ntr = (upper ? (c.ny + T3_Y - 1) / T3_Y : (Q + T3_Y - 1) / T3_Y) - tr0;
     const int per_part = (ntr + nparts - 1) / nparts;
     if ((int)blockIdx.y >= per_part) return;
-    tile_row = ntr - (part + 1) * per_part + (int)blockIdx.y;
-    if (tile_row < 0) return;
+    tile_row = upper ? tr0 + part * per_part + (int)blockIdx.y
+                     : tr0 + ntr - (part + 1) * per_part + (int)blockIdx.y;
+    if (tile_row < tr0 || tile_row >= tr0 + ntr) return;
   }
   const int i = blockIdx.x * T3_X - 2 + tx, j = tile_row * T3_Y - 2 + ty;
-  // the node of row Q-1 in the tile that owns it hands its levels 1 and 2 to the rows above
-  const bool hand = BAND && j == Q - 1 && ty >= 2 && ty <= T3_H - 3 && tx >= 2 && tx <= T3_W - 3 && i >= 0 && i < c.nx;
+  // the band's row next to the seam, in the tile that owns it, hands its levels 1 and 2 to the
+  // rows outside the band
+  const bool hand = BAND && j == (upper ? Q : Q - 1) && ty >= 2 && ty <= T3_H - 3 && tx >= 2 && tx <= T3_W - 3 &&
+                    i >= 0 && i < c.nx;
+  // rows of the band's side that level 1 / 2 / 3 cover
+  const bool in1 = !BAND || (upper ? j >= Q - 2 : j <= Q + 1);
+  const bool in2 = !BAND || (upper ? j >= Q - 1 : j <= Q);
+  const bool in3 = !BAND || (upper ? j >= Q : j < Q);
   // periodic x: the columns -2, -1 and nx, nx+1 are images of nx-2, nx-1 and 0, 1
   int iw = i;
   if (c.periodic_x) iw = i < 0 ? i + c.nx : (i >= c.nx ? i - c.nx : i);
   const bool col1 = c.periodic_x ? (i >= -2 && i <= c.nx + 1 && iw >= 0 && iw < c.nx) : (i >= 0 && i < c.nx);
-  const bool ex1 = col1 && j >= 0 && j < c.ny && (!BAND || j <= Q + 1);
+  const bool ex1 = col1 && j >= 0 && j < c.ny && in1;
   double f[9], g[5];
   // level 1: t -> t+1, from global memory
   if (ex1) {
@@ -512,7 +524,7 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
   row_wait(rb, ty, 1, T3_H);
   // level 2: t+1 -> t+2 on the tile dilated by one node, written back in place
   const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2 &&
-                   (!c.periodic_x || (i >= -1 && i <= c.nx)) && (!BAND || j <= Q);
+                   (!c.periodic_x || (i >= -1 && i <= c.nx)) && in2;
   if (ex2) pull_tile3(s_pop, tid, iw, j, c, f, g);
   row_publish(rb, ty, 2);
   if (ex2) mrt_collide(f, g, c);
@@ -527,7 +539,7 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
   row_publish(rb, ty, 3);
   row_wait(rb, ty, 3, T3_H);
   // level 3: t+2 -> t+3 on the tile's own nodes, to global memory
-  if (!(ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3 && i >= 0 && i < c.nx && (!BAND || j < Q))) return;
+  if (!(ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3 && i >= 0 && i < c.nx && in3)) return;
   pull_tile3(s_pop, tid, iw, j, c, f, g);
   mrt_collide(f, g, c);
   store_node(B, c, i, j, f, g);

@@ -656,11 +656,12 @@ def test_two_step_band_above_a_settled_suspension_equals_plain_schedule_bitwise(
     ref = gpu.Simulation.from_workload(w)
     ref.set_band(False)
     ref.set_graph(False)
-    sims = [gpu.Simulation.from_workload(w) for _ in range(3)]
+    sims = [gpu.Simulation.from_workload(w) for _ in range(4)]
     for s_ in sims:
         s_.set_band(2)
     sims[1].set_graph(False)
     sims[2].set_overlap(False)
+    sims[3].set_band_steps(2)                                 # two steps per pass (the default is three)
     q_seen = []
     for nst in (16, 29, 64, 402, 7, 900):
         ref.step(nst)
