@@ -568,12 +568,14 @@ static int add_shapes(lbm_t* h, int n, const double* x, const double* y, const d
   // overlap test through a host cell grid (cell >= largest diameter): flat cells filled in particle
   // order (counting sort), each new particle tested against the earlier ones in its 3 x 3 cells
   {
-    const double cell = std::max(dmax, 1.0);
+    double cell = std::max(dmax, 1.0);
     double xlo = X[0], ylo = Y[0], xhi = X[0], yhi = Y[0];
     for (int k = 1; k < nt; ++k) {
       xlo = std::min(xlo, X[k]); xhi = std::max(xhi, X[k]);
       ylo = std::min(ylo, Y[k]); yhi = std::max(yhi, Y[k]);
     }
+    // (a few tiny particles far apart: coarser cells rather than a huge empty grid)
+    while ((std::floor((xhi - xlo) / cell) + 1.0) * (std::floor((yhi - ylo) / cell) + 1.0) > 16.0 * nt + 4096.0) cell *= 2.0;
     const int gx = (int)std::floor((xhi - xlo) / cell) + 1, gy = (int)std::floor((yhi - ylo) / cell) + 1;
     std::vector<int> ci(nt), cj(nt), start((size_t)gx * gy + 1, 0), order(nt);
     for (int k = 0; k < nt; ++k) {
