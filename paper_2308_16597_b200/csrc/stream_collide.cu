@@ -291,10 +291,13 @@ __device__ __forceinline__ void mbar_arrive(void* bar) {
 // complete [row][0], phases 2 and 4 [row][1], so that two completions of one barrier are always
 // separated by the neighbours' observation of the first (a row cannot publish phase p + 2 before
 // both neighbours have published p + 1, i.e. have seen p) and the parity wait stays unambiguous
-__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase) {
+// dep: a value the arrival must come after (an operand the instruction does not use: a collided
+// population, which depends on every value the thread pulled, so the warp's shared-memory reads
+// have completed when the arrival issues)
+__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase, double dep = 0.0) {
   __syncwarp();
   if ((threadIdx.x & 31) == 0)
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))) : "memory");
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))), "d"(dep) : "memory");
 }
 __device__ __forceinline__ void row_wait(unsigned long long* rb, int row, int phase, int rows) {
   const unsigned parity = (unsigned)((phase - 1) >> 1) & 1u;   // two completions per barrier and tile
@@ -525,9 +528,11 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
   // level 2: t+1 -> t+2 on the tile dilated by one node, written back in place
   const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2 &&
                    (!c.periodic_x || (i >= -1 && i <= c.nx)) && in2;
-  if (ex2) pull_tile3(s_pop, tid, iw, j, c, f, g);
-  row_publish(rb, ty, 2);
-  if (ex2) mrt_collide(f, g, c);
+  if (ex2) {
+    pull_tile3(s_pop, tid, iw, j, c, f, g);
+    mrt_collide(f, g, c);             // (consumes every loaded value: the reads have completed ...
+  }
+  row_publish(rb, ty, 2, ex2 ? f[0] : 0.0);   //  ... before "pulled" is published)
   row_wait(rb, ty, 2, T3_H);          // the neighbour rows have read this row's level-1 values
   if (ex2) {
     if (hand) store_node_at(Aspare, c.ps, c.px, i, c.ny, f, g);
@@ -576,7 +581,7 @@ constexpr int TP_IMG_DOUBLES = 14 * TP_PLANE;
 constexpr int TP_IMG_BYTES = TP_IMG_DOUBLES * (int)sizeof(double);   // 72,576 = 567 x 128
 constexpr int TP_STAGES = 3, TP_GROUPS = 2;
 constexpr int TP_THREADS = TP_GROUPS * T3_THREADS;
-constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 64 + TP_GROUPS * 2 * T3_H * 8;   // + the stage and the row mbarriers
+constexpr int TP_SMEM = TP_STAGES * TP_IMG_BYTES + 80 + TP_GROUPS * 2 * T3_H * 8;   // + the stage and the row mbarriers
 
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, void* bar) {
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
@@ -659,18 +664,24 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     const int st = m % TP_STAGES;
     const int i0 = (tile % ntx) * T3_X - 4, j0 = (tile / ntx) * T3_Y - 3;
     double* img = imgs + st * TP_IMG_DOUBLES;
-    mbar_expect_tx(full + st, TP_IMG_BYTES);
-    tma_load_3d(img, &tm_pair, 2 * i0, j0, 0, full + st);
-    tma_load_3d(img + TP_PAIR_DOUBLES, &tm_diag, i0, j0, 0, full + st);
+    // One "full" barrier per stage AND consuming group (tile m belongs to group m % 2): with the
+    // row-wise hand-over a warp can be more than three tiles of its group ahead of the slowest one,
+    // i.e. at the stage's NEXT BUT ONE use -- on a barrier shared by both groups that use has the
+    // parity of the one still in progress and the wait would pass on the old image (seen as one
+    // corrupted run in 150-250).  Per group, consecutive completions are six tiles apart.
+    unsigned long long* bar = full + st + TP_STAGES * (m % TP_GROUPS);
+    mbar_expect_tx(bar, TP_IMG_BYTES);
+    tma_load_3d(img, &tm_pair, 2 * i0, j0, 0, bar);
+    tma_load_3d(img + TP_PAIR_DOUBLES, &tm_diag, i0, j0, 0, bar);
   };
-  unsigned long long* const empty = full + 4;                   // ROWSYNC: image handed back (16 warps)
-  unsigned long long* const rb = full + 8 + grp * (2 * T3_H);   // the group's row barriers [row][2]
+  unsigned long long* const empty = full + 6;                   // ROWSYNC: image handed back (16 warps)
+  unsigned long long* const rb = full + 10 + grp * (2 * T3_H);  // the group's row barriers [row][2]
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int st = 0; st < TP_STAGES; ++st) mbar_init(full + st, 1);
+    for (int k = 0; k < TP_STAGES * TP_GROUPS; ++k) mbar_init(full + k, 1);
     if (ROWSYNC) {
       for (int st = 0; st < TP_STAGES; ++st) mbar_init(empty + st, T3_THREADS / 32);
-      for (int k = 0; k < TP_GROUPS * 2 * T3_H; ++k) mbar_init(full + 8 + k, 1);
+      for (int k = 0; k < TP_GROUPS * 2 * T3_H; ++k) mbar_init(full + 10 + k, 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -690,20 +701,28 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2;
     const bool ex3 = ex2 && tx >= 2 && tx <= T3_W - 3 && ty >= 2 && ty <= T3_H - 3;
     double f[9], g[5];
-    mbar_wait(full + st, (unsigned)(m / TP_STAGES) & 1u);
+    mbar_wait(full + st + TP_STAGES * grp, (unsigned)(m / (TP_STAGES * TP_GROUPS)) & 1u);
     if (ROWSYNC) {
+      // "pulled" is published AFTER the collision: the collision consumes every loaded value, so
+      // the shared-memory reads have completed by then -- an arrival right behind the loads could
+      // overtake them in the memory pipeline, and the neighbour's write-back with it (seen once as
+      // a 1e-9 mass defect in 300 steps of config 1)
       // level 1: t -> t+1
-      if (ex1) pull_img(img, s, i, j, c, f, g);
-      row_publish(rb, ty, 1);
-      if (ex1) mrt_collide(f, g, c);
+      if (ex1) {
+        pull_img(img, s, i, j, c, f, g);
+        mrt_collide(f, g, c);
+      }
+      row_publish(rb, ty, 1, ex1 ? f[0] : 0.0);
       row_wait(rb, ty, 1, T3_H);                                 // the neighbour rows have pulled
       if (ex1) put_img(img, s, f, g);
       row_publish(rb, ty, 2);
       // level 2: t+1 -> t+2
       row_wait(rb, ty, 2, T3_H);                                 // ... have written level 1
-      if (ex2) pull_img(img, s, i, j, c, f, g);
-      row_publish(rb, ty, 3);
-      if (ex2) mrt_collide(f, g, c);
+      if (ex2) {
+        pull_img(img, s, i, j, c, f, g);
+        mrt_collide(f, g, c);
+      }
+      row_publish(rb, ty, 3, ex2 ? f[0] : 0.0);
       row_wait(rb, ty, 3, T3_H);
       if (ex2) put_img(img, s, f, g);
       row_publish(rb, ty, 4);
@@ -730,12 +749,18 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
       // level 3: t+2 -> t+3
       if (ex3) pull_img(img, s, i, j, c, f, g);
     }
-    // ... to global memory; the image is free once everybody has pulled
+    // ... to global memory; the image is free once everybody has pulled -- and collided: as above,
+    // the hand-back must not overtake the loads
+    if (ex3) mrt_collide(f, g, c);
+    // every thread orders its own generic-proxy accesses to the image (the in-place writes of
+    // levels 1 and 2, the pulls) before the copy engine's writes that follow the hand-back
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (ROWSYNC) {
       // the warps of a group may be tiles apart here, so the image is handed back through an
       // mbarrier of its own (one arrival per warp; a named barrier would count a fast warp twice)
       __syncwarp();
-      if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + st)) : "memory");
+      if ((tid & 31) == 0)
+        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + st)), "d"(ex3 ? f[0] : 0.0) : "memory");
       if (tid < 32) {
         mbar_wait(empty + st, (unsigned)(m / TP_STAGES) & 1u);
         if (tid == 0) {
@@ -754,10 +779,7 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     } else {
       group_arrive(3 + grp);
     }
-    if (ex3) {
-      mrt_collide(f, g, c);
-      store_node(B, c, i, j, f, g);
-    }
+    if (ex3) store_node(B, c, i, j, f, g);
   }
 }
 
