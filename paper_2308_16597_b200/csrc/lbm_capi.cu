@@ -419,12 +419,6 @@ static int create_impl(int is_slab, int nx, int ny, int yoff, int NY, int own0, 
   {
     const char* eb = getenv("LBM_BAND");
     h->band_on = eb ? std::min(std::max(atoi(eb), 0), 2) : 1;   // 0 off, 1 where it pays, 2 every band
-    if (cudaStreamCreateWithFlags(&h->band_own, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaEventCreateWithFlags(&h->ev_bs, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&h->ev_bp, cudaEventDisableTiming) != cudaSuccess) {
-      cudaGetLastError();
-      h->band_own = nullptr;
-    }
     if (cudaEventCreateWithFlags(&h->ev_p2, cudaEventDisableTiming) != cudaSuccess) {
       cudaGetLastError();
       h->band_on = 0;
@@ -732,8 +726,6 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
   // half period, so the band kernel needs no second source and the one-step kernel never computes
   // a band row: it reads row Q-1 in place in the first step of a half period and from the spare
   // row, where the band kernel's top tiles put it, in the other two
-  static const int xovl = getenv("LBM_X_BANDOVL") ? atoi(getenv("LBM_X_BANDOVL")) : 0;
-  const bool bovl = banded && h->band3 && fork && xovl > 0 && h->band_own != nullptr && h->np > 0;
   const int half = h->band3 ? 3 : 2;
   double* band_src = phase < half ? X : Y;
   double* band_dst = phase < half ? Y : X;
@@ -751,18 +743,7 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     if (fork) cudaEventRecord(h->ev_bb, S1);
   }
   if (banded) {
-    if (bovl) {
-      // experiment (LBM_X_BANDOVL): the band's part on a stream of its own, free to run beside
-      // this step's one-step kernel; the next step's work on S0 follows it
-      cudaEventRecord(h->ev_bs, S0);
-      cudaStreamWaitEvent(h->band_own, h->ev_bs, 0);
-      cudaStream_t keep = h->stream;
-      h->stream = h->band_own;
-      { Timed tm(h, K_STREAM_COLLIDE_3STEP, h->band_own); launch_stream_collide_band3(h, band_src, band_dst, 3, phase % 3); }
-      h->stream = keep;
-      cudaEventRecord(h->ev_bp, h->band_own);
-      if (xovl >= 2) cudaStreamWaitEvent(S1, h->ev_bp, 0);
-    } else if (h->band3) {
+    if (h->band3) {
       Timed tm(h, K_STREAM_COLLIDE_3STEP, S0);
       launch_stream_collide_band3(h, band_src, band_dst, 3, phase % 3);
     } else {
@@ -772,7 +753,7 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
     // the particle chain holds register space the band kernel's large CTAs need (measured: the band
     // part takes 115 us beside the bounce-back kernel alone, 190 us beside the chain): the chain
     // starts after the band's part and still has the whole one-step kernel to hide under
-    if (fork && !bovl) {
+    if (fork) {
       cudaEventRecord(h->ev_p2, S0);
       cudaStreamWaitEvent(S1, h->ev_p2, 0);
     }
@@ -785,7 +766,6 @@ static void enqueue_step(lbm* h, int phase, bool plan = true) {
   }
   if (h->np > 0) {
     if (fork) cudaEventRecord(h->ev_sc, S0);
-    if (bovl) cudaStreamWaitEvent(S0, h->ev_bp, 0);
     { Timed tm(h, K_MOVE, S1); launch_move(h, S1, pdl); }
     note_chain_node(h, S1);
     { Timed tm(h, K_COVER, S1); launch_cover(h, sp ^ 1, S1, pdl); }

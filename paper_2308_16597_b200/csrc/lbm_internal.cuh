@@ -161,8 +161,6 @@ struct lbm {
   int want3;                 // this call may use periods of six steps (band under the suspension, band_steps == 3)
   int band3;                 // the unit being enqueued is such a period: the band advances three steps per pass
   cudaEvent_t ev_p2;         // the band kernel's part of a step has been issued (the particle chain follows it)
-  cudaStream_t band_own;     // experiment: the band's parts on a stream of their own
-  cudaEvent_t ev_bs, ev_bp;
   cudaEvent_t ev_plan;       // the band plan of a period has been issued (the caller's stream follows it)
   int primed;                // 0: A holds pre-collision f(x,0); 1: A holds post-collision f+(x,t)
   long long steps_done;
