@@ -291,13 +291,12 @@ __device__ __forceinline__ void mbar_arrive(void* bar) {
 // complete [row][0], phases 2 and 4 [row][1], so that two completions of one barrier are always
 // separated by the neighbours' observation of the first (a row cannot publish phase p + 2 before
 // both neighbours have published p + 1, i.e. have seen p) and the parity wait stays unambiguous
-// dep: a value the arrival must come after (an operand the instruction does not use: a collided
-// population, which depends on every value the thread pulled, so the warp's shared-memory reads
-// have completed when the arrival issues)
-__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase, double dep = 0.0) {
+// (mbarrier.arrive is a release at CTA scope: the warp's shared-memory reads and writes before it --
+// __syncwarp orders the other lanes' -- are performed before a waiter that acquires it goes on)
+__device__ __forceinline__ void row_publish(unsigned long long* rb, int row, int phase) {
   __syncwarp();
   if ((threadIdx.x & 31) == 0)
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))), "d"(dep) : "memory");
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(rb + 2 * row + ((phase - 1) & 1))) : "memory");
 }
 __device__ __forceinline__ void row_wait(unsigned long long* rb, int row, int phase, int rows) {
   const unsigned parity = (unsigned)((phase - 1) >> 1) & 1u;   // two completions per barrier and tile
@@ -528,11 +527,9 @@ k_stream_collide_3step(const double* __restrict__ A, double* __restrict__ B, dou
   // level 2: t+1 -> t+2 on the tile dilated by one node, written back in place
   const bool ex2 = ex1 && tx >= 1 && tx <= T3_W - 2 && ty >= 1 && ty <= T3_H - 2 &&
                    (!c.periodic_x || (i >= -1 && i <= c.nx)) && in2;
-  if (ex2) {
-    pull_tile3(s_pop, tid, iw, j, c, f, g);
-    mrt_collide(f, g, c);             // (consumes every loaded value: the reads have completed ...
-  }
-  row_publish(rb, ty, 2, ex2 ? f[0] : 0.0);   //  ... before "pulled" is published)
+  if (ex2) pull_tile3(s_pop, tid, iw, j, c, f, g);
+  row_publish(rb, ty, 2);
+  if (ex2) mrt_collide(f, g, c);
   row_wait(rb, ty, 2, T3_H);          // the neighbour rows have read this row's level-1 values
   if (ex2) {
     if (hand) store_node_at(Aspare, c.ps, c.px, i, c.ny, f, g);
@@ -703,26 +700,18 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     double f[9], g[5];
     mbar_wait(full + st + TP_STAGES * grp, (unsigned)(m / (TP_STAGES * TP_GROUPS)) & 1u);
     if (ROWSYNC) {
-      // "pulled" is published AFTER the collision: the collision consumes every loaded value, so
-      // the shared-memory reads have completed by then -- an arrival right behind the loads could
-      // overtake them in the memory pipeline, and the neighbour's write-back with it (seen once as
-      // a 1e-9 mass defect in 300 steps of config 1)
       // level 1: t -> t+1
-      if (ex1) {
-        pull_img(img, s, i, j, c, f, g);
-        mrt_collide(f, g, c);
-      }
-      row_publish(rb, ty, 1, ex1 ? f[0] : 0.0);
+      if (ex1) pull_img(img, s, i, j, c, f, g);
+      row_publish(rb, ty, 1);                              // (release: the pulls are ordered before it)
+      if (ex1) mrt_collide(f, g, c);
       row_wait(rb, ty, 1, T3_H);                                 // the neighbour rows have pulled
       if (ex1) put_img(img, s, f, g);
       row_publish(rb, ty, 2);
       // level 2: t+1 -> t+2
       row_wait(rb, ty, 2, T3_H);                                 // ... have written level 1
-      if (ex2) {
-        pull_img(img, s, i, j, c, f, g);
-        mrt_collide(f, g, c);
-      }
-      row_publish(rb, ty, 3, ex2 ? f[0] : 0.0);
+      if (ex2) pull_img(img, s, i, j, c, f, g);
+      row_publish(rb, ty, 3);
+      if (ex2) mrt_collide(f, g, c);
       row_wait(rb, ty, 3, T3_H);
       if (ex2) put_img(img, s, f, g);
       row_publish(rb, ty, 4);
@@ -749,18 +738,12 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
       // level 3: t+2 -> t+3
       if (ex3) pull_img(img, s, i, j, c, f, g);
     }
-    // ... to global memory; the image is free once everybody has pulled -- and collided: as above,
-    // the hand-back must not overtake the loads
-    if (ex3) mrt_collide(f, g, c);
-    // every thread orders its own generic-proxy accesses to the image (the in-place writes of
-    // levels 1 and 2, the pulls) before the copy engine's writes that follow the hand-back
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    // ... to global memory; the image is free once everybody has pulled
     if (ROWSYNC) {
       // the warps of a group may be tiles apart here, so the image is handed back through an
       // mbarrier of its own (one arrival per warp; a named barrier would count a fast warp twice)
       __syncwarp();
-      if ((tid & 31) == 0)
-        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + st)), "d"(ex3 ? f[0] : 0.0) : "memory");
+      if ((tid & 31) == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(empty + st)) : "memory");
       if (tid < 32) {
         mbar_wait(empty + st, (unsigned)(m / TP_STAGES) & 1u);
         if (tid == 0) {
@@ -779,7 +762,10 @@ k_stream_collide_3step_tma(const __grid_constant__ CUtensorMap tm_pair, const __
     } else {
       group_arrive(3 + grp);
     }
-    if (ex3) store_node(B, c, i, j, f, g);
+    if (ex3) {
+      mrt_collide(f, g, c);
+      store_node(B, c, i, j, f, g);
+    }
   }
 }
 
